@@ -1,0 +1,19 @@
+"""paper_2605_30842_b200 — B200-native paged decode attention (CoMem's decode hot path).
+
+The product is the C-ABI library built from ``csrc/`` (``include/comem_decode_attn.h``);
+this package is its thin Python binding plus the seeded input generators
+(``workloads``).  Importing the package does not load the library; the first
+call does, and raises if it has not been built (no CPU fallback exists).
+"""
+from .binding import (  # noqa: F401
+    ComemError,
+    comem_decode_attn,
+    comem_decode_attn_async,
+    comem_decode_attn_host,
+    comem_decode_attn_workspace_bytes,
+    comem_kv_append_async,
+    comem_status_string,
+    comem_version,
+    library_path,
+    load_library,
+)
