@@ -1,0 +1,165 @@
+/*
+ * comem_decode_attn.h — C ABI of libcomem_decode.so (B200 / sm_100a only).
+ *
+ * The one operation: single-query ("decode step") grouped-query attention over a
+ * paged bf16 KV cache addressed through a block table, computed as split-KV
+ * partial softmax + log-sum-exp combine.
+ *
+ * Where the operation is defined (P:Lnn = /root/reference/PAPER.md line nn):
+ *   P:L49  §2.2  Q in R^{l x h_q x d_h}, K, V in R^{l x h_kv x d_h}; the KV cache
+ *                [K_1; ...; K_l], [V_1; ...; V_l] kept per KV head.
+ *   P:L51  fn.1  KV heads are distinct from attention heads because of GQA.
+ *   P:L61  §2.2  decode step t appends one (K, V) row to the cache
+ *                (comem_kv_append_async) and then reads the WHOLE cache for the
+ *                one new query (comem_decode_attn*); it is memory-bound.
+ *   P:L25        the cache is paged (PagedAttention is named, no layout given).
+ *   P:L184 eq.5  t = L*S/W: the roofline this library is measured against.
+ * The softmax-attention formula itself is not written in the paper; the
+ * readings this ABI fixes are listed in DESIGN.md ("Readings", R1..R13):
+ *   out[b,h,:] = sum_t softmax_t(softmax_scale * q[b,h,:].k_t[kvh,:]) * v_t[kvh,:]
+ *   over t in [0, seq_lens[b]), kvh = h / (num_q_heads / num_kv_heads),
+ *   (k_t, v_t) = row (page block_table[b][t / page_size], slot t % page_size).
+ *
+ * Conventions for every entry point
+ *   - "device" pointers are CUDA device memory of the CURRENT device; "host"
+ *     pointers are ordinary (preferably pinned) host memory.
+ *   - The caller owns every buffer.  The library never allocates device memory,
+ *     never frees and never keeps a pointer after the call returns (it caches
+ *     only TMA descriptors keyed by pool address and shape).
+ *   - Tensor base pointers must be 16-byte aligned (k_pages / v_pages: 128-byte).
+ *   - Return value: a COMEM_* status; no exceptions or aborts cross the ABI.
+ *   - Device-side DATA (seq_lens, block_table contents) is not validated:
+ *     seq_lens[b] > max_pages_per_seq * page_size, or a page id outside
+ *     [0, num_pages) in a USED table entry, is undefined behaviour.  Table
+ *     entries j >= ceil(seq_lens[b] / page_size), slots past seq_lens[b] in the
+ *     last page, and pages no sequence uses are never read semantically: the
+ *     result does not depend on their contents (NaN / Inf / wild ids included).
+ *   - Results are deterministic: the same logical inputs give bit-identical
+ *     output regardless of physical page placement, stream, or concurrent work.
+ */
+#ifndef COMEM_DECODE_ATTN_H
+#define COMEM_DECODE_ATTN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    COMEM_OK = 0,
+    COMEM_ERR_INVALID_ARG = 1, /* null required pointer, batch <= 0, Hq % Hkv != 0, bad scale, misaligned */
+    COMEM_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}; page_size not in {16,32}; G not in {1,2,4,8};
+                                  batch > COMEM_MAX_BATCH; device is not sm_100 */
+    COMEM_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than comem_decode_attn_workspace_bytes() */
+    COMEM_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+};
+
+#define COMEM_MAX_BATCH 4096
+
+/*
+ * comem_decode_attn_async — enqueue one decode-attention step on `cuda_stream`.
+ *
+ * Enqueue-only: no host synchronisation, no device->host copy, no allocation;
+ * safe inside CUDA-graph capture.  Launches 2 kernels (split-KV, combine).
+ * Returns launch-time errors only.
+ *
+ *   q            device, bf16 [batch][num_q_heads][head_dim], contiguous
+ *   k_pages      device, bf16 [num_pages][page_size][num_kv_heads][head_dim]
+ *   v_pages      device, same shape, separate allocation
+ *   block_table  device, int32 [batch][max_pages_per_seq]; entry j = physical page
+ *                of logical page j of that sequence
+ *   seq_lens     device, int32 [batch]; tokens valid in each sequence (0 allowed:
+ *                that row of out is +0.0 and its lse is -inf)
+ *   softmax_scale  fp32, finite, >= 0; applied to the fp32 dot product
+ *   out          device, bf16 [batch][num_q_heads][head_dim]; fp32 accumulate,
+ *                round-to-nearest-even
+ *   lse_out      device, fp32 [batch][num_q_heads] natural-log log-sum-exp of the
+ *                scaled logits, or NULL
+ *   workspace    device scratch of >= comem_decode_attn_workspace_bytes(...) bytes,
+ *                256-byte aligned.  Holds split partials; contents need no
+ *                initialisation and are garbage afterwards.  Calls that may run
+ *                concurrently (different streams) need DIFFERENT workspaces.
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream)
+ */
+int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
+                            const int32_t *block_table, const int32_t *seq_lens,
+                            int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                            float softmax_scale, void *out, int batch, int max_pages_per_seq,
+                            int64_t num_pages, float *lse_out, void *workspace,
+                            size_t workspace_bytes, void *cuda_stream);
+
+/* Same on the legacy default stream, then cudaStreamSynchronize: also returns
+ * execution errors (COMEM_ERR_CUDA). */
+int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,
+                      const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                      int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                      void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                      float *lse_out, void *workspace, size_t workspace_bytes);
+
+/* Scratch bytes needed by the calls above and below for this problem shape.
+ * Pure host arithmetic (no CUDA call); depends only on the arguments. */
+size_t comem_decode_attn_workspace_bytes(int batch, int num_q_heads, int num_kv_heads,
+                                         int head_dim, int page_size, int max_pages_per_seq);
+
+/*
+ * comem_kv_append_async — the step before attention (P:L61,
+ * K_cache^(t) = [K_cache^(t-1); K^(t)]): for every sequence b write new_k[b], new_v[b]
+ * (device, bf16 [batch][num_kv_heads][head_dim]) at logical position seq_lens[b]
+ * (page block_table[b][seq_lens[b] / page_size], which the caller must already have
+ * placed in the table), then seq_lens[b] += 1 on the device.  Enqueue-only, 1 kernel.
+ */
+int comem_kv_append_async(void *k_pages, void *v_pages, const int32_t *block_table,
+                          int32_t *seq_lens, const void *new_k, const void *new_v,
+                          int num_kv_heads, int head_dim, int page_size, int batch,
+                          int max_pages_per_seq, void *cuda_stream);
+
+/*
+ * comem_decode_step_host — one whole decode step driven from HOST buffers: the
+ * end-to-end call bench.py's "e2e" times.  The KV cache is the model's resident
+ * state and stays in HBM (decode waits "for the KV cache to arrive from
+ * HBM"); what a step brings from the host is the new token's q, k, v rows and
+ * what it returns is the attention output.
+ *
+ *   q_host                  host, bf16 [batch][num_q_heads][head_dim]
+ *   new_k_host, new_v_host  host, bf16 [batch][num_kv_heads][head_dim], or both
+ *                           NULL to skip the append
+ *   out_host                host, bf16 [batch][num_q_heads][head_dim]
+ *   lse_host                host, fp32 [batch][num_q_heads], or NULL
+ *   k_pages, v_pages, block_table, seq_lens, workspace: device, as above
+ *
+ * Sequence on `cuda_stream`: H2D(q, new_k, new_v) -> kv_append -> decode_attn ->
+ * D2H(out[, lse]) -> cudaStreamSynchronize.  Returns execution errors too.
+ */
+int comem_decode_step_host(const void *q_host, const void *new_k_host, const void *new_v_host,
+                           void *k_pages, void *v_pages, const int32_t *block_table,
+                           int32_t *seq_lens, int num_q_heads, int num_kv_heads, int head_dim,
+                           int page_size, float softmax_scale, void *out_host, int batch,
+                           int max_pages_per_seq, int64_t num_pages, float *lse_host,
+                           void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * Split-KV schedule introspection (host arithmetic mirroring the device
+ * scheduler; used by tests and DESIGN.md).  Given host copies of seq_lens,
+ * writes for each CTA i in [0, *num_ctas) its half-open range of 16-token tiles
+ * [tile_begin[i], tile_begin[i+1]) in the linearised (b, kv_head, tile) order.
+ * tile_begin must hold grid_ctas + 1 entries.  Returns COMEM_OK.
+ */
+int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_heads, int grid_ctas,
+                        int64_t *tile_begin, int *num_ctas);
+
+/* Persistent-grid size (CTAs) the split kernel uses on the current device, or a
+ * negative COMEM_ERR_* value.  comem_set_grid_ctas(n > 0) overrides it for later
+ * calls from this process (n <= 0 restores the default); used to give each of two
+ * concurrently running batches a share of the SMs. */
+int comem_grid_ctas(int head_dim);
+int comem_set_grid_ctas(int n);
+
+const char *comem_status_string(int status);
+int comem_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COMEM_DECODE_ATTN_H */

@@ -6,12 +6,21 @@ this package is its thin Python binding plus the seeded input generators
 call does, and raises if it has not been built (no CPU fallback exists).
 """
 from .binding import (  # noqa: F401
+    COMEM_ERR_CUDA,
+    COMEM_ERR_INVALID_ARG,
+    COMEM_ERR_UNSUPPORTED,
+    COMEM_ERR_WORKSPACE,
+    COMEM_OK,
     ComemError,
+    alloc_workspace,
     comem_decode_attn,
     comem_decode_attn_async,
-    comem_decode_attn_host,
     comem_decode_attn_workspace_bytes,
+    comem_decode_step_host,
+    comem_grid_ctas,
     comem_kv_append_async,
+    comem_schedule_host,
+    comem_set_grid_ctas,
     comem_status_string,
     comem_version,
     library_path,

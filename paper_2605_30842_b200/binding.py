@@ -1,8 +1,207 @@
-# placeholder, replaced below
+"""Thin ctypes binding over libcomem_decode.so — same names as include/comem_decode_attn.h.
+
+Argument marshalling only: shapes are read off the tensors, pointers are
+``tensor.data_ptr()``, the stream is torch's current CUDA stream unless given.
+Every step of the path runs in the library's kernels; there is no fallback —
+if the library is missing or the device is not sm_100 the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libcomem_decode.so")
+_lib = None
+
+COMEM_OK = 0
+COMEM_ERR_INVALID_ARG = 1
+COMEM_ERR_UNSUPPORTED = 2
+COMEM_ERR_WORKSPACE = 3
+COMEM_ERR_CUDA = 4
+
+
 class ComemError(RuntimeError):
-    pass
-def _todo(*a, **k):
-    raise ComemError("not built yet")
-comem_decode_attn = comem_decode_attn_async = comem_decode_attn_host = _todo
-comem_decode_attn_workspace_bytes = comem_kv_append_async = comem_status_string = _todo
-comem_version = library_path = load_library = _todo
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {comem_status_string(status)} (status {status})")
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen the C-ABI library (built in-tree by ``python -m paper_2605_30842_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2605_30842_b200.build` "
+            "(or __graft_entry__.build()). There is no CPU or PyTorch fallback for this path.")
+    lib = ctypes.CDLL(_LIB_PATH)
+    c = ctypes
+    vp, i32, i64, f32, sz = c.c_void_p, c.c_int, c.c_int64, c.c_float, c.c_size_t
+    lib.comem_decode_attn_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
+                                            i64, vp, vp, sz, vp]
+    lib.comem_decode_attn_async.restype = i32
+    lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
+                                      vp, vp, sz]
+    lib.comem_decode_attn.restype = i32
+    lib.comem_decode_attn_workspace_bytes.argtypes = [i32] * 6
+    lib.comem_decode_attn_workspace_bytes.restype = sz
+    lib.comem_kv_append_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
+    lib.comem_kv_append_async.restype = i32
+    lib.comem_decode_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
+                                           i32, i64, vp, vp, sz, vp]
+    lib.comem_decode_step_host.restype = i32
+    lib.comem_schedule_host.argtypes = [vp, i32, i32, i32, vp, vp]
+    lib.comem_schedule_host.restype = i32
+    lib.comem_grid_ctas.argtypes = [i32]
+    lib.comem_grid_ctas.restype = i32
+    lib.comem_set_grid_ctas.argtypes = [i32]
+    lib.comem_set_grid_ctas.restype = i32
+    lib.comem_status_string.argtypes = [i32]
+    lib.comem_status_string.restype = c.c_char_p
+    lib.comem_version.restype = i32
+    _lib = lib
+    return lib
+
+
+def comem_status_string(status: int) -> str:
+    return load_library().comem_status_string(int(status)).decode()
+
+
+def comem_version() -> int:
+    return int(load_library().comem_version())
+
+
+def comem_grid_ctas(head_dim: int) -> int:
+    g = int(load_library().comem_grid_ctas(int(head_dim)))
+    if g < 0:
+        raise ComemError(-g, "comem_grid_ctas")
+    return g
+
+
+def comem_set_grid_ctas(n: int) -> None:
+    load_library().comem_set_grid_ctas(int(n))
+
+
+def comem_schedule_host(seq_lens, num_kv_heads: int, grid_ctas: int):
+    """Host mirror of the device split-KV schedule: list of CTA tile-range boundaries."""
+    import numpy as np
+
+    sl = np.ascontiguousarray(np.asarray(seq_lens, dtype=np.int32))
+    begins = np.zeros(grid_ctas + 1, dtype=np.int64)
+    nc = ctypes.c_int(0)
+    st = load_library().comem_schedule_host(sl.ctypes.data, len(sl), int(num_kv_heads), int(grid_ctas),
+                                            begins.ctypes.data, ctypes.byref(nc))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_schedule_host")
+    return begins[:nc.value + 1].tolist()
+
+
+def comem_decode_attn_workspace_bytes(batch: int, num_q_heads: int, num_kv_heads: int, head_dim: int,
+                                      page_size: int, max_pages_per_seq: int) -> int:
+    return int(load_library().comem_decode_attn_workspace_bytes(
+        int(batch), int(num_q_heads), int(num_kv_heads), int(head_dim), int(page_size),
+        int(max_pages_per_seq)))
+
+
+def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.Tensor) -> torch.Tensor:
+    """torch.empty of the size the library asks for (device memory is torch's job)."""
+    n = comem_decode_attn_workspace_bytes(q.shape[0], q.shape[1], k_pages.shape[2], q.shape[2],
+                                          k_pages.shape[1], block_table.shape[1])
+    return torch.empty(n, dtype=torch.uint8, device=q.device)
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    if isinstance(stream, torch.cuda.Stream):
+        return ctypes.c_void_p(stream.cuda_stream)
+    return ctypes.c_void_p(int(stream))
+
+
+def _check_inputs(q, k_pages, v_pages, block_table, seq_lens):
+    assert q.dtype == torch.bfloat16 and k_pages.dtype == torch.bfloat16 and v_pages.dtype == torch.bfloat16
+    assert block_table.dtype == torch.int32 and seq_lens.dtype == torch.int32
+    assert q.is_contiguous() and k_pages.is_contiguous() and v_pages.is_contiguous()
+    assert block_table.is_contiguous() and seq_lens.is_contiguous()
+    assert q.dim() == 3 and k_pages.dim() == 4 and k_pages.shape == v_pages.shape
+    assert block_table.dim() == 2 and block_table.shape[0] == q.shape[0] == seq_lens.shape[0]
+    assert k_pages.shape[3] == q.shape[2]
+
+
+def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
+                            workspace, lse_out=None, stream=None) -> None:
+    """Enqueue one decode-attention step (2 kernel launches) on ``stream``; returns at once."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_async")
+
+
+def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out=None,
+                      workspace=None, lse_out=None):
+    """Synchronous form (legacy default stream + cudaStreamSynchronize).  Returns ``out``."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    if out is None:
+        out = torch.empty_like(q)
+    if workspace is None:
+        workspace = alloc_workspace(q, k_pages, block_table)
+    torch.cuda.current_stream().synchronize()  # inputs were produced on torch's stream
+    st = load_library().comem_decode_attn(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size())
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn")
+    return out
+
+
+def comem_kv_append_async(k_pages, v_pages, block_table, seq_lens, new_k, new_v, stream=None) -> None:
+    """Enqueue the KV append of one new (k, v) row per sequence; seq_lens += 1 on device."""
+    assert new_k.dtype == torch.bfloat16 and new_v.dtype == torch.bfloat16
+    assert new_k.is_contiguous() and new_v.is_contiguous() and new_k.shape == new_v.shape
+    assert new_k.shape == (block_table.shape[0], k_pages.shape[2], k_pages.shape[3])
+    st = load_library().comem_kv_append_async(
+        _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), _ptr(new_k), _ptr(new_v),
+        k_pages.shape[2], k_pages.shape[3], k_pages.shape[1], block_table.shape[0],
+        block_table.shape[1], _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_kv_append_async")
+
+
+def comem_decode_step_host(q_host, new_k_host, new_v_host, k_pages, v_pages, block_table, seq_lens,
+                           softmax_scale: float, out_host, workspace, lse_host=None, stream=None) -> None:
+    """One whole decode step from HOST q / new k / new v rows to a HOST output (synchronous)."""
+    assert q_host.device.type == "cpu" and out_host.device.type == "cpu"
+    assert q_host.dtype == torch.bfloat16 and out_host.dtype == torch.bfloat16
+    assert q_host.is_contiguous() and out_host.is_contiguous() and out_host.shape == q_host.shape
+    st = load_library().comem_decode_step_host(
+        _ptr(q_host), _ptr(new_k_host), _ptr(new_v_host), _ptr(k_pages), _ptr(v_pages),
+        _ptr(block_table), _ptr(seq_lens), q_host.shape[1], k_pages.shape[2], q_host.shape[2],
+        k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out_host), q_host.shape[0],
+        block_table.shape[1], k_pages.shape[0], _ptr(lse_host), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_step_host")
+
+
+# kept for symmetry with the header's name list
+comem_decode_attn_host = comem_decode_step_host

@@ -1,0 +1,355 @@
+// api.cu — the C ABI of libcomem_decode.so (include/comem_decode_attn.h): argument
+// validation, TMA descriptor cache, workspace carving, launches.  No torch types, no device
+// allocation, no CPU fallback: without a sm_100 device every compute entry point returns
+// COMEM_ERR_CUDA / COMEM_ERR_UNSUPPORTED.
+#include "../../include/comem_decode_attn.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "decode_params.cuh"
+#include "schedule.cuh"
+
+namespace comem {
+namespace {
+
+constexpr int kMaxGridCtas = 1024;  // workspace is sized for this many persistent CTAs
+constexpr float kLog2e = 1.4426950408889634f;
+static_assert(kMaxBatch == COMEM_MAX_BATCH, "header and scheduler disagree on the batch limit");
+
+std::atomic<int> g_grid_override{0};
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct WorkspaceLayout {
+    size_t partials, q, new_k, new_v, out, lse, total;
+};
+
+WorkspaceLayout workspace_layout(int batch, int hq, int hkv, int d)
+{
+    WorkspaceLayout w;
+    size_t off = 0;
+    w.partials = off;
+    off = align_up(off + (size_t)2 * kMaxGridCtas * partial_stride_floats(d) * sizeof(float), 256);
+    w.q = off;
+    off = align_up(off + (size_t)batch * hq * d * 2, 256);
+    w.new_k = off;
+    off = align_up(off + (size_t)batch * hkv * d * 2, 256);
+    w.new_v = off;
+    off = align_up(off + (size_t)batch * hkv * d * 2, 256);
+    w.out = off;
+    off = align_up(off + (size_t)batch * hq * d * 2, 256);
+    w.lse = off;
+    off = align_up(off + (size_t)batch * hq * 4, 256);
+    w.total = off;
+    return w;
+}
+
+int check_shape(int hq, int hkv, int d, int ps, int batch, int max_pages, int64_t num_pages)
+{
+    if (batch <= 0 || hq <= 0 || hkv <= 0 || max_pages <= 0 || num_pages <= 0) return COMEM_ERR_INVALID_ARG;
+    if (hq % hkv != 0) return COMEM_ERR_INVALID_ARG;
+    const int g = hq / hkv;
+    if (d != 64 && d != 128) return COMEM_ERR_UNSUPPORTED;
+    if (ps != 16 && ps != 32) return COMEM_ERR_UNSUPPORTED;
+    if (g != 1 && g != 2 && g != 4 && g != 8) return COMEM_ERR_UNSUPPORTED;
+    if (batch > COMEM_MAX_BATCH) return COMEM_ERR_UNSUPPORTED;
+    // TMA row coordinate (page * page_size) and the linear tile count must fit in int32
+    if (num_pages * ps >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
+    if ((int64_t)batch * max_pages * (ps / kTileTokens) * hkv >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
+    return COMEM_OK;
+}
+
+// ---- device capability (cached per device) ---------------------------------------------------
+int check_device()
+{
+    static std::mutex mu;
+    static int cached_dev = -1, cached_status = COMEM_ERR_CUDA;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev == cached_dev) return cached_status;
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    cached_dev = dev;
+    cached_status = (major == 10) ? COMEM_OK : COMEM_ERR_UNSUPPORTED;
+    return cached_status;
+}
+
+// ---- TMA descriptors --------------------------------------------------------------------------
+// The pool [P][ps][Hkv][D] is described to the TMA unit as a 4-D tensor
+//   dim0 = 64 elements of d (128 B, the swizzle span)     stride 2 B
+//   dim1 = P * ps token rows                               stride Hkv*D*2 B
+//   dim2 = D / 64 halves of the head vector                stride 128 B
+//   dim3 = Hkv                                             stride D*2 B
+// with box {64, 16, D/64, 1}: one load brings a [16 tokens][D] tile of one kv head and lays
+// it in shared memory as D/64 sub-tiles of [16 rows][128 B], 128-byte swizzled, which
+// ldmatrix then reads without bank conflicts.
+using EncodeFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                              const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                              CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                              CUtensorMapFloatOOBfill);
+
+EncodeFn encode_fn()
+{
+    static EncodeFn fn = [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+        }
+        return reinterpret_cast<EncodeFn>(p);
+    }();
+    return fn;
+}
+
+struct MapKey {
+    const void *ptr;
+    int64_t num_pages;
+    int ps, hkv, d;
+    bool operator==(const MapKey &o) const
+    {
+        return ptr == o.ptr && num_pages == o.num_pages && ps == o.ps && hkv == o.hkv && d == o.d;
+    }
+};
+struct MapEntry {
+    MapKey key;
+    CUtensorMap map;
+};
+
+int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out)
+{
+    static std::mutex mu;
+    static std::vector<MapEntry> cache;
+    static size_t next_evict = 0;
+    const MapKey key{pool, num_pages, ps, hkv, d};
+    std::lock_guard<std::mutex> lock(mu);
+    for (const MapEntry &e : cache)
+        if (e.key == key) { *out = e.map; return COMEM_OK; }
+    EncodeFn enc = encode_fn();
+    if (!enc) return COMEM_ERR_CUDA;
+    const cuuint64_t gdim[4] = {64, (cuuint64_t)num_pages * ps, (cuuint64_t)(d / 64), (cuuint64_t)hkv};
+    const cuuint64_t gstride[3] = {(cuuint64_t)hkv * d * 2, 128, (cuuint64_t)d * 2};
+    const cuuint32_t box[4] = {64, (cuuint32_t)kTileTokens, (cuuint32_t)(d / 64), 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    MapEntry e;
+    e.key = key;
+    const CUresult r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(pool), gdim, gstride,
+                           box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           d == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return COMEM_ERR_CUDA;
+    if (cache.size() < 64) cache.push_back(e);
+    else { cache[next_evict] = e; next_evict = (next_evict + 1) % cache.size(); }
+    *out = e.map;
+    return COMEM_OK;
+}
+
+int grid_for(int head_dim, int *grid)
+{
+    static std::mutex mu;
+    static int cached[2] = {0, 0};
+    const int ov = g_grid_override.load();
+    if (ov > 0) { *grid = ov < kMaxGridCtas ? ov : kMaxGridCtas; return COMEM_OK; }
+    std::lock_guard<std::mutex> lock(mu);
+    int &c = cached[head_dim == 128 ? 1 : 0];
+    if (c == 0) {
+        int g = 0;
+        if (split_default_grid(head_dim, &g) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+        c = g < kMaxGridCtas ? g : kMaxGridCtas;
+    }
+    *grid = c;
+    return COMEM_OK;
+}
+
+bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+}  // namespace
+}  // namespace comem
+
+using namespace comem;
+
+extern "C" {
+
+int comem_version(void) { return 100; }
+
+const char *comem_status_string(int status)
+{
+    switch (status) {
+        case COMEM_OK: return "ok";
+        case COMEM_ERR_INVALID_ARG: return "invalid argument";
+        case COMEM_ERR_UNSUPPORTED: return "unsupported shape or device (needs sm_100; head_dim 64/128; page_size 16/32; group 1/2/4/8)";
+        case COMEM_ERR_WORKSPACE: return "workspace missing or too small";
+        case COMEM_ERR_CUDA: return "CUDA error (no device, driver entry point missing, or launch/execution failure)";
+        default: return "unknown status";
+    }
+}
+
+size_t comem_decode_attn_workspace_bytes(int batch, int num_q_heads, int num_kv_heads, int head_dim,
+                                         int page_size, int max_pages_per_seq)
+{
+    (void)page_size;
+    (void)max_pages_per_seq;
+    if (batch <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || head_dim <= 0) return 0;
+    return workspace_layout(batch, num_q_heads, num_kv_heads, head_dim).total;
+}
+
+int comem_set_grid_ctas(int n)
+{
+    g_grid_override.store(n > 0 ? n : 0);
+    return COMEM_OK;
+}
+
+int comem_grid_ctas(int head_dim)
+{
+    if (head_dim != 64 && head_dim != 128) return -COMEM_ERR_UNSUPPORTED;
+    const int st = check_device();
+    if (st != COMEM_OK) return -st;
+    int g = 0;
+    const int r = grid_for(head_dim, &g);
+    return r == COMEM_OK ? g : -r;
+}
+
+int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_heads, int grid_ctas,
+                        int64_t *tile_begin, int *num_ctas)
+{
+    if (!seq_lens_host || !tile_begin || !num_ctas || batch <= 0 || num_kv_heads <= 0 || grid_ctas <= 0)
+        return COMEM_ERR_INVALID_ARG;
+    int64_t tiles = 0;
+    for (int b = 0; b < batch; ++b) tiles += tiles_of(seq_lens_host[b]);
+    const int64_t total = tiles * num_kv_heads;
+    const int nc = total == 0 ? 0 : sched_num_ctas(total, grid_ctas);
+    *num_ctas = nc;
+    for (int i = 0; i <= nc; ++i) tile_begin[i] = nc ? cta_begin(i, total, nc) : 0;
+    return COMEM_OK;
+}
+
+int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
+                            const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                            int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
+                            int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                            void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;
+    int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
+    if (st != COMEM_OK) return st;
+    if (!std::isfinite(softmax_scale) || softmax_scale < 0.f) return COMEM_ERR_INVALID_ARG;
+    if (!aligned(q, 16) || !aligned(out, 16) || !aligned(k_pages, 128) || !aligned(v_pages, 128) ||
+        !aligned(block_table, 4) || !aligned(seq_lens, 4) || (lse_out && !aligned(lse_out, 4)))
+        return COMEM_ERR_INVALID_ARG;
+    const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
+    if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
+    if ((st = check_device()) != COMEM_OK) return st;
+
+    CUtensorMap tm_k, tm_v;
+    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v)) != COMEM_OK) return st;
+
+    DecodeParams p;
+    p.q = static_cast<const __nv_bfloat16 *>(q);
+    p.block_table = block_table;
+    p.seq_lens = seq_lens;
+    p.out = static_cast<__nv_bfloat16 *>(out);
+    p.lse_out = lse_out;
+    p.partials = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.partials);
+    p.batch = batch;
+    p.num_q_heads = num_q_heads;
+    p.num_kv_heads = num_kv_heads;
+    p.group = num_q_heads / num_kv_heads;
+    p.max_pages = max_pages_per_seq;
+    p.page_size = page_size;
+    p.page_tile_shift = page_size == 32 ? 1 : 0;
+    p.scale_log2 = softmax_scale * kLog2e;
+    if ((st = grid_for(head_dim, &p.grid_ctas)) != COMEM_OK) return st;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (launch_decode_split(tm_k, tm_v, p, head_dim, stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    if (launch_combine(p, head_dim, stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    return COMEM_OK;
+}
+
+int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,
+                      const int32_t *seq_lens, int num_q_heads, int num_kv_heads, int head_dim,
+                      int page_size, float softmax_scale, void *out, int batch, int max_pages_per_seq,
+                      int64_t num_pages, float *lse_out, void *workspace, size_t workspace_bytes)
+{
+    const int st = comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, num_q_heads,
+                                           num_kv_heads, head_dim, page_size, softmax_scale, out, batch,
+                                           max_pages_per_seq, num_pages, lse_out, workspace,
+                                           workspace_bytes, nullptr);
+    if (st != COMEM_OK) return st;
+    if (cudaStreamSynchronize(nullptr) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    return COMEM_OK;
+}
+
+int comem_kv_append_async(void *k_pages, void *v_pages, const int32_t *block_table, int32_t *seq_lens,
+                          const void *new_k, const void *new_v, int num_kv_heads, int head_dim,
+                          int page_size, int batch, int max_pages_per_seq, void *cuda_stream)
+{
+    if (!k_pages || !v_pages || !block_table || !seq_lens || !new_k || !new_v) return COMEM_ERR_INVALID_ARG;
+    if (batch <= 0 || num_kv_heads <= 0 || max_pages_per_seq <= 0) return COMEM_ERR_INVALID_ARG;
+    if (head_dim != 64 && head_dim != 128) return COMEM_ERR_UNSUPPORTED;
+    if (page_size != 16 && page_size != 32) return COMEM_ERR_UNSUPPORTED;
+    if (!aligned(k_pages, 16) || !aligned(v_pages, 16) || !aligned(new_k, 16) || !aligned(new_v, 16))
+        return COMEM_ERR_INVALID_ARG;
+    const int st = check_device();
+    if (st != COMEM_OK) return st;
+    if (launch_kv_append(static_cast<__nv_bfloat16 *>(k_pages), static_cast<__nv_bfloat16 *>(v_pages),
+                         block_table, seq_lens, static_cast<const __nv_bfloat16 *>(new_k),
+                         static_cast<const __nv_bfloat16 *>(new_v), num_kv_heads * head_dim, page_size,
+                         batch, max_pages_per_seq, static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return COMEM_OK;
+}
+
+int comem_decode_step_host(const void *q_host, const void *new_k_host, const void *new_v_host, void *k_pages,
+                           void *v_pages, const int32_t *block_table, int32_t *seq_lens, int num_q_heads,
+                           int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                           void *out_host, int batch, int max_pages_per_seq, int64_t num_pages,
+                           float *lse_host, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!q_host || !out_host || ((new_k_host == nullptr) != (new_v_host == nullptr))) return COMEM_ERR_INVALID_ARG;
+    int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
+    if (st != COMEM_OK) return st;
+    const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
+    if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
+    if ((st = check_device()) != COMEM_OK) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    char *ws = static_cast<char *>(workspace);
+    const size_t q_bytes = (size_t)batch * num_q_heads * head_dim * 2;
+    const size_t kv_bytes = (size_t)batch * num_kv_heads * head_dim * 2;
+    bool ok = cudaMemcpyAsync(ws + wl.q, q_host, q_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    if (ok && new_k_host) {
+        ok = cudaMemcpyAsync(ws + wl.new_k, new_k_host, kv_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess &&
+             cudaMemcpyAsync(ws + wl.new_v, new_v_host, kv_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+        if (ok) {
+            st = comem_kv_append_async(k_pages, v_pages, block_table, seq_lens, ws + wl.new_k, ws + wl.new_v,
+                                       num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, cuda_stream);
+            if (st != COMEM_OK) return st;
+        }
+    }
+    if (!ok) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    st = comem_decode_attn_async(ws + wl.q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads,
+                                 head_dim, page_size, softmax_scale, ws + wl.out, batch, max_pages_per_seq,
+                                 num_pages, lse_host ? reinterpret_cast<float *>(ws + wl.lse) : nullptr,
+                                 workspace, workspace_bytes, cuda_stream);
+    if (st != COMEM_OK) return st;
+    ok = cudaMemcpyAsync(out_host, ws + wl.out, q_bytes, cudaMemcpyDeviceToHost, stream) == cudaSuccess;
+    if (ok && lse_host)
+        ok = cudaMemcpyAsync(lse_host, ws + wl.lse, (size_t)batch * num_q_heads * 4, cudaMemcpyDeviceToHost,
+                             stream) == cudaSuccess;
+    if (!ok || cudaStreamSynchronize(stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    return COMEM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,40 @@
+// decode_params.cuh — kernel argument block shared by the split and combine launchers.
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+namespace comem {
+
+struct DecodeParams {
+    const __nv_bfloat16 *q;      // [batch][Hq][D]
+    const int32_t *block_table;  // [batch][max_pages]
+    const int32_t *seq_lens;     // [batch]
+    __nv_bfloat16 *out;          // [batch][Hq][D]
+    float *lse_out;              // [batch][Hq] or nullptr
+    float *partials;             // workspace: [2 * grid_ctas][partial_stride_floats(D)]
+    int batch;
+    int num_q_heads;
+    int num_kv_heads;
+    int group;                   // Hq / Hkv
+    int max_pages;               // block-table row length
+    int page_size;               // 16 or 32
+    int page_tile_shift;         // log2(page_size / 16): tiles per page
+    int grid_ctas;               // persistent grid size the schedule was sized for
+    float scale_log2;            // softmax_scale * log2(e)
+};
+
+// launchers (defined in decode_split.cu / combine.cu / kv_append.cu)
+cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
+                                const DecodeParams &p, int head_dim, cudaStream_t stream);
+cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
+cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
+                             const int32_t *block_table, int32_t *seq_lens,
+                             const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v, int row_elems,
+                             int page_size, int batch, int max_pages, cudaStream_t stream);
+// occupancy-derived persistent grid for the split kernel on the current device
+cudaError_t split_default_grid(int head_dim, int *grid_ctas);
+size_t split_smem_bytes(int head_dim, int batch);
+
+}  // namespace comem

@@ -1,0 +1,430 @@
+// decode_split.cu — K1, the split-KV kernel: page-gather loader + QK^T + online softmax + PV
+// for one decode step of paged GQA attention.
+//
+// Shape of the kernel (sm_100a):
+//   * persistent grid, one contiguous range of 16-token tiles per CTA (schedule.cuh);
+//   * warp 4 = producer: reads the block table 32 entries at a time and issues, per tile,
+//     one TMA tiled load for K and one for V ([16 tokens][D] of one kv head, 128-byte
+//     swizzle) into a kStages-deep shared-memory ring guarded by full/empty mbarriers —
+//     up to kStages * 8 KiB in flight per CTA, two CTAs per SM;
+//   * warps 0..3 = consumers: tile n of the CTA goes to warp n % 4, so four independent
+//     online-softmax states stream concurrently.  Per tile and warp:
+//        S[G(pad 16) x 16 tok] = Q_g K^T      mma.sync m16n8k16 (Q fragments live in registers)
+//        m, p = online softmax in the log2 domain (quad shuffles for the row max)
+//        O^T[D x G] += V^T P^T                mma.sync with V^T via ldmatrix.trans; P is
+//                                             rounded to bf16 and l sums the ROUNDED p, so
+//                                             out is an exact weighted mean of V rows;
+//   * at the end of a (b, kv head) segment the four warp states are merged through shared
+//     memory in warp-index order and either written as the final bf16 row (the CTA owned the
+//     whole segment) or as an fp32 partial (acc, m, l) for the combine kernel.
+// The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
+// G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
+#include "decode_params.cuh"
+#include "ptx.cuh"
+#include "schedule.cuh"
+
+namespace comem {
+
+namespace {
+
+constexpr int kConsumerWarps = 4;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+constexpr int kThreads = kConsumerThreads + 32;
+constexpr unsigned kFull = 0xffffffffu;
+
+template <int D>
+struct Cfg {
+    static constexpr int kTileBytes = kTileTokens * D * 2;  // one K (or V) tile
+    static constexpr int kStageBytes = 2 * kTileBytes;      // K + V
+    static constexpr int kStages = (D == 128) ? 10 : 16;
+    static constexpr int kScratchFloatsPerWarp = D * kMaxGroup + 2 * kMaxGroup;
+    static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
+};
+
+template <int D>
+__host__ __device__ constexpr size_t smem_bytes_for(int batch)
+{
+    return 1024 /* alignment slack */ + (size_t)Cfg<D>::kStages * Cfg<D>::kStageBytes +
+           (size_t)kConsumerWarps * Cfg<D>::kScratchFloatsPerWarp * 4 + 2 * Cfg<D>::kStages * 8 +
+           ((size_t)batch + 1) * 4 + 16;
+}
+
+struct SegPos {
+    int b, kvh, j, T;  // sequence, kv head, tile index within the sequence, tiles in the sequence
+};
+
+// Locate linear tile x: the b with Hkv*prefix[b] <= x < Hkv*prefix[b+1].
+__device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch, int hkv)
+{
+    int lo = 0, hi = batch;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((int64_t)hkv * prefix[mid] <= x) lo = mid; else hi = mid;
+    }
+    SegPos s;
+    s.b = lo;
+    s.T = prefix[lo + 1] - prefix[lo];
+    const int rel = (int)(x - (int64_t)hkv * prefix[lo]);
+    s.kvh = rel / s.T;
+    s.j = rel - s.kvh * s.T;
+    return s;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 2)
+decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
+                    const DecodeParams p)
+{
+    using C = Cfg<D>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t ring = (raw + 1023u) & ~1023u;  // 1024-aligned: the 128B-swizzle atom
+    uint8_t *ring_ptr = smem_raw + (ring - raw);
+    float *scratch = reinterpret_cast<float *>(ring_ptr + C::kStages * C::kStageBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(scratch + kConsumerWarps * C::kScratchFloatsPerWarp);
+    int *prefix = reinterpret_cast<int *>(bars + 2 * C::kStages);
+    const uint32_t full0 = smem_u32(bars);
+    const uint32_t empty0 = full0 + 8 * C::kStages;
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 1);
+        }
+        fence_mbar_init();
+    }
+    if (warp == kConsumerWarps && lane == 0) {
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+    }
+    // Everything above touched no global data; inputs may come from the previous kernel.
+    pdl_wait_prior_grid();
+
+    // S1: exclusive prefix of tiles per sequence (warp 0), the whole schedule follows from it.
+    if (warp == 0) {
+        const int per = (p.batch + 31) >> 5;
+        const int b0 = lane * per;
+        int sum = 0;
+        for (int i = 0; i < per; ++i)
+            if (b0 + i < p.batch) sum += tiles_of(p.seq_lens[b0 + i]);
+        int incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += v;
+        }
+        int run = incl - sum;
+        for (int i = 0; i < per; ++i)
+            if (b0 + i < p.batch) {
+                prefix[b0 + i] = run;
+                run += tiles_of(p.seq_lens[b0 + i]);
+            }
+        if (lane == 31) prefix[p.batch] = incl;
+    }
+    __syncthreads();
+    pdl_launch_dependents();
+
+    const int64_t total = (int64_t)p.num_kv_heads * prefix[p.batch];
+    if (total == 0) return;
+    const int nc = sched_num_ctas(total, (int)gridDim.x);
+    const int cta = blockIdx.x;
+    if (cta >= nc) return;
+    const int64_t c0 = cta_begin(cta, total, nc);
+    const int64_t c1 = cta_begin(cta + 1, total, nc);
+    if (c0 >= c1) return;
+
+    if (warp == kConsumerWarps) {
+        // ------------------------------ S2: page-gather producer ------------------------------
+        const int tiles_per_page_mask = (1 << p.page_tile_shift) - 1;
+        int stage = 0;
+        uint32_t phase = 0;
+        int64_t x = c0;
+        while (x < c1) {
+            const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
+            const int64_t rem = c1 - x;
+            const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
+            const int32_t *bt = p.block_table + (int64_t)sp.b * p.max_pages;
+            for (int base = 0; base < cnt; base += 32) {
+                const int jj = sp.j + base + lane;
+                int pid = 0;
+                if (base + lane < cnt) pid = __ldg(bt + (jj >> p.page_tile_shift));
+                const int m = cnt - base < 32 ? cnt - base : 32;
+                for (int i = 0; i < m; ++i) {
+                    mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                    const int pid_i = __shfl_sync(kFull, pid, i);
+                    if (lane == 0) {
+                        const int row = pid_i * p.page_size +
+                                        (((sp.j + base + i) & tiles_per_page_mask) << kTileShift);
+                        const uint32_t dst = ring + stage * C::kStageBytes;
+                        const uint32_t bar = full0 + 8 * stage;
+                        mbar_arrive_expect_tx(bar, C::kStageBytes);
+                        tma_load_4d(dst, &tm_k, bar, 0, row, 0, sp.kvh);
+                        tma_load_4d(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh);
+                    }
+                    if (++stage == C::kStages) {
+                        stage = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+            x += cnt;
+        }
+        return;
+    }
+
+    // ------------------------------ consumers: S3..S6 -----------------------------------------
+    const int quad = lane >> 2;  // score row = query head within the group
+    const int qlane = lane & 3;
+    // ldmatrix lane addressing inside a tile: matrix (lane / 8), row (lane % 8)
+    const int ld_mat = lane >> 3;
+    const int ld_tok = ((ld_mat >> 1) << 3) + (lane & 7);
+    const uint32_t ld_row_off = ld_tok * 128;
+    const uint32_t ld_xor = ld_tok & 7;
+    const uint32_t ld_half = ld_mat & 1;
+
+    float *my_scratch = scratch + warp * C::kScratchFloatsPerWarp;
+
+    int64_t x = c0;
+    int n = 0;        // CTA-local index of the segment's first tile
+    int t = warp;     // this warp's next tile (CTA-local index)
+    int stage = warp; // == t % kStages (kStages > kConsumerWarps)
+    uint32_t phase = 0;
+
+    while (x < c1) {
+        const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
+        const int64_t rem = c1 - x;
+        const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
+        const bool whole_segment = (sp.j == 0 && cnt == sp.T);
+        const int seq_len = p.seq_lens[sp.b];
+        const int head0 = sp.kvh * p.group;
+
+        // Q fragments (A operand of S = Q K^T): row = head `quad`, rows 8..15 are zero padding.
+        uint32_t qf[C::kKSteps][2];
+        {
+            const uint32_t *qrow = reinterpret_cast<const uint32_t *>(
+                p.q + ((int64_t)sp.b * p.num_q_heads + head0 + quad) * D);
+            const bool live = quad < p.group;
+#pragma unroll
+            for (int kk = 0; kk < C::kKSteps; ++kk) {
+                qf[kk][0] = live ? __ldg(qrow + 8 * kk + qlane) : 0u;
+                qf[kk][1] = live ? __ldg(qrow + 8 * kk + 4 + qlane) : 0u;
+            }
+        }
+
+        float m_run = -INFINITY;  // running max (log2 domain) of head `quad`
+        float l_run = 0.f;        // this thread's share of the running sum of head `quad`
+        float acc[C::kKSteps][4]; // O^T: rows d = 16*mt + quad (+8), cols heads 2*qlane (+1)
+#pragma unroll
+        for (int mt = 0; mt < C::kKSteps; ++mt) acc[mt][0] = acc[mt][1] = acc[mt][2] = acc[mt][3] = 0.f;
+
+        for (; t < n + cnt; t += kConsumerWarps) {
+            mbar_wait(full0 + 8 * stage, phase);
+            const uint32_t k_base = ring + stage * C::kStageBytes;
+            const uint32_t v_base = k_base + C::kTileBytes;
+            const int valid = seq_len - ((sp.j + (t - n)) << kTileShift);  // >= 1; < 16 only on the last tile
+
+            // S3: scores for 2 n-tiles of 8 tokens
+            float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+            for (int kk = 0; kk < C::kKSteps; ++kk) {
+                uint32_t kf[4];
+                const uint32_t chunk = ((2 * kk) & 7) | ld_half;
+                ldmatrix_x4(kf, k_base + (kk >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                mma_bf16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, kf[0], kf[1]);
+                mma_bf16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, kf[2], kf[3]);
+            }
+            float s0 = s[0][0] * p.scale_log2, s1 = s[0][1] * p.scale_log2;
+            float s2 = s[1][0] * p.scale_log2, s3 = s[1][1] * p.scale_log2;
+            if (valid < kTileTokens) {
+                // ragged tail: mask by index (never by arithmetic) and zero the dead V rows so
+                // that NaN/Inf garbage past seq_len cannot reach the accumulators (0 * NaN).
+                const int tok = 2 * qlane;
+                if (tok >= valid) s0 = -INFINITY;
+                if (tok + 1 >= valid) s1 = -INFINITY;
+                if (tok + 8 >= valid) s2 = -INFINITY;
+                if (tok + 9 >= valid) s3 = -INFINITY;
+                constexpr int kChunksPerRow = D / 8;  // 16-byte chunks per V row
+                const int dead = (kTileTokens - valid) * kChunksPerRow;
+                for (int idx = lane; idx < dead; idx += 32) {
+                    const int row = valid + idx / kChunksPerRow;
+                    const int ch = idx % kChunksPerRow;
+                    const uint32_t a = v_base + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+                }
+                fence_proxy_async_smem();
+                __syncwarp();
+            }
+
+            // S4: online softmax for head `quad` over this tile's 16 tokens
+            float tmax = fmaxf(fmaxf(s0, s1), fmaxf(s2, s3));
+            tmax = fmaxf(tmax, __shfl_xor_sync(kFull, tmax, 1));
+            tmax = fmaxf(tmax, __shfl_xor_sync(kFull, tmax, 2));
+            const float m_new = fmaxf(m_run, tmax);
+            const float alpha = ex2(m_run - m_new);
+            m_run = m_new;
+            const uint32_t p01 = pack_bf16x2(ex2(s0 - m_new), ex2(s1 - m_new));  // tokens 2q, 2q+1
+            const uint32_t p23 = pack_bf16x2(ex2(s2 - m_new), ex2(s3 - m_new));  // tokens 2q+8, 2q+9
+            l_run = l_run * alpha + ((bf16lo_to_f32(p01) + bf16hi_to_f32(p01)) +
+                                     (bf16lo_to_f32(p23) + bf16hi_to_f32(p23)));
+            if (__any_sync(kFull, alpha != 1.f)) {
+                // acc columns are heads 2*qlane, 2*qlane+1: fetch their alphas from those quads
+                const float a_lo = __shfl_sync(kFull, alpha, (2 * qlane) << 2);
+                const float a_hi = __shfl_sync(kFull, alpha, (2 * qlane + 1) << 2);
+#pragma unroll
+                for (int mt = 0; mt < C::kKSteps; ++mt) {
+                    acc[mt][0] *= a_lo;
+                    acc[mt][1] *= a_hi;
+                    acc[mt][2] *= a_lo;
+                    acc[mt][3] *= a_hi;
+                }
+            }
+
+            // S5: O^T[16 d x 8 heads] += V^T[16 d x 16 tok] * P^T[16 tok x 8 heads]
+#pragma unroll
+            for (int mt = 0; mt < C::kKSteps; ++mt) {
+                uint32_t vf[4];
+                const uint32_t chunk = ((2 * mt) & 7) | ld_half;
+                ldmatrix_x4_trans(vf, v_base + (mt >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                mma_bf16_16816(acc[mt], vf[0], vf[1], vf[2], vf[3], p01, p23);
+            }
+
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+            stage += kConsumerWarps;
+            if (stage >= C::kStages) {
+                stage -= C::kStages;
+                phase ^= 1u;
+            }
+        }
+
+        // S6: merge the four warp states (warp-index order) and write the row or a partial.
+        l_run += __shfl_xor_sync(kFull, l_run, 1);
+        l_run += __shfl_xor_sync(kFull, l_run, 2);
+#pragma unroll
+        for (int mt = 0; mt < C::kKSteps; ++mt) {
+            const int d = 16 * mt + quad;
+            *reinterpret_cast<float2 *>(my_scratch + d * kMaxGroup + 2 * qlane) = make_float2(acc[mt][0], acc[mt][1]);
+            *reinterpret_cast<float2 *>(my_scratch + (d + 8) * kMaxGroup + 2 * qlane) = make_float2(acc[mt][2], acc[mt][3]);
+        }
+        if (qlane == 0) {
+            my_scratch[D * kMaxGroup + quad] = m_run;
+            my_scratch[D * kMaxGroup + kMaxGroup + quad] = l_run;
+        }
+        named_bar_sync(1, kConsumerThreads);
+        {
+            const int tid = threadIdx.x;       // 0..127
+            const int head = tid & (kMaxGroup - 1);
+            if (head < p.group) {
+                float mw[kConsumerWarps], M = -INFINITY;
+#pragma unroll
+                for (int w = 0; w < kConsumerWarps; ++w) {
+                    mw[w] = scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + head];
+                    M = fmaxf(M, mw[w]);
+                }
+                float ww[kConsumerWarps], den = 0.f;
+#pragma unroll
+                for (int w = 0; w < kConsumerWarps; ++w) {
+                    ww[w] = ex2(mw[w] - M);  // a warp that saw no tile has m = -inf -> weight 0
+                    den += ww[w] * scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + kMaxGroup + head];
+                }
+                const int64_t row = (int64_t)sp.b * p.num_q_heads + head0 + head;
+                float *part = nullptr;
+                if (!whole_segment) {
+                    const int slot = 2 * cta + (x == c0 ? 0 : 1);
+                    part = p.partials + (int64_t)slot * partial_stride_floats(D);
+                }
+                const float inv = 1.f / den;
+#pragma unroll
+                for (int it = 0; it < D / 16; ++it) {
+                    const int d = (tid >> 3) + 16 * it;
+                    float num = 0.f;
+#pragma unroll
+                    for (int w = 0; w < kConsumerWarps; ++w)
+                        num += ww[w] * scratch[w * C::kScratchFloatsPerWarp + d * kMaxGroup + head];
+                    if (whole_segment) p.out[row * D + d] = __float2bfloat16_rn(num * inv);
+                    else part[head * D + d] = num;
+                }
+                if (tid < kMaxGroup) {
+                    if (whole_segment) {
+                        if (p.lse_out) p.lse_out[row] = (M + log2f(den)) * 0.69314718055994530942f;
+                    } else {
+                        part[kMaxGroup * D + head] = M;
+                        part[kMaxGroup * D + kMaxGroup + head] = den;
+                    }
+                }
+            }
+        }
+        named_bar_sync(1, kConsumerThreads);
+
+        x += cnt;
+        n += cnt;
+    }
+}
+
+template <int D>
+cudaError_t configure_once()
+{
+    static cudaError_t status = cudaFuncSetAttribute(decode_split_kernel<D>,
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     (int)smem_bytes_for<D>(kMaxBatch));
+    return status;
+}
+
+}  // namespace
+
+size_t split_smem_bytes(int head_dim, int batch)
+{
+    return head_dim == 128 ? smem_bytes_for<128>(batch) : smem_bytes_for<64>(batch);
+}
+
+cudaError_t split_default_grid(int head_dim, int *grid_ctas)
+{
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    if (head_dim == 128) {
+        if ((e = configure_once<128>()) != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decode_split_kernel<128>, kThreads,
+                                                          smem_bytes_for<128>(64));
+    } else {
+        if ((e = configure_once<64>()) != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decode_split_kernel<64>, kThreads,
+                                                          smem_bytes_for<64>(64));
+    }
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 2) per_sm = 2;
+    *grid_ctas = sms * per_sm;
+    return cudaSuccess;
+}
+
+cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
+                                int head_dim, cudaStream_t stream)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(p.grid_ctas);
+    cfg.blockDim = dim3(kThreads);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (head_dim == 128) {
+        cudaError_t e = configure_once<128>();
+        if (e != cudaSuccess) return e;
+        cfg.dynamicSmemBytes = smem_bytes_for<128>(p.batch);
+        return cudaLaunchKernelEx(&cfg, decode_split_kernel<128>, tm_k, tm_v, p);
+    }
+    cudaError_t e = configure_once<64>();
+    if (e != cudaSuccess) return e;
+    cfg.dynamicSmemBytes = smem_bytes_for<64>(p.batch);
+    return cudaLaunchKernelEx(&cfg, decode_split_kernel<64>, tm_k, tm_v, p);
+}
+
+}  // namespace comem

@@ -1,0 +1,48 @@
+// kv_append.cu — K3: K_cache^(t) = [K_cache^(t-1); K^(t)], V likewise (typo
+// corrected per DESIGN.md reading R3).  One CTA per sequence copies the new token's
+// [Hkv][D] K row and V row (contiguous in the paged layout) into slot seq_len % page_size of
+// page block_table[b][seq_len / page_size] with 16-byte stores, then bumps seq_lens[b].
+#include "decode_params.cuh"
+#include "ptx.cuh"
+
+namespace comem {
+
+namespace {
+
+__global__ void __launch_bounds__(128)
+kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *block_table,
+                 int32_t *seq_lens, const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v,
+                 int row_elems, int page_size, int max_pages)
+{
+    pdl_wait_prior_grid();
+    const int b = blockIdx.x;
+    const int t = seq_lens[b];
+    const int page = t / page_size;
+    const int slot = t - page * page_size;
+    const int64_t pid = block_table[(int64_t)b * max_pages + page];
+    const int64_t dst = (pid * page_size + slot) * (int64_t)row_elems;
+    const int vecs = row_elems / 8;  // uint4 = 8 bf16
+    const uint4 *sk = reinterpret_cast<const uint4 *>(new_k + (int64_t)b * row_elems);
+    const uint4 *sv = reinterpret_cast<const uint4 *>(new_v + (int64_t)b * row_elems);
+    uint4 *dk = reinterpret_cast<uint4 *>(k_pages + dst);
+    uint4 *dv = reinterpret_cast<uint4 *>(v_pages + dst);
+    for (int i = threadIdx.x; i < vecs; i += blockDim.x) {
+        dk[i] = sk[i];
+        dv[i] = sv[i];
+    }
+    __syncthreads();  // every thread has read seq_lens[b] before it changes
+    if (threadIdx.x == 0) seq_lens[b] = t + 1;
+}
+
+}  // namespace
+
+cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *block_table,
+                             int32_t *seq_lens, const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v,
+                             int row_elems, int page_size, int batch, int max_pages, cudaStream_t stream)
+{
+    kv_append_kernel<<<batch, 128, 0, stream>>>(k_pages, v_pages, block_table, seq_lens, new_k, new_v,
+                                               row_elems, page_size, max_pages);
+    return cudaGetLastError();
+}
+
+}  // namespace comem

@@ -1,0 +1,108 @@
+"""CPU-side checks of the C-ABI library: it loads without a GPU, exports every symbol
+include/comem_decode_attn.h declares, validates arguments, and its host scheduler mirror
+partitions the tile space exactly.  No compute calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2605_30842_b200 as comem
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "comem_decode_attn.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2605_30842_b200 import build
+
+    build.build()
+    return comem.load_library()
+
+
+def declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(comem_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_header_symbols_all_exported(lib):
+    names = declared_symbols()
+    assert {"comem_decode_attn", "comem_decode_attn_async", "comem_decode_attn_workspace_bytes",
+            "comem_kv_append_async", "comem_decode_step_host", "comem_schedule_host",
+            "comem_status_string", "comem_version"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in the header but not exported"
+
+
+def test_version_and_status_strings(lib):
+    assert comem.comem_version() >= 100
+    seen = {comem.comem_status_string(s) for s in range(5)}
+    assert len(seen) == 5 and "ok" in seen
+    assert comem.comem_status_string(99) == "unknown status"
+
+
+def test_workspace_bytes_pure_host(lib):
+    a = comem.comem_decode_attn_workspace_bytes(1, 64, 8, 128, 16, 2048)
+    b = comem.comem_decode_attn_workspace_bytes(32, 64, 8, 128, 16, 4096)
+    assert 0 < a < b < 64 << 20 and a % 256 == 0
+    assert comem.comem_decode_attn_workspace_bytes(0, 64, 8, 128, 16, 1) == 0
+
+
+def _call(lib, **over):
+    """comem_decode_attn_async with dummy non-null pointers; validation must reject before any launch."""
+    a = dict(q=256, k=256, v=512, bt=256, sl=256, hq=64, hkv=8, d=128, ps=16, scale=0.1, out=256,
+             batch=1, maxp=16, npages=16, lse=None, ws=256, wsb=1 << 26, stream=None)
+    a.update(over)
+    return lib.comem_decode_attn_async(a["q"], a["k"], a["v"], a["bt"], a["sl"], a["hq"], a["hkv"],
+                                       a["d"], a["ps"], ctypes.c_float(a["scale"]), a["out"],
+                                       a["batch"], a["maxp"], a["npages"], a["lse"], a["ws"], a["wsb"],
+                                       a["stream"])
+
+
+def test_argument_validation(lib):
+    assert _call(lib, q=None) == comem.COMEM_ERR_INVALID_ARG
+    assert _call(lib, out=None) == comem.COMEM_ERR_INVALID_ARG
+    assert _call(lib, batch=0) == comem.COMEM_ERR_INVALID_ARG
+    assert _call(lib, hq=60) == comem.COMEM_ERR_INVALID_ARG            # 60 % 8 != 0
+    assert _call(lib, scale=float("nan")) == comem.COMEM_ERR_INVALID_ARG
+    assert _call(lib, scale=-1.0) == comem.COMEM_ERR_INVALID_ARG
+    assert _call(lib, q=258) == comem.COMEM_ERR_INVALID_ARG            # misaligned
+    assert _call(lib, d=96) == comem.COMEM_ERR_UNSUPPORTED
+    assert _call(lib, ps=8) == comem.COMEM_ERR_UNSUPPORTED
+    assert _call(lib, hq=128) == comem.COMEM_ERR_UNSUPPORTED           # group 16
+    assert _call(lib, batch=5000) == comem.COMEM_ERR_UNSUPPORTED
+    assert _call(lib, npages=1 << 28) == comem.COMEM_ERR_UNSUPPORTED   # row coordinate overflows int32
+    assert _call(lib, ws=None) == comem.COMEM_ERR_WORKSPACE
+    assert _call(lib, wsb=1024) == comem.COMEM_ERR_WORKSPACE
+    # fully valid arguments but no usable device here -> CUDA error, never a crash or a CPU fallback
+    import torch
+    if not torch.cuda.is_available():
+        assert _call(lib) in (comem.COMEM_ERR_CUDA, comem.COMEM_ERR_UNSUPPORTED)
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    from paper_2605_30842_b200 import binding
+
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "_LIB_PATH", "/nonexistent/libcomem_decode.so")
+    with pytest.raises(RuntimeError, match="no CPU or PyTorch fallback"):
+        binding.load_library()
+
+
+@pytest.mark.parametrize("lens,hkv,grid", [([32768], 8, 296), ([512], 1, 296), ([1], 1, 296),
+                                            ([0, 0], 2, 8), ([100, 0, 37, 5000, 16], 8, 296),
+                                            (list(range(1, 200)), 4, 296)])
+def test_schedule_partitions_tile_space(lib, lens, hkv, grid):
+    begins = comem.comem_schedule_host(lens, hkv, grid)
+    tiles = sum((l + 15) // 16 for l in lens) * hkv
+    if tiles == 0:
+        assert begins == [0]
+        return
+    assert begins[0] == 0 and begins[-1] == tiles
+    sizes = np.diff(begins)
+    assert (sizes >= 0).all() and sizes.max() - sizes.min() <= 1       # balanced to one tile
+    nc = len(begins) - 1
+    assert nc == min(grid, max(1, -(-tiles // 8)))

@@ -1,0 +1,200 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 oracle, element by element, on
+the same seeded inputs; plus the properties that must hold bit-exactly."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2605_30842_b200 as comem
+from paper_2605_30842_b200 import workloads as W
+from parity_util import (all_pairs, assert_parity, check_batch, errors, gpu_run, oracle_rows)
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def bits(t: torch.Tensor) -> torch.Tensor:
+    return t.contiguous().view(torch.int16)
+
+
+# ---- small shapes: every G / D / page_size, lengths straddling tile, page and CTA boundaries ------
+@pytest.mark.parametrize("G", [1, 2, 4, 8])
+@pytest.mark.parametrize("D", [64, 128])
+@pytest.mark.parametrize("ps", [16, 32])
+def test_small_grid(oracle, G, D, ps):
+    lens = [1, 15, 16, 17, 31, 32, 33, 127, 128, 129, 512, 1000, 0, 2049]
+    b = W.make_batch(lens, 2 * G, 2, D, ps, seed=100 + G + D + ps, device=DEV, poison_unused=True)
+    check_batch(oracle, b, what=f"G{G} D{D} ps{ps}")
+
+
+@pytest.mark.parametrize("hkv", [1, 3, 8])
+def test_kv_head_counts(oracle, hkv):
+    b = W.make_batch([700, 33, 4097], 4 * hkv, hkv, 128, 16, seed=7 + hkv, device=DEV, poison_unused=True)
+    check_batch(oracle, b, what=f"hkv{hkv}")
+
+
+def test_config1_tiny(oracle):
+    b = W.config1_tiny(DEV, poison_unused=True)
+    _, _, err = check_batch(oracle, b, what="C1")
+    print("C1", err)
+
+
+def test_ragged_many_ctas(oracle):
+    # long enough that segments are cut by CTA-range boundaries (partials + combine) and short
+    # enough that others are owned by one CTA (direct write), in one launch
+    lens = [20000, 37, 0, 50001, 8191, 16, 300]
+    b = W.make_batch(lens, 64, 8, 128, 16, seed=21, device=DEV, poison_unused=True)
+    check_batch(oracle, b, what="ragged")
+    b32 = W.make_batch(lens, 32, 8, 128, 32, seed=22, device=DEV, poison_unused=True)
+    check_batch(oracle, b32, what="ragged ps32")
+
+
+def test_single_cta_path_vs_split_path_same_row(oracle):
+    """The same logical row computed with 1 CTA (no split) and with the full grid must both match
+    the oracle; forcing the grid exercises comem_set_grid_ctas."""
+    b = W.make_batch([6000], 8, 1, 128, 16, seed=31, device=DEV)
+    try:
+        comem.comem_set_grid_ctas(1)
+        o1, _, _ = check_batch(oracle, b, what="grid1")
+        comem.comem_set_grid_ctas(7)
+        o7, _, _ = check_batch(oracle, b, what="grid7")
+    finally:
+        comem.comem_set_grid_ctas(0)
+    ofull, _, _ = check_batch(oracle, b, what="gridfull")
+    assert float((o1.float() - ofull.float()).abs().max()) < 2e-2
+
+
+# ---- closed forms on the GPU --------------------------------------------------------------------------
+def test_o1_single_token_bit_exact():
+    b = W.make_batch([1, 1, 1, 1], 64, 8, 128, 16, seed=41, device=DEV, poison_unused=True)
+    out, lse = gpu_run(b)
+    for i in range(4):
+        pid = int(b.block_table[i, 0])
+        v = b.v_pages[pid, 0]                                   # [Hkv, D]
+        want = v.repeat_interleave(8, dim=0)
+        assert torch.equal(bits(out[i]), bits(want))
+
+
+def test_o2_identical_keys_mean_of_v(oracle):
+    b = W.make_batch([777], 8, 1, 128, 16, seed=42, device=DEV)
+    b.k_pages[:] = b.k_pages[0, 0, 0].clone()
+    out, _ = gpu_run(b)
+    pid = b.block_table[0, :49].long()
+    v = b.v_pages[pid].reshape(-1, 128)[:777].double().mean(dim=0)
+    assert float((out[0].double() - v).abs().max()) <= 2.0 ** -8 * float(v.abs().max()) + 1e-6
+
+
+def test_o5_constant_v():
+    b = W.make_batch([5000, 90], 16, 2, 128, 16, seed=43, device=DEV)
+    c = torch.randn(128, generator=torch.Generator().manual_seed(1)).to(torch.bfloat16).to(DEV)
+    b.v_pages[:] = c
+    out, _ = gpu_run(b)
+    # out is an exact weighted mean of identical rows: only the final bf16 rounding may differ
+    assert float((out.double() - c.double()).abs().max()) <= 2.0 ** -8 * float(c.double().abs().max())
+
+
+def test_o8_large_logits_no_overflow(oracle):
+    b = W.make_batch([300], 8, 1, 128, 16, seed=44, device=DEV)
+    b.q[:] = 0
+    b.q[0, :, 0] = 16.0
+    b.k_pages[:] = 0
+    b.k_pages[:, :, :, 0] = 30.0
+    pid, slot = int(b.block_table[0, 13]), 5
+    b.k_pages[pid, slot, 0, 0] = 640.0                       # logit 16*640/sqrt(128) ~ 905 vs 42
+    out, lse = gpu_run(b)
+    assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
+    assert torch.equal(bits(out[0, 3]), bits(b.v_pages[pid, slot, 0]))
+    check_batch(oracle, b, what="large logits")
+
+
+# ---- bit-identity properties ---------------------------------------------------------------------------
+def test_o9_page_permutation_bit_identical():
+    lens = [20000, 37, 50001, 8191]
+    b = W.make_batch(lens, 64, 8, 128, 16, seed=51, device=DEV, num_pages=6000)
+    o1, l1 = gpu_run(b)
+    for s in (5, 6):
+        b2 = W.permute_pages(b, seed=s)
+        o2, l2 = gpu_run(b2)
+        assert torch.equal(bits(o1), bits(o2)) and torch.equal(l1, l2)
+
+
+def test_o12_tail_poison_bit_identical():
+    lens = [37, 16, 5, 4000, 1]
+    clean = W.make_batch(lens, 32, 8, 128, 32, seed=52, device=DEV, num_pages=300, max_pages_per_seq=200)
+    o1, l1 = gpu_run(clean)
+    for poison in (float("nan"), float("inf"), -float("inf"), 1e38):
+        dirty = W.make_batch(lens, 32, 8, 128, 32, seed=52, device=DEV, num_pages=300,
+                             max_pages_per_seq=200, poison_unused=True)
+        nanmask_k = torch.isnan(dirty.k_pages.float())
+        dirty.k_pages[nanmask_k] = poison
+        dirty.v_pages[torch.isnan(dirty.v_pages.float())] = poison
+        dirty.block_table[dirty.block_table < 0] = 2 ** 30
+        o2, l2 = gpu_run(dirty)
+        assert torch.equal(bits(o1), bits(o2)) and torch.equal(l1, l2), poison
+
+
+def test_run_to_run_and_cross_stream_determinism():
+    b = W.make_batch([30000, 9000, 123], 64, 8, 128, 16, seed=53, device=DEV)
+    o0, l0 = gpu_run(b)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for i in range(10):
+        o, l = gpu_run(b, stream=side if i % 2 else None)
+        torch.cuda.synchronize()
+        assert torch.equal(bits(o), bits(o0)) and torch.equal(l, l0)
+
+
+# ---- API surface -------------------------------------------------------------------------------------------
+def test_sync_entry_point_and_no_lse(oracle):
+    b = W.make_batch([1234, 77], 16, 2, 64, 16, seed=61, device=DEV)
+    out = comem.comem_decode_attn(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale)
+    ref, _ = oracle_rows(oracle, b, all_pairs(b))
+    assert_parity(errors(out, ref, all_pairs(b)), "sync")
+
+
+def test_kv_append_matches_oracle(oracle):
+    b = W.make_batch([15, 16, 31, 1000], 16, 2, 128, 16, seed=62, device=DEV, spare_tokens=40)
+    kb = oracle.as_bits(b.k_pages.cpu()).copy()
+    vb = oracle.as_bits(b.v_pages.cpu()).copy()
+    sl = b.seq_lens.cpu().numpy().copy()
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    out = torch.empty_like(b.q)
+    for step in range(35):
+        q, nk, nv = W.decode_step_rows(b, step, 6200)
+        comem.comem_kv_append_async(b.k_pages, b.v_pages, b.block_table, b.seq_lens, nk, nv)
+        comem.comem_decode_attn_async(q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                      b.softmax_scale, out, ws)
+        oracle.kv_append(kb, vb, b.block_table.cpu(), sl, nk.cpu(), nv.cpu())
+        if step in (0, 1, 16, 17, 34):
+            torch.cuda.synchronize()
+            assert np.array_equal(b.seq_lens.cpu().numpy(), sl)
+            assert np.array_equal(oracle.as_bits(b.k_pages.cpu()), kb)       # append is byte-exact
+            assert np.array_equal(oracle.as_bits(b.v_pages.cpu()), vb)
+            ref, _ = oracle.decode_attn(q.cpu(), kb, vb, b.block_table.cpu(), sl, b.softmax_scale)
+            assert_parity(errors(out, ref.reshape(-1, 128), all_pairs(b)), f"step {step}")
+
+
+def test_decode_step_host(oracle):
+    b = W.make_batch([4000, 333], 64, 8, 128, 16, seed=63, device=DEV, spare_tokens=4)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    q, nk, nv = (t.cpu().pin_memory() for t in W.decode_step_rows(b, 0, 6300))
+    out_h = torch.empty_like(q).pin_memory()
+    lse_h = torch.empty((2, 64), dtype=torch.float32).pin_memory()
+    comem.comem_decode_step_host(q, nk, nv, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                 b.softmax_scale, out_h, ws, lse_host=lse_h)
+    assert b.seq_lens.cpu().tolist() == [4001, 334]
+    b2 = W.DecodeBatch(q=q.to(DEV), k_pages=b.k_pages, v_pages=b.v_pages, block_table=b.block_table,
+                       seq_lens=b.seq_lens, softmax_scale=b.softmax_scale)
+    ref, ref_lse = oracle_rows(oracle, b2, all_pairs(b2))
+    assert_parity(errors(out_h.to(DEV), ref, all_pairs(b2)), "step_host")
+    assert np.max(np.abs(lse_h.numpy().reshape(-1) - ref_lse)) < 1e-3
+
+
+def test_unsupported_and_invalid_raise():
+    b = W.make_batch([100], 16, 1, 128, 16, seed=64, device=DEV)                # group 16
+    with pytest.raises(comem.ComemError) as e:
+        gpu_run(b)
+    assert e.value.status == comem.COMEM_ERR_UNSUPPORTED
+    b = W.make_batch([100], 8, 1, 128, 16, seed=64, device=DEV)
+    with pytest.raises(comem.ComemError) as e:
+        gpu_run(b, workspace=torch.empty(1024, dtype=torch.uint8, device=DEV))
+    assert e.value.status == comem.COMEM_ERR_WORKSPACE
