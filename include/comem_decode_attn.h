@@ -90,6 +90,24 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                             int64_t num_pages, float *lse_out, void *workspace,
                             size_t workspace_bytes, void *cuda_stream);
 
+/*
+ * comem_decode_attn_phases_async — the same step with its two kernels selectable:
+ * COMEM_PHASE_SPLIT runs K1 (page-gather + QK^T + online softmax + PV; writes finished rows
+ * and the split partials into `workspace`), COMEM_PHASE_COMBINE runs K2 (LSE merge of the
+ * partials in `workspace`; also writes the rows of empty sequences).  SPLIT|COMBINE is
+ * comem_decode_attn_async.  Running the phases in separate calls (same arguments, same
+ * workspace, same stream order) gives the identical result; bench.py uses SPLIT alone to time
+ * the dominant kernel with CUDA events.
+ */
+enum { COMEM_PHASE_SPLIT = 1, COMEM_PHASE_COMBINE = 2 };
+int comem_decode_attn_phases_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens,
+                                   int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                                   float softmax_scale, void *out, int batch,
+                                   int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream,
+                                   int phases);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,

@@ -15,6 +15,9 @@ from .binding import (  # noqa: F401
     alloc_workspace,
     comem_decode_attn,
     comem_decode_attn_async,
+    comem_decode_attn_phases_async,
+    COMEM_PHASE_SPLIT,
+    COMEM_PHASE_COMBINE,
     comem_decode_attn_workspace_bytes,
     comem_decode_step_host,
     comem_grid_ctas,

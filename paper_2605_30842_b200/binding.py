@@ -49,6 +49,9 @@ def load_library():
     lib.comem_decode_attn_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
                                             i64, vp, vp, sz, vp]
     lib.comem_decode_attn_async.restype = i32
+    lib.comem_decode_attn_phases_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
+                                                   i32, i64, vp, vp, sz, vp, i32]
+    lib.comem_decode_attn_phases_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
     lib.comem_decode_attn.restype = i32
@@ -139,6 +142,25 @@ def _check_inputs(q, k_pages, v_pages, block_table, seq_lens):
     assert q.dim() == 3 and k_pages.dim() == 4 and k_pages.shape == v_pages.shape
     assert block_table.dim() == 2 and block_table.shape[0] == q.shape[0] == seq_lens.shape[0]
     assert k_pages.shape[3] == q.shape[2]
+
+
+COMEM_PHASE_SPLIT = 1
+COMEM_PHASE_COMBINE = 2
+
+
+def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
+                                   workspace, lse_out=None, stream=None,
+                                   phases: int = COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) -> None:
+    """Enqueue the selected kernels of one decode-attention step on ``stream``; returns at once."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_phases_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream), int(phases))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_phases_async")
 
 
 def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,

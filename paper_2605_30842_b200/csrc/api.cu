@@ -232,12 +232,14 @@ int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_head
     return COMEM_OK;
 }
 
-int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
-                            const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
-                            int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
-                            int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
-                            void *workspace, size_t workspace_bytes, void *cuda_stream)
+int comem_decode_attn_phases_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                                   void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                                   float *lse_out, void *workspace, size_t workspace_bytes,
+                                   void *cuda_stream, int phases)
 {
+    if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;
     int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
     if (st != COMEM_OK) return st;
@@ -271,9 +273,27 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
     if ((st = grid_for(head_dim, &p.grid_ctas)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    if (launch_decode_split(tm_k, tm_v, p, head_dim, stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
-    if (launch_combine(p, head_dim, stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    if ((phases & COMEM_PHASE_COMBINE) && launch_combine(p, head_dim, stream) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
     return COMEM_OK;
+}
+
+int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
+                            const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                            int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
+                            int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                            void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    return comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads,
+                                          head_dim, page_size, softmax_scale, out, batch, max_pages_per_seq,
+                                          num_pages, lse_out, workspace, workspace_bytes, cuda_stream,
+                                          COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
 }
 
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,

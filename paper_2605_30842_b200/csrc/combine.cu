@@ -2,7 +2,8 @@
 //
 // One CTA per output row (sequence b, query head h).  It recomputes the same schedule as the split kernel
 // (schedule.cuh) to learn which CTAs cut this segment, then merges their fp32 partials
-// (acc, m, l) in CTA-index order:
+// (acc, m, l, lx) in CTA-index order (l sums the bf16-rounded p and normalises out; lx sums the
+// unrounded p and only feeds lse_out):
 //     M = max_s m_s;  w_s = 2^(m_s - M);  out = (sum_s w_s acc_s) / (sum_s w_s l_s)
 // Segments owned by a single CTA were already written by the split kernel and are skipped;
 // empty sequences (seq_len == 0) get +0.0 rows and lse = -inf here (reading R9).
@@ -25,7 +26,7 @@ combine_kernel(const DecodeParams p)
     static_assert(kCombineThreads / kVec >= kParts, "layout");
     __shared__ int s_before, s_total;
     __shared__ float s_m[kCombineThreads / 32];
-    __shared__ float s_den[kParts];
+    __shared__ float s_den[kParts], s_denx[kParts];
     __shared__ float4 s_red[kParts][kVec];
 
     const int b = blockIdx.x / p.num_q_heads;
@@ -90,7 +91,7 @@ combine_kernel(const DecodeParams p)
     const int vec = tid % kVec;
     const int part = tid / kVec;
     float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
-    float den = 0.f;
+    float den = 0.f, den_x = 0.f;
     if (part < kParts) {
 #pragma unroll 4
         for (int s = part; s < nsplit; s += kParts) {
@@ -98,20 +99,22 @@ combine_kernel(const DecodeParams p)
             const float w = ex2(rec[kMaxGroup * D + g] - M);
             const float4 a = *reinterpret_cast<const float4 *>(rec + g * D + 4 * vec);
             den += w * rec[kMaxGroup * D + kMaxGroup + g];
+            den_x += w * rec[kMaxGroup * D + 2 * kMaxGroup + g];
             num.x += w * a.x; num.y += w * a.y; num.z += w * a.z; num.w += w * a.w;
         }
         s_red[part][vec] = num;
-        if (vec == 0) s_den[part] = den;
+        if (vec == 0) { s_den[part] = den; s_denx[part] = den_x; }
     }
     __syncthreads();
     if (part == 0) {  // merge the stripes in stripe order
         float4 r = s_red[0][vec];
-        float dsum = s_den[0];
+        float dsum = s_den[0], dxsum = s_denx[0];
 #pragma unroll
         for (int q = 1; q < kParts; ++q) {
             const float4 o = s_red[q][vec];
             r.x += o.x; r.y += o.y; r.z += o.z; r.w += o.w;
             dsum += s_den[q];
+            dxsum += s_denx[q];
         }
         const float inv = 1.f / dsum;
         __nv_bfloat162 lo = __floats2bfloat162_rn(r.x * inv, r.y * inv);
@@ -120,7 +123,7 @@ combine_kernel(const DecodeParams p)
         packed.x = *reinterpret_cast<uint32_t *>(&lo);
         packed.y = *reinterpret_cast<uint32_t *>(&hi);
         *reinterpret_cast<uint2 *>(p.out + row * D + 4 * vec) = packed;
-        if (p.lse_out && vec == 0) p.lse_out[row] = (M + log2f(dsum)) * 0.69314718055994530942f;
+        if (p.lse_out && vec == 0) p.lse_out[row] = (M + log2f(dxsum)) * 0.69314718055994530942f;
     }
 }
 

@@ -36,8 +36,12 @@ template <int D>
 struct Cfg {
     static constexpr int kTileBytes = kTileTokens * D * 2;  // one K (or V) tile
     static constexpr int kStageBytes = 2 * kTileBytes;      // K + V
-    static constexpr int kStages = (D == 128) ? 10 : 16;
-    static constexpr int kScratchFloatsPerWarp = D * kMaxGroup + 2 * kMaxGroup;
+    // kStages % kConsumerWarps == 0 so that a ring stage always belongs to the same consumer warp:
+    // a warp then never waits on a stage more than one phase ahead of the barrier (mbarrier waits
+    // carry only the phase PARITY; out-of-order TMA completion could otherwise alias two phases).
+    static constexpr int kStages = (D == 128) ? 8 : 16;
+    static_assert(kStages % kConsumerWarps == 0, "ring stages must map to a fixed consumer warp");
+    static constexpr int kScratchFloatsPerWarp = D * kMaxGroup + 3 * kMaxGroup;
     static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
 };
 
@@ -215,7 +219,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         }
 
         float m_run = -INFINITY;  // running max (log2 domain) of head `quad`
-        float l_run = 0.f;        // this thread's share of the running sum of head `quad`
+        float l_run = 0.f;        // this thread's share of the running sum of the bf16-ROUNDED p (normaliser)
+        float lx_run = 0.f;       // same for the unrounded p (only feeds lse_out)
         float acc[C::kKSteps][4]; // O^T: rows d = 16*mt + quad (+8), cols heads 2*qlane (+1)
 #pragma unroll
         for (int mt = 0; mt < C::kKSteps; ++mt) acc[mt][0] = acc[mt][1] = acc[mt][2] = acc[mt][3] = 0.f;
@@ -265,8 +270,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const float m_new = fmaxf(m_run, tmax);
             const float alpha = ex2(m_run - m_new);
             m_run = m_new;
-            const uint32_t p01 = pack_bf16x2(ex2(s0 - m_new), ex2(s1 - m_new));  // tokens 2q, 2q+1
-            const uint32_t p23 = pack_bf16x2(ex2(s2 - m_new), ex2(s3 - m_new));  // tokens 2q+8, 2q+9
+            const float e0 = ex2(s0 - m_new), e1 = ex2(s1 - m_new), e2 = ex2(s2 - m_new), e3 = ex2(s3 - m_new);
+            const uint32_t p01 = pack_bf16x2(e0, e1);  // tokens 2q, 2q+1
+            const uint32_t p23 = pack_bf16x2(e2, e3);  // tokens 2q+8, 2q+9
+            lx_run = lx_run * alpha + ((e0 + e1) + (e2 + e3));
             l_run = l_run * alpha + ((bf16lo_to_f32(p01) + bf16hi_to_f32(p01)) +
                                      (bf16lo_to_f32(p23) + bf16hi_to_f32(p23)));
             if (__any_sync(kFull, alpha != 1.f)) {
@@ -303,6 +310,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // S6: merge the four warp states (warp-index order) and write the row or a partial.
         l_run += __shfl_xor_sync(kFull, l_run, 1);
         l_run += __shfl_xor_sync(kFull, l_run, 2);
+        lx_run += __shfl_xor_sync(kFull, lx_run, 1);
+        lx_run += __shfl_xor_sync(kFull, lx_run, 2);
 #pragma unroll
         for (int mt = 0; mt < C::kKSteps; ++mt) {
             const int d = 16 * mt + quad;
@@ -312,6 +321,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         if (qlane == 0) {
             my_scratch[D * kMaxGroup + quad] = m_run;
             my_scratch[D * kMaxGroup + kMaxGroup + quad] = l_run;
+            my_scratch[D * kMaxGroup + 2 * kMaxGroup + quad] = lx_run;
         }
         named_bar_sync(1, kConsumerThreads);
         {
@@ -324,11 +334,12 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     mw[w] = scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + head];
                     M = fmaxf(M, mw[w]);
                 }
-                float ww[kConsumerWarps], den = 0.f;
+                float ww[kConsumerWarps], den = 0.f, den_x = 0.f;
 #pragma unroll
                 for (int w = 0; w < kConsumerWarps; ++w) {
                     ww[w] = ex2(mw[w] - M);  // a warp that saw no tile has m = -inf -> weight 0
                     den += ww[w] * scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + kMaxGroup + head];
+                    den_x += ww[w] * scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + 2 * kMaxGroup + head];
                 }
                 const int64_t row = (int64_t)sp.b * p.num_q_heads + head0 + head;
                 float *part = nullptr;
@@ -349,10 +360,11 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 }
                 if (tid < kMaxGroup) {
                     if (whole_segment) {
-                        if (p.lse_out) p.lse_out[row] = (M + log2f(den)) * 0.69314718055994530942f;
+                        if (p.lse_out) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
                     } else {
                         part[kMaxGroup * D + head] = M;
                         part[kMaxGroup * D + kMaxGroup + head] = den;
+                        part[kMaxGroup * D + 2 * kMaxGroup + head] = den_x;
                     }
                 }
             }
