@@ -1,0 +1,471 @@
+#!/usr/bin/env python
+"""bench.py — decode-attention µs/step and achieved HBM GB/s (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4] [--impl reference]
+
+A "step" is one pass of the whole hot path (split-KV kernel + LSE combine)
+over one synthetic decode batch.  The default workload is BASELINE.json configs[1] (C2: batch 1,
+64q/8kv heads, D 128, 32 768-token context, page_size 16, pages permuted in a 4 096-page pool).
+
+What the ONE JSON line on stdout holds (rank 0):
+  value / ms_per_step  whole-job GB/s = algorithmic KV+Q bytes of all ranks / max-over-ranks device
+                       time of EXACTLY K steps, inputs resident in HBM, CUDA events on the launch stream
+  roofline             the dominant kernel (split-KV) timed alone over K launches, against
+                       MEASURED_PEAKS.json's hbm_gbs
+  e2e                  the same metric through comem_decode_step_host: every step copies q and the new
+                       (k, v) rows from pinned host memory, appends, attends, copies out back
+  cpu_baseline         the fp64 oracle (oracle/, test infrastructure) on this box's host cores
+  parity               GPU vs oracle on the bench's own inputs (max-abs / mean-abs / rel-l2)
+
+L2-cold rule: C2's KV (128 MiB) is about one L2 (126 MB), so steps rotate over R = 8 disjoint pools
+(2 GiB of K+V); C3/C4 read 4.8 / 8.6 GB per step, nothing survives between steps.
+
+`--impl reference`: this tier has no reference implementation; the arm times the oracle, as it
+stands, on a bounded sample of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "decode_attn_achieved_hbm_gbs"
+UNIT = "GB/s"
+FALLBACK_PEAK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+L2_BYTES_NOMINAL = 126e6
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE split-KV launch from the committed
+# `ncu --set full` capture (profiles/README.md names the command); None until captured.
+NCU_TRAFFIC_BYTES = {"c2": None, "c3": None, "c4": None}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8192)
+    ap.add_argument("--warmup", type=int, default=64)
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-budget-s", type=float, default=120.0,
+                    help="--impl reference: wall-clock budget for the whole run")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------------------------
+def workload_desc(name: str) -> dict:
+    if name == "c2":
+        return {"workload": "C2 agent decode: batch 1, 64q/8kv, D128, ctx 32768, page 16, 4096-page pool",
+                "batch": 1, "num_q_heads": 64, "num_kv_heads": 8, "head_dim": 128, "page_size": 16,
+                "context": 32768}
+    if name == "c3":
+        return {"workload": "C3 agent decode: batch 32, 64q/8kv, D128, ctx U[8192,65536], page 16",
+                "batch": 32, "num_q_heads": 64, "num_kv_heads": 8, "head_dim": 128, "page_size": 16,
+                "context": "U[8192,65536] seed 1003"}
+    return {"workload": "C4 memory-model decode: batch 16, 32q/8kv, D128, ctx 131072, page 32, 1% peaked keys",
+            "batch": 16, "num_q_heads": 32, "num_kv_heads": 8, "head_dim": 128, "page_size": 32,
+            "context": 131072}
+
+
+def make_pools(name: str, device, rank: int, spare_tokens: int):
+    """The rotating set of decode batches for one rank (seeds differ per rank and per pool)."""
+    from paper_2605_30842_b200 import workloads as W
+
+    if name == "c2":
+        pools = []
+        for i in range(8):
+            pools.append(W.make_batch([32768], 64, 8, 128, 16, 1002 + i + 100 * rank, device, k_scale=0.5,
+                                      num_pages=4096,
+                                      max_pages_per_seq=W.pages_needed(32768 + spare_tokens, 16),
+                                      spare_tokens=spare_tokens, name="C2-agent-1x32K"))
+        return pools
+    if name == "c3":
+        return [W.config3_agent_ragged(device, spare_tokens=spare_tokens)]
+    return [W.make_batch([131072] * 16, 32, 8, 128, 32, 1004 + 100 * rank, device,
+                         num_pages=16 * W.pages_needed(131072 + spare_tokens, 32) + 4096,
+                         max_pages_per_seq=max(4096, W.pages_needed(131072 + spare_tokens, 32)),
+                         spare_tokens=spare_tokens, peaked_frac=0.01, peaked_offset=4.0,
+                         name="C4-memory-16x128K")]
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks (sampled DURING the timed regions)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Polls NVML every few ms from a thread: SM clock and clock-event (throttle) reasons."""
+
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, uuid: str, index: int):
+        self.samples, self.reasons, self.active = [], set(), False
+        self.max_mhz, self.err = None, None
+        self._stop = threading.Event()
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid).encode())
+            except Exception:  # noqa: BLE001
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self._reasons_fn = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+        except Exception as e:  # noqa: BLE001
+            self.nv, self.err = None, repr(e)
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set():
+            if self.active and self.nv is not None:
+                try:
+                    mhz = int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                    r = int(self._reasons_fn(self.h))
+                    self.samples.append(mhz)
+                    for bit, nm in self.REASONS.items():
+                        if r & bit:
+                            self.reasons.add(nm)
+                except Exception as e:  # noqa: BLE001
+                    self.err = repr(e)
+            time.sleep(0.002)
+
+    def start(self):
+        self.t.start()
+
+    def stop(self):
+        self._stop.set()
+        self.t.join(timeout=1.0)
+
+    def summary(self) -> dict:
+        s = sorted(self.samples)
+        out = {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(self.reasons), "samples": len(s)}
+        if self.err:
+            out["error"] = self.err
+        return out
+
+
+# ---------------------------------------------------------------------------------------------
+# the timed loops
+# ---------------------------------------------------------------------------------------------
+def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, phases, use_graph, sampler,
+                device):
+    """`warmup` untimed steps, then EXACTLY `steps` steps on `stream`, bracketed by barrier +
+    synchronize on both sides; CUDA events on that stream.  Returns this rank's milliseconds."""
+    R = len(pools)
+
+    def enqueue(first, n):
+        for i in range(first, first + n):
+            b = pools[i % R]
+            comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                                 b.softmax_scale, outs[i % R], ws, stream=stream, phases=phases)
+
+    with torch.cuda.stream(stream):
+        enqueue(0, max(warmup, 3))
+        stream.synchronize()
+        graph = None
+        if use_graph and steps >= R:
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=stream):
+                enqueue(0, R)
+            graph.replay()
+            stream.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        replicas.barrier()
+        torch.cuda.synchronize(device)
+        sampler.active = True
+        e0.record(stream)
+        done = 0
+        if graph is not None:
+            for _ in range(steps // R):
+                graph.replay()
+            done = (steps // R) * R
+        enqueue(done, steps - done)
+        e1.record(stream)
+        torch.cuda.synchronize(device)
+        sampler.active = False
+        replicas.barrier()
+    return e0.elapsed_time(e1)
+
+
+def timed_e2e(torch, comem, replicas, pools, ws, stream, steps, warmup, sampler, device, seed_base):
+    """End to end through comem_decode_step_host: per step H2D(q, new k, new v) from pinned host
+    memory -> append -> attention -> D2H(out), host-synchronous.  Returns (ms, bytes, h2d, d2h)."""
+    from paper_2605_30842_b200 import workloads as W
+
+    R = len(pools)
+    nrows = 4  # distinct pre-generated host rows per pool, cycled (no RNG in the timed loop)
+    host = []
+    for i, b in enumerate(pools):
+        rows = []
+        for j in range(nrows):
+            q, nk, nv = W.decode_step_rows(b, j, seed_base + 16 * i)
+            rows.append(tuple(t.cpu().pin_memory() for t in (q, nk, nv)))
+        host.append(rows)
+    out_h = [torch.empty(tuple(b.q.shape), dtype=torch.bfloat16).pin_memory() for b in pools]
+    per_tok = [b.batch * b.num_kv_heads * b.head_dim * 2 * 2 for b in pools]
+    base = [b.algorithmic_bytes() for b in pools]
+    visits = [0] * R
+    h2d = sum(t.numel() * 2 for t in host[0][0])
+    d2h = out_h[0].numel() * 2
+
+    def step(i):
+        p = i % R
+        b = pools[p]
+        q, nk, nv = host[p][visits[p] % nrows]
+        comem.comem_decode_step_host(q, nk, nv, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                     b.softmax_scale, out_h[p], ws, stream=stream)
+        visits[p] += 1
+        return base[p] + visits[p] * per_tok[p]  # context grew by one token per earlier visit
+
+    for i in range(max(warmup, 3)):
+        step(i)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier()
+    torch.cuda.synchronize(device)
+    sampler.active = True
+    t0 = time.perf_counter()
+    e0.record(stream)
+    nbytes = 0
+    for i in range(steps):
+        nbytes += step(max(warmup, 3) + i)
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    sampler.active = False
+    replicas.barrier()
+    return max(e0.elapsed_time(e1), wall_ms), nbytes, h2d, d2h
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): the only places bench.py runs oracle/
+# ---------------------------------------------------------------------------------------------
+def oracle_inputs_cpu(batch, seqs):
+    """Gather the pages of sequences `seqs` into a compact CPU pool (pure data movement)."""
+    import torch
+    from paper_2605_30842_b200 import workloads as W
+
+    ps = batch.page_size
+    lens = batch.seq_lens.cpu()
+    ids, off = [], 0
+    maxp = max(1, max(W.pages_needed(int(lens[b]), ps) for b in seqs))
+    bt = torch.zeros((len(seqs), maxp), dtype=torch.int32)
+    for i, b in enumerate(seqs):
+        n = W.pages_needed(int(lens[b]), ps)
+        ids.append(batch.block_table[b, :n].to(torch.int64))
+        bt[i, :n] = torch.arange(off, off + n, dtype=torch.int32)
+        off += n
+    ids = torch.cat(ids)
+    sel = torch.tensor(list(seqs), dtype=torch.int64)
+    return (batch.q.cpu()[sel].contiguous(), batch.k_pages[ids.to(batch.k_pages.device)].cpu(),
+            batch.v_pages[ids.to(batch.v_pages.device)].cpu(), bt, lens[sel].contiguous())
+
+
+def cpu_baseline_and_parity(batch, gpu_out, budget_s=20.0):
+    """Time the oracle on a bounded sample of `batch` (all host cores) and compare the GPU's output
+    on the same rows.  Sample: whole sequences, first-come, until ~budget_s of CPU work."""
+    import numpy as np
+    import oracle
+
+    oracle.build()
+    cores = oracle.max_threads()
+    lens = [int(x) for x in batch.seq_lens.cpu()]
+    hq, g = batch.num_q_heads, batch.num_q_heads // batch.num_kv_heads
+    # calibrate on one row of sequence 0
+    q, kp, vp, bt, sl = oracle_inputs_cpu(batch, [0])
+    t0 = time.perf_counter()
+    oracle.decode_attn(q, kp, vp, bt, sl, batch.softmax_scale, pairs=[(0, 0)], num_threads=1)
+    row_s_per_tok = (time.perf_counter() - t0) / max(1, lens[0])
+    seqs, est = [], 0.0
+    for b, l in enumerate(lens):
+        cost = row_s_per_tok * l * hq / max(1, cores) * 1.5
+        if seqs and est + cost > budget_s:
+            break
+        seqs.append(b)
+        est += cost
+    if seqs != [0]:
+        q, kp, vp, bt, sl = oracle_inputs_cpu(batch, seqs)
+    reps = 3 if est * 3 <= budget_s else 1
+    best = float("inf")
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        ref, _ = oracle.decode_attn(q, kp, vp, bt, sl, batch.softmax_scale)
+        best = min(best, time.perf_counter() - t0)
+    toks = sum(lens[b] for b in seqs)
+    nbytes = toks * batch.num_kv_heads * batch.head_dim * 4 + len(seqs) * hq * batch.head_dim * 2
+    got = gpu_out[seqs].double().cpu().numpy()
+    d = np.abs(got - ref)
+    parity = {"rows": len(seqs) * hq, "max_abs": float(d.max()), "mean_abs": float(d.mean()),
+              "rel_l2": float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)),
+              "tol": {"max_abs": 2e-2, "mean_abs": 2e-3, "rel_l2": 5e-3}}
+    parity["ok"] = bool(parity["max_abs"] <= 2e-2 and parity["mean_abs"] <= 2e-3 and parity["rel_l2"] <= 5e-3)
+    base = {"value": nbytes / best / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(seqs)} of {len(lens)} sequences, all {hq} query heads, full context "
+                      f"({toks} tokens), best of {reps}; {best:.3f} s per pass",
+            "seconds": best}
+    return base, parity
+
+
+def run_reference(args, rank: int) -> int:
+    """--impl reference: the oracle, as it stands, on host cores, K steps of a bounded sample of the
+    same workload (rank 0 only; other ranks exit 0 without work)."""
+    if rank != 0:
+        return 0
+    import numpy as np  # noqa: F401
+    import oracle
+    from paper_2605_30842_b200 import workloads as W
+
+    oracle.build()
+    cores = oracle.max_threads()
+    desc = workload_desc(args.workload)
+    # The sample is a prefix of sequence 0's context, all query heads: T tokens chosen from a
+    # calibration pass so that (warmup + steps) passes fit the budget.
+    hq, hkv, d, ps = desc["num_q_heads"], desc["num_kv_heads"], desc["head_dim"], desc["page_size"]
+    full_ctx = {"c2": 32768, "c3": 36864, "c4": 131072}[args.workload]
+    calib = W.make_batch([4096], hq, hkv, d, ps, 4242, "cpu", k_scale=0.5 if args.workload == "c2" else 1.0)
+    oracle.decode_attn(calib.q, calib.k_pages, calib.v_pages, calib.block_table, calib.seq_lens, calib.softmax_scale)
+    t0 = time.perf_counter()
+    oracle.decode_attn(calib.q, calib.k_pages, calib.v_pages, calib.block_table, calib.seq_lens, calib.softmax_scale)
+    s_per_tok = (time.perf_counter() - t0) / 4096
+    n_pass = args.steps + max(args.warmup, 1)
+    T = int(min(full_ctx, max(ps, args.ref_budget_s / n_pass / s_per_tok / 1.3)))
+    T = max(ps, T // ps * ps)
+    b = W.make_batch([T], hq, hkv, d, ps, 1002, "cpu", k_scale=0.5 if args.workload == "c2" else 1.0,
+                     name=f"{args.workload}-prefix-{T}")
+    run = lambda: oracle.decode_attn(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale)  # noqa: E731
+    for _ in range(max(args.warmup, 1)):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    sec = time.perf_counter() - t0
+    nbytes = b.algorithmic_bytes()
+    value = nbytes * args.steps / sec / 1e9
+    cfg = dict(desc)
+    cfg["l2"] = "n/a (host)"
+    sample = (f"each step = all {hq} query heads over the first {T} of {full_ctx} tokens of one sequence "
+              f"({nbytes} algorithmic bytes), fp64 oracle, {cores} OpenMP threads")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": cfg, "gpu_launches": 0,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main() -> int:
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import replicas
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
+    rank, local_rank, world = replicas.init("nccl")
+    assert world == args.gpus or world == 1, f"--gpus {args.gpus} but WORLD_SIZE={world}"
+    device = torch.device("cuda", local_rank)
+    torch.cuda.set_device(device)
+    if rank == 0:
+        cuda_build.build()
+    replicas.barrier()
+    comem.load_library()
+
+    R_spare = 8 if args.workload == "c2" else 1
+    spare = (args.steps + max(args.warmup, 3)) // R_spare + 8
+    pools = make_pools(args.workload, device, rank, spare)
+    R = len(pools)
+    outs = [torch.empty_like(b.q) for b in pools]
+    ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table)
+    stream = torch.cuda.Stream(device)
+    step_bytes = [b.algorithmic_bytes() for b in pools]
+    kv_pool_bytes = sum(int(b.seq_lens.sum().item()) * b.num_kv_heads * b.head_dim * 4 for b in pools)
+    sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), local_rank)
+    sampler.start()
+
+    both = comem.COMEM_PHASE_SPLIT | comem.COMEM_PHASE_COMBINE
+    # one checked step on pool 0 first (also feeds the parity block)
+    with torch.cuda.stream(stream):
+        comem.comem_decode_attn_async(pools[0].q, pools[0].k_pages, pools[0].v_pages, pools[0].block_table,
+                                      pools[0].seq_lens, pools[0].softmax_scale, outs[0], ws, stream=stream)
+    stream.synchronize()
+    first_out = outs[0].clone()
+
+    ms = timed_steps(torch, comem, replicas, pools, outs, ws, stream, args.steps, args.warmup, both,
+                     not args.no_graph, sampler, device)
+    ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, args.steps, args.warmup,
+                           comem.COMEM_PHASE_SPLIT, not args.no_graph, sampler, device)
+    bytes_k_steps = sum(step_bytes[i % R] for i in range(args.steps))
+    ms_max = replicas.max_over_ranks(ms, device)
+    ms_split_max = replicas.max_over_ranks(ms_split, device)
+    total_bytes = replicas.sum_over_ranks(bytes_k_steps, device)
+
+    cpu_base, parity = None, None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_base, parity = cpu_baseline_and_parity(pools[0], first_out)
+
+    e2e_ms, e2e_bytes, h2d, d2h = timed_e2e(torch, comem, replicas, pools, ws, stream, args.steps, args.warmup,
+                                            sampler, device, 5000 + 1000 * rank)
+    e2e_ms_max = replicas.max_over_ranks(e2e_ms, device)
+    e2e_total = replicas.sum_over_ranks(e2e_bytes, device)
+    sampler.stop()
+
+    if rank == 0:
+        peak, peak_src = FALLBACK_PEAK_GBS, "fallback (B200_PROFILING.md)"
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                peak, peak_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+        except Exception:  # noqa: BLE001
+            pass
+        value = total_bytes / (ms_max * 1e-3) / 1e9
+        achieved = (bytes_k_steps / args.steps) / (ms_split_max / args.steps * 1e-3) / 1e9
+        cfg = workload_desc(args.workload)
+        cfg.update({"l2": (f"cold: steps rotate over {R} disjoint KV pools ({kv_pool_bytes / 2**30:.2f} GiB) > L2"
+                           if R > 1 else f"cold: one step reads {kv_pool_bytes / 2**30:.2f} GiB of KV >> L2"),
+                    "launch": "CUDA graph of %d steps, replayed" % R if not args.no_graph else "host launches",
+                    "algorithmic_bytes_per_step": bytes_k_steps // args.steps,
+                    "grid_ctas": comem.comem_grid_ctas(cfg["head_dim"]),
+                    "replicas": world})
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "us_per_step": ms_max / args.steps * 1e3,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+                "data": "synthetic", "config": cfg,
+                "frac_of_8TBps": value / world / 8000.0,
+                "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128>", "achieved": achieved,
+                             "peak": peak, "peak_source": peak_src, "unit": UNIT, "frac": achieved / peak,
+                             "us_per_launch": ms_split_max / args.steps * 1e3,
+                             "traffic": NCU_TRAFFIC_BYTES.get(args.workload)},
+                "e2e": {"value": e2e_total / (e2e_ms_max * 1e-3) / 1e9, "unit": UNIT,
+                        "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "us_per_step": e2e_ms_max / args.steps * 1e3,
+                        "api": "comem_decode_step_host (H2D q,k,v rows -> kv_append -> split -> combine -> D2H out, sync)"},
+                "gpu_launches": 2 * args.steps,
+                "clocks": sampler.summary()}
+        if cpu_base is not None:
+            line["cpu_baseline"] = cpu_base
+            line["parity"] = parity
+        print(json.dumps(line), flush=True)
+    replicas.finalize()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
