@@ -62,7 +62,8 @@ enum {
  * comem_decode_attn_async — enqueue one decode-attention step on `cuda_stream`.
  *
  * Enqueue-only: no host synchronisation, no device->host copy, no allocation;
- * safe inside CUDA-graph capture.  Launches 2 kernels (split-KV, combine).
+ * safe inside CUDA-graph capture.  Launches 1 kernel: the split-KV kernel, in which the
+ * last CTA to finish a cut (b, kv head) segment also runs the log-sum-exp combine for it.
  * Returns launch-time errors only.
  *
  *   q            device, bf16 [batch][num_q_heads][head_dim], contiguous
@@ -78,9 +79,13 @@ enum {
  *   lse_out      device, fp32 [batch][num_q_heads] natural-log log-sum-exp of the
  *                scaled logits, or NULL
  *   workspace    device scratch of >= comem_decode_attn_workspace_bytes(...) bytes,
- *                256-byte aligned.  Holds split partials; contents need no
- *                initialisation and are garbage afterwards.  Calls that may run
- *                concurrently (different streams) need DIFFERENT workspaces.
+ *                256-byte aligned.  Holds the per-segment arrival counters and the
+ *                split partials.  The counters must be zero when a call starts:
+ *                run comem_workspace_init_async once on a fresh (or foreign-written)
+ *                buffer; every call that completes leaves them zero again, so the
+ *                same workspace serves any number of later calls of any shape it is
+ *                large enough for.  Calls that may run concurrently (different
+ *                streams) need DIFFERENT workspaces.
  *   cuda_stream  a cudaStream_t (NULL = legacy default stream)
  */
 int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
@@ -91,13 +96,23 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                             size_t workspace_bytes, void *cuda_stream);
 
 /*
- * comem_decode_attn_phases_async — the same step with its two kernels selectable:
- * COMEM_PHASE_SPLIT runs K1 (page-gather + QK^T + online softmax + PV; writes finished rows
- * and the split partials into `workspace`), COMEM_PHASE_COMBINE runs K2 (LSE merge of the
- * partials in `workspace`; also writes the rows of empty sequences).  SPLIT|COMBINE is
- * comem_decode_attn_async.  Running the phases in separate calls (same arguments, same
- * workspace, same stream order) gives the identical result; bench.py uses SPLIT alone to time
- * the dominant kernel with CUDA events.
+ * comem_workspace_init_async — zero the arrival counters at the head of `workspace`
+ * (one cudaMemsetAsync of workspace_bytes' counter prefix on `cuda_stream`).  Needed once
+ * per buffer, before its first use (see `workspace` above).  The prefix length depends only
+ * on (batch, num_kv_heads); pass the largest shape the buffer will serve.
+ */
+int comem_workspace_init_async(void *workspace, size_t workspace_bytes, int batch, int num_q_heads,
+                               int num_kv_heads, int head_dim, void *cuda_stream);
+
+/*
+ * comem_decode_attn_phases_async — the same step with its two phases as separate kernels:
+ * COMEM_PHASE_SPLIT alone runs K1 un-fused (page-gather + QK^T + online softmax + PV; writes
+ * finished rows and the split partials into `workspace`, merges nothing), COMEM_PHASE_COMBINE
+ * alone runs K2 (stand-alone LSE merge of the partials in `workspace`; also writes the rows of
+ * empty sequences).  SPLIT|COMBINE is comem_decode_attn_async (one fused launch).  The
+ * two-call form (same arguments, same workspace, same stream order) gives a result within
+ * rounding of the fused one (K2 sums the partials in 4 interleaved stripes, the fused merge in
+ * plain split order); tests use it to check K2 and the partial format on their own.
  */
 enum { COMEM_PHASE_SPLIT = 1, COMEM_PHASE_COMBINE = 2 };
 int comem_decode_attn_phases_async(const void *q, const void *k_pages, const void *v_pages,

@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     comem_set_grid_ctas,
     comem_status_string,
     comem_version,
+    comem_workspace_init_async,
     library_path,
     load_library,
 )

@@ -57,6 +57,8 @@ def load_library():
     lib.comem_decode_attn.restype = i32
     lib.comem_decode_attn_workspace_bytes.argtypes = [i32] * 6
     lib.comem_decode_attn_workspace_bytes.restype = sz
+    lib.comem_workspace_init_async.argtypes = [vp, sz, i32, i32, i32, i32, vp]
+    lib.comem_workspace_init_async.restype = i32
     lib.comem_kv_append_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
     lib.comem_kv_append_async.restype = i32
     lib.comem_decode_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
@@ -115,11 +117,24 @@ def comem_decode_attn_workspace_bytes(batch: int, num_q_heads: int, num_kv_heads
         int(max_pages_per_seq)))
 
 
-def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.Tensor) -> torch.Tensor:
-    """torch.empty of the size the library asks for (device memory is torch's job)."""
+def comem_workspace_init_async(workspace: torch.Tensor, batch: int, num_q_heads: int, num_kv_heads: int,
+                               head_dim: int, stream=None) -> None:
+    st = load_library().comem_workspace_init_async(_ptr(workspace), workspace.numel(), int(batch),
+                                                   int(num_q_heads), int(num_kv_heads), int(head_dim),
+                                                   _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_workspace_init_async")
+
+
+def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.Tensor, stream=None) -> torch.Tensor:
+    """torch.empty of the size the library asks for (device memory is torch's job), then the
+    library's one-time comem_workspace_init_async on it (on `stream` or the current stream)."""
     n = comem_decode_attn_workspace_bytes(q.shape[0], q.shape[1], k_pages.shape[2], q.shape[2],
                                           k_pages.shape[1], block_table.shape[1])
-    return torch.empty(n, dtype=torch.uint8, device=q.device)
+    ws = torch.empty(n, dtype=torch.uint8, device=q.device)
+    with torch.cuda.device(q.device):
+        comem_workspace_init_async(ws, q.shape[0], q.shape[1], k_pages.shape[2], q.shape[2], stream)
+    return ws
 
 
 def _ptr(t: Optional[torch.Tensor]):

@@ -25,13 +25,15 @@ std::atomic<int> g_grid_override{0};
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct WorkspaceLayout {
-    size_t partials, q, new_k, new_v, out, lse, total;
+    size_t counters, partials, q, new_k, new_v, out, lse, total;
 };
 
 WorkspaceLayout workspace_layout(int batch, int hq, int hkv, int d)
 {
     WorkspaceLayout w;
     size_t off = 0;
+    w.counters = off;  // first, so that a buffer initialised for a large shape is initialised for smaller ones
+    off = align_up(off + (size_t)batch * hkv * sizeof(int), 256);
     w.partials = off;
     off = align_up(off + (size_t)2 * kMaxGridCtas * partial_stride_floats(d) * sizeof(float), 256);
     w.q = off;
@@ -170,6 +172,10 @@ int grid_for(int head_dim, int *grid)
     return COMEM_OK;
 }
 
+#ifdef COMEM_TRACE
+unsigned long long *g_trace = nullptr;
+#endif
+
 bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 }  // namespace
@@ -179,7 +185,7 @@ using namespace comem;
 
 extern "C" {
 
-int comem_version(void) { return 100; }
+int comem_version(void) { return 110; }
 
 const char *comem_status_string(int status)
 {
@@ -201,6 +207,26 @@ size_t comem_decode_attn_workspace_bytes(int batch, int num_q_heads, int num_kv_
     if (batch <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || head_dim <= 0) return 0;
     return workspace_layout(batch, num_q_heads, num_kv_heads, head_dim).total;
 }
+
+int comem_workspace_init_async(void *workspace, size_t workspace_bytes, int batch, int num_q_heads,
+                               int num_kv_heads, int head_dim, void *cuda_stream)
+{
+    if (batch <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || head_dim <= 0) return COMEM_ERR_INVALID_ARG;
+    const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
+    if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
+    const int st = check_device();
+    if (st != COMEM_OK) return st;
+    if (cudaMemsetAsync(static_cast<char *>(workspace) + wl.counters, 0, wl.partials - wl.counters,
+                        static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return COMEM_OK;
+}
+
+#ifdef COMEM_TRACE
+int comem_set_trace(void *buf) { g_trace = static_cast<unsigned long long *>(buf); return COMEM_OK; }
+#endif
 
 int comem_set_grid_ctas(int n)
 {
@@ -262,6 +288,12 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
     p.out = static_cast<__nv_bfloat16 *>(out);
     p.lse_out = lse_out;
     p.partials = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.partials);
+    p.seg_counters = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.counters);
+    const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
+    p.fuse_combine = fused ? 1 : 0;
+#ifdef COMEM_TRACE
+    p.trace = g_trace;
+#endif
     p.batch = batch;
     p.num_q_heads = num_q_heads;
     p.num_kv_heads = num_kv_heads;
@@ -277,7 +309,7 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }
-    if ((phases & COMEM_PHASE_COMBINE) && launch_combine(p, head_dim, stream) != cudaSuccess) {
+    if (!fused && (phases & COMEM_PHASE_COMBINE) && launch_combine(p, head_dim, stream) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }

@@ -14,6 +14,11 @@ struct DecodeParams {
     __nv_bfloat16 *out;          // [batch][Hq][D]
     float *lse_out;              // [batch][Hq] or nullptr
     float *partials;             // workspace: [2 * grid_ctas][partial_stride_floats(D)]
+    int *seg_counters;           // workspace: [batch][Hkv] arrival counters, zero between launches
+    int fuse_combine;            // 1: the last CTA to finish a cut segment merges it inside K1
+#ifdef COMEM_TRACE
+    unsigned long long *trace;   // development builds only: [grid][8] %globaltimer stamps per CTA
+#endif
     int batch;
     int num_q_heads;
     int num_kv_heads;

@@ -22,14 +22,16 @@
 #include "decode_params.cuh"
 #include "ptx.cuh"
 #include "schedule.cuh"
+#include "merge.cuh"
 
 namespace comem {
 
 namespace {
 
-constexpr int kConsumerWarps = 4;
+constexpr int kConsumerWarps = 8;
 constexpr int kConsumerThreads = kConsumerWarps * 32;
-constexpr int kThreads = kConsumerThreads + 32;
+constexpr int kProducerWarps = 2;  // one elected lane each; tiles alternate between them (issue-rate bound otherwise)
+constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
 constexpr unsigned kFull = 0xffffffffu;
 
 template <int D>
@@ -39,9 +41,15 @@ struct Cfg {
     // kStages % kConsumerWarps == 0 so that a ring stage always belongs to the same consumer warp:
     // a warp then never waits on a stage more than one phase ahead of the barrier (mbarrier waits
     // carry only the phase PARITY; out-of-order TMA completion could otherwise alias two phases).
-    static constexpr int kStages = (D == 128) ? 8 : 16;
+    static constexpr int kStages = (D == 128) ? 16 : 32;  // 128 KiB of K+V in flight per SM
     static_assert(kStages % kConsumerWarps == 0, "ring stages must map to a fixed consumer warp");
-    static constexpr int kScratchFloatsPerWarp = D * kMaxGroup + 3 * kMaxGroup;
+    static constexpr int kRowPitch = D + 4;                       // floats; see S6
+    static constexpr int kStateOff = kMaxGroup * kRowPitch;       // m[8], l[8], lx[8] follow the rows
+    static constexpr int kScratchFloatsPerWarp = kStateOff + 3 * kMaxGroup;
+    // the scratch area doubles as merge.cuh's staging area (never live at the same time)
+    static constexpr int kScratchBytes =
+        kConsumerWarps * kScratchFloatsPerWarp * 4 > MergeCfg<D>::kStageBytes
+            ? kConsumerWarps * kScratchFloatsPerWarp * 4 : MergeCfg<D>::kStageBytes;
     static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
 };
 
@@ -49,7 +57,7 @@ template <int D>
 __host__ __device__ constexpr size_t smem_bytes_for(int batch)
 {
     return 1024 /* alignment slack */ + (size_t)Cfg<D>::kStages * Cfg<D>::kStageBytes +
-           (size_t)kConsumerWarps * Cfg<D>::kScratchFloatsPerWarp * 4 + 2 * Cfg<D>::kStages * 8 +
+           (size_t)Cfg<D>::kScratchBytes + 2 * Cfg<D>::kStages * 8 +
            ((size_t)batch + 1) * 4 + 16;
 }
 
@@ -75,7 +83,7 @@ __device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch
 }
 
 template <int D>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, 1)
 decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                     const DecodeParams p)
 {
@@ -85,13 +93,16 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     const uint32_t ring = (raw + 1023u) & ~1023u;  // 1024-aligned: the 128B-swizzle atom
     uint8_t *ring_ptr = smem_raw + (ring - raw);
     float *scratch = reinterpret_cast<float *>(ring_ptr + C::kStages * C::kStageBytes);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(scratch + kConsumerWarps * C::kScratchFloatsPerWarp);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(scratch) + C::kScratchBytes);
     int *prefix = reinterpret_cast<int *>(bars + 2 * C::kStages);
     const uint32_t full0 = smem_u32(bars);
     const uint32_t empty0 = full0 + 8 * C::kStages;
 
+    __shared__ int s_merge[4];  // {this CTA merges?, first_slot, i_first, nsplit} of the segment just published
+
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    COMEM_STAMP(0);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
@@ -100,36 +111,83 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         }
         fence_mbar_init();
     }
-    if (warp == kConsumerWarps && lane == 0) {
+    if (warp == kConsumerWarps && lane == 0) {  // first producer warp
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
     }
-    // Everything above touched no global data; inputs may come from the previous kernel.
+    // Nothing above touched global data.  The inputs may still be written by the kernel running
+    // before this one (kv_append bumps seq_lens), so they are only READ after the wait -- but an L2
+    // prefetch is a hint on a coherent cache and may run now: the small control inputs (seq_lens,
+    // block table, q) are pulled from DRAM while the previous grid drains, and the dependent
+    // chain seq_lens -> block table -> first TMA below then runs at L2 latency.
+    {
+        const int64_t gtid = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+        if (gtid < (((int64_t)p.batch * 4 + 127) >> 7))
+            prefetch_l2(reinterpret_cast<const char *>(p.seq_lens) + (gtid << 7));
+        if (gtid < (((int64_t)p.batch * p.max_pages * 4 + 127) >> 7))
+            prefetch_l2(reinterpret_cast<const char *>(p.block_table) + (gtid << 7));
+        if (gtid < (((int64_t)p.batch * p.num_q_heads * D * 2 + 127) >> 7))
+            prefetch_l2(reinterpret_cast<const char *>(p.q) + (gtid << 7));
+    }
     pdl_wait_prior_grid();
+    COMEM_STAMP(1);
 
     // S1: exclusive prefix of tiles per sequence (warp 0), the whole schedule follows from it.
+    // Executed once per CTA on the critical path of the launch: kept small (no unrolling; the
+    // instruction fetch of cold straight-line code costs more than the arithmetic).
     if (warp == 0) {
-        const int per = (p.batch + 31) >> 5;
-        const int b0 = lane * per;
-        int sum = 0;
-        for (int i = 0; i < per; ++i)
-            if (b0 + i < p.batch) sum += tiles_of(p.seq_lens[b0 + i]);
-        int incl = sum;
+        if (p.batch <= 32) {
+            const int mine = lane < p.batch ? tiles_of(__ldg(p.seq_lens + lane)) : 0;
+            int incl = mine;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(kFull, incl, o);
-            if (lane >= o) incl += v;
-        }
-        int run = incl - sum;
-        for (int i = 0; i < per; ++i)
-            if (b0 + i < p.batch) {
-                prefix[b0 + i] = run;
-                run += tiles_of(p.seq_lens[b0 + i]);
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += v;
             }
-        if (lane == 31) prefix[p.batch] = incl;
+            if (lane < p.batch) prefix[lane] = incl - mine;
+            if (lane == 31) prefix[p.batch] = incl;
+        } else {
+            const int per = (p.batch + 31) >> 5;
+            const int b0 = lane * per;
+            int sum = 0;
+#pragma unroll 1
+            for (int i = 0; i < per; ++i)
+                if (b0 + i < p.batch) sum += tiles_of(__ldg(p.seq_lens + b0 + i));
+            int incl = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += v;
+            }
+            int run = incl - sum;
+#pragma unroll 1
+            for (int i = 0; i < per; ++i)
+                if (b0 + i < p.batch) {
+                    prefix[b0 + i] = run;
+                    run += tiles_of(__ldg(p.seq_lens + b0 + i));
+                }
+            if (lane == 31) prefix[p.batch] = incl;
+        }
     }
+#ifdef COMEM_TRACE
+    if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
+    if (p.trace && threadIdx.x == kConsumerThreads) p.trace[blockIdx.x * 16 + 12] = globaltimer_ns();
+    if (p.trace && threadIdx.x == 32) p.trace[blockIdx.x * 16 + 13] = globaltimer_ns();
+#endif
     __syncthreads();
     pdl_launch_dependents();
+    COMEM_STAMP(2);
+
+    // S8: rows of empty sequences (reading R9): +0.0 and lse = -inf, dealt round-robin to the CTAs.
+    if (p.fuse_combine) {
+        for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
+            if (prefix[b + 1] != prefix[b]) continue;
+            const int64_t row0 = (int64_t)b * p.num_q_heads;
+            for (int e = threadIdx.x; e < p.num_q_heads * D; e += kThreads) p.out[row0 * D + e] = __float2bfloat16_rn(0.f);
+            if (p.lse_out)
+                for (int h = threadIdx.x; h < p.num_q_heads; h += kThreads) p.lse_out[row0 + h] = -INFINITY;
+        }
+    }
 
     const int64_t total = (int64_t)p.num_kv_heads * prefix[p.batch];
     if (total == 0) return;
@@ -140,11 +198,16 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     const int64_t c1 = cta_begin(cta + 1, total, nc);
     if (c0 >= c1) return;
 
-    if (warp == kConsumerWarps) {
-        // ------------------------------ S2: page-gather producer ------------------------------
+    if (warp >= kConsumerWarps) {
+        // ------------------------------ S2: page-gather producers -----------------------------
+        // Producer warp pw issues the CTA's tiles with (CTA-local index) % kProducerWarps == pw; tile
+        // tl always lands in ring stage tl % kStages, in the ring's pass number tl / kStages.
+        static_assert((C::kStages & (C::kStages - 1)) == 0 && C::kStages % kProducerWarps == 0, "ring indexing");
+        constexpr int kStageShift = (C::kStages == 16) ? 4 : 5;
+        static_assert((1 << kStageShift) == C::kStages, "kStageShift");
+        const int pw = warp - kConsumerWarps;
         const int tiles_per_page_mask = (1 << p.page_tile_shift) - 1;
-        int stage = 0;
-        uint32_t phase = 0;
+        int tl0 = 0;  // CTA-local index of the current segment's first tile
         int64_t x = c0;
         while (x < c1) {
             const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
@@ -156,7 +219,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 int pid = 0;
                 if (base + lane < cnt) pid = __ldg(bt + (jj >> p.page_tile_shift));
                 const int m = cnt - base < 32 ? cnt - base : 32;
-                for (int i = 0; i < m; ++i) {
+                for (int i = ((tl0 + base) ^ pw) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
+                    const int tl = tl0 + base + i;
+                    const int stage = tl & (C::kStages - 1);
+                    const uint32_t phase = (uint32_t)(tl >> kStageShift) & 1u;
                     mbar_wait(empty0 + 8 * stage, phase ^ 1u);
                     const int pid_i = __shfl_sync(kFull, pid, i);
                     if (lane == 0) {
@@ -168,13 +234,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                         tma_load_4d(dst, &tm_k, bar, 0, row, 0, sp.kvh);
                         tma_load_4d(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh);
                     }
-                    if (++stage == C::kStages) {
-                        stage = 0;
-                        phase ^= 1u;
-                    }
                 }
             }
             x += cnt;
+            tl0 += cnt;
         }
         return;
     }
@@ -202,6 +265,14 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         const int64_t rem = c1 - x;
         const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
         const bool whole_segment = (sp.j == 0 && cnt == sp.T);
+        if (!whole_segment && p.fuse_combine && threadIdx.x == 0) {
+            // which CTAs cut this segment (64-bit divisions: done now, under the streaming, not in the tail)
+            const int64_t seg0 = x - sp.j, seg1 = seg0 + sp.T;
+            const int i_first = cta_of_tile(seg0, total, nc);
+            s_merge[1] = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
+            s_merge[2] = i_first;
+            s_merge[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
+        }
         const int seq_len = p.seq_lens[sp.b];
         const int head0 = sp.kvh * p.group;
 
@@ -227,6 +298,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 
         for (; t < n + cnt; t += kConsumerWarps) {
             mbar_wait(full0 + 8 * stage, phase);
+#ifdef COMEM_TRACE
+            if (t == 0) COMEM_STAMP(3);
+#endif
             const uint32_t k_base = ring + stage * C::kStageBytes;
             const uint32_t v_base = k_base + C::kTileBytes;
             const int valid = seq_len - ((sp.j + (t - n)) << kTileShift);  // >= 1; < 16 only on the last tile
@@ -307,69 +381,106 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             }
         }
 
-        // S6: merge the four warp states (warp-index order) and write the row or a partial.
+        // S6: merge the consumer warps' states (warp-index order) and write the row or a partial.
+        // Scratch layout per warp: acc as [head][D + 4] (the +4 pad makes both the fragment
+        // scatter below and the float4 row reads after the barrier bank-conflict free), then m, l, lx.
+        COMEM_STAMP(4);
         l_run += __shfl_xor_sync(kFull, l_run, 1);
         l_run += __shfl_xor_sync(kFull, l_run, 2);
         lx_run += __shfl_xor_sync(kFull, lx_run, 1);
         lx_run += __shfl_xor_sync(kFull, lx_run, 2);
+        {
+            float *lo = my_scratch + (2 * qlane) * C::kRowPitch + quad;
+            float *hi = lo + C::kRowPitch;
 #pragma unroll
-        for (int mt = 0; mt < C::kKSteps; ++mt) {
-            const int d = 16 * mt + quad;
-            *reinterpret_cast<float2 *>(my_scratch + d * kMaxGroup + 2 * qlane) = make_float2(acc[mt][0], acc[mt][1]);
-            *reinterpret_cast<float2 *>(my_scratch + (d + 8) * kMaxGroup + 2 * qlane) = make_float2(acc[mt][2], acc[mt][3]);
+            for (int mt = 0; mt < C::kKSteps; ++mt) {
+                lo[16 * mt] = acc[mt][0];
+                hi[16 * mt] = acc[mt][1];
+                lo[16 * mt + 8] = acc[mt][2];
+                hi[16 * mt + 8] = acc[mt][3];
+            }
         }
         if (qlane == 0) {
-            my_scratch[D * kMaxGroup + quad] = m_run;
-            my_scratch[D * kMaxGroup + kMaxGroup + quad] = l_run;
-            my_scratch[D * kMaxGroup + 2 * kMaxGroup + quad] = lx_run;
+            my_scratch[C::kStateOff + quad] = m_run;
+            my_scratch[C::kStateOff + kMaxGroup + quad] = l_run;
+            my_scratch[C::kStateOff + 2 * kMaxGroup + quad] = lx_run;
         }
         named_bar_sync(1, kConsumerThreads);
-        {
-            const int tid = threadIdx.x;       // 0..127
-            const int head = tid & (kMaxGroup - 1);
-            if (head < p.group) {
-                float mw[kConsumerWarps], M = -INFINITY;
+        if (warp < p.group) {  // warp w merges head w; lane -> one float4 of the row
+            const int head = warp;
+            float ww[kConsumerWarps], M = -INFINITY;
+#pragma unroll
+            for (int w = 0; w < kConsumerWarps; ++w) {
+                ww[w] = scratch[w * C::kScratchFloatsPerWarp + C::kStateOff + head];
+                M = fmaxf(M, ww[w]);
+            }
+            float den = 0.f, den_x = 0.f;
+#pragma unroll
+            for (int w = 0; w < kConsumerWarps; ++w) {
+                ww[w] = ex2(ww[w] - M);  // a warp that saw no tile has m = -inf -> weight 0
+                den += ww[w] * scratch[w * C::kScratchFloatsPerWarp + C::kStateOff + kMaxGroup + head];
+                den_x += ww[w] * scratch[w * C::kScratchFloatsPerWarp + C::kStateOff + 2 * kMaxGroup + head];
+            }
+            const int64_t row = (int64_t)sp.b * p.num_q_heads + head0 + head;
+            float *part = nullptr;
+            if (!whole_segment)
+                part = p.partials + (int64_t)(2 * cta + (x == c0 ? 0 : 1)) * partial_stride_floats(D);
+            if (lane < D / 4) {
+                float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
                 for (int w = 0; w < kConsumerWarps; ++w) {
-                    mw[w] = scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + head];
-                    M = fmaxf(M, mw[w]);
+                    const float4 a = *reinterpret_cast<const float4 *>(
+                        scratch + w * C::kScratchFloatsPerWarp + head * C::kRowPitch + 4 * lane);
+                    num.x += ww[w] * a.x; num.y += ww[w] * a.y; num.z += ww[w] * a.z; num.w += ww[w] * a.w;
                 }
-                float ww[kConsumerWarps], den = 0.f, den_x = 0.f;
-#pragma unroll
-                for (int w = 0; w < kConsumerWarps; ++w) {
-                    ww[w] = ex2(mw[w] - M);  // a warp that saw no tile has m = -inf -> weight 0
-                    den += ww[w] * scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + kMaxGroup + head];
-                    den_x += ww[w] * scratch[w * C::kScratchFloatsPerWarp + D * kMaxGroup + 2 * kMaxGroup + head];
+                if (whole_segment) {
+                    const float inv = 1.f / den;
+                    uint2 packed;
+                    packed.x = pack_bf16x2(num.x * inv, num.y * inv);
+                    packed.y = pack_bf16x2(num.z * inv, num.w * inv);
+                    *reinterpret_cast<uint2 *>(p.out + row * D + 4 * lane) = packed;
+                } else {
+                    *reinterpret_cast<float4 *>(part + head * D + 4 * lane) = num;
                 }
-                const int64_t row = (int64_t)sp.b * p.num_q_heads + head0 + head;
-                float *part = nullptr;
-                if (!whole_segment) {
-                    const int slot = 2 * cta + (x == c0 ? 0 : 1);
-                    part = p.partials + (int64_t)slot * partial_stride_floats(D);
-                }
-                const float inv = 1.f / den;
-#pragma unroll
-                for (int it = 0; it < D / 16; ++it) {
-                    const int d = (tid >> 3) + 16 * it;
-                    float num = 0.f;
-#pragma unroll
-                    for (int w = 0; w < kConsumerWarps; ++w)
-                        num += ww[w] * scratch[w * C::kScratchFloatsPerWarp + d * kMaxGroup + head];
-                    if (whole_segment) p.out[row * D + d] = __float2bfloat16_rn(num * inv);
-                    else part[head * D + d] = num;
-                }
-                if (tid < kMaxGroup) {
-                    if (whole_segment) {
-                        if (p.lse_out) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
-                    } else {
-                        part[kMaxGroup * D + head] = M;
-                        part[kMaxGroup * D + kMaxGroup + head] = den;
-                        part[kMaxGroup * D + 2 * kMaxGroup + head] = den_x;
-                    }
+            }
+            if (lane == 0) {
+                if (whole_segment) {
+                    if (p.lse_out) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
+                } else {
+                    part[kMaxGroup * D + head] = M;
+                    part[kMaxGroup * D + kMaxGroup + head] = den;
+                    part[kMaxGroup * D + 2 * kMaxGroup + head] = den_x;
                 }
             }
         }
+        if (!whole_segment && p.fuse_combine) {
+            // S7: publish the partial, take a ticket on the segment's arrival counter; the CTA that
+            // arrives last merges all of the segment's partials and re-arms the counter.
+            named_bar_sync(1, kConsumerThreads);  // every consumer's partial stores are issued
+            COMEM_STAMP(5);
+            if (threadIdx.x == 0) {
+                // release = fence + relaxed ticket (cumulative over the barrier above: the whole CTA's
+                // partial stores happen-before the ticket); acquire = ticket + fence, paid only by the
+                // CTA that merges.  The merge reads the partials with L2 (ld.cg) loads.
+                int *ctr = p.seg_counters + sp.b * p.num_kv_heads + sp.kvh;
+                fence_acq_rel_gpu();
+                const int ticket = atomicAdd(ctr, 1);
+                const int last = (ticket == s_merge[3] - 1);
+                if (last) {
+                    *ctr = 0;  // re-armed for the next launch (ordered by the kernel boundary)
+                    fence_acq_rel_gpu();
+                }
+                s_merge[0] = last;
+            }
+            named_bar_sync(1, kConsumerThreads);
+            COMEM_STAMP(6);
+            if (s_merge[0]) {
+                merge_partials<D>(p, warp, lane, s_merge[1], s_merge[2], s_merge[3],
+                                  (int64_t)sp.b * p.num_q_heads + head0, scratch);
+            }
+        }
         named_bar_sync(1, kConsumerThreads);
+        COMEM_STAMP(7);
 
         x += cnt;
         n += cnt;
@@ -410,7 +521,7 @@ cudaError_t split_default_grid(int head_dim, int *grid_ctas)
     }
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    if (per_sm > 2) per_sm = 2;
+    if (per_sm > 1) per_sm = 1;
     *grid_ctas = sms * per_sm;
     return cudaSuccess;
 }

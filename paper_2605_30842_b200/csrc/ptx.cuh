@@ -70,6 +70,26 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void *tmap,
         : "memory");
 }
 
+__device__ __forceinline__ void prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+__device__ __forceinline__ void fence_acq_rel_gpu()
+{
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+}
+
+// 16-byte asynchronous copy global -> shared, cached in L2 only
+__device__ __forceinline__ void cp_async_16(uint32_t dst_smem, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.wait_all;" ::: "memory");
+}
+
 // ---- tensor-core fragments ------------------------------------------------------------------
 __device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr)
 {
@@ -115,6 +135,18 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
 }
 __device__ __forceinline__ float bf16lo_to_f32(uint32_t v) { return __uint_as_float(v << 16); }
 __device__ __forceinline__ float bf16hi_to_f32(uint32_t v) { return __uint_as_float(v & 0xffff0000u); }
+
+#ifdef COMEM_TRACE
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)::"memory");
+    return t;
+}
+#define COMEM_STAMP(i) do { if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + (i)] = globaltimer_ns(); } while (0)
+#else
+#define COMEM_STAMP(i) do { } while (0)
+#endif
 
 // ---- named barriers (sub-CTA sync among the consumer warps) ----------------------------------
 __device__ __forceinline__ void named_bar_sync(int id, int threads)

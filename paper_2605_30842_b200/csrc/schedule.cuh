@@ -28,7 +28,7 @@ namespace comem {
 constexpr int kTileTokens = 16;
 constexpr int kTileShift = 4;
 // Fewer than this many tiles per CTA is not worth a partial + combine round trip.
-constexpr int kMinTilesPerCta = 8;
+constexpr int kMinTilesPerCta = 16;
 // Partial record per (CTA, slot): acc fp32 [8 heads][D] + m[8] + l[8] (rounded-p sum) + lx[8] (exact-p sum).
 constexpr int kMaxGroup = 8;
 // Largest batch the split kernel's shared-memory prefix table is sized for (== COMEM_MAX_BATCH).

@@ -22,7 +22,8 @@ def gpu_run(batch: W.DecodeBatch, want_lse: bool = True, stream=None, workspace=
     out = torch.full_like(batch.q, float("nan"))
     lse = torch.full((batch.batch, batch.num_q_heads), float("nan"), dtype=torch.float32,
                      device=batch.q.device) if want_lse else None
-    ws = workspace if workspace is not None else comem.alloc_workspace(batch.q, batch.k_pages, batch.block_table)
+    ws = workspace if workspace is not None else comem.alloc_workspace(batch.q, batch.k_pages, batch.block_table,
+                                                                        stream=stream)
     comem.comem_decode_attn_async(batch.q, batch.k_pages, batch.v_pages, batch.block_table,
                                   batch.seq_lens, batch.softmax_scale, out, ws, lse_out=lse, stream=stream)
     return out, lse

@@ -105,4 +105,4 @@ def test_schedule_partitions_tile_space(lib, lens, hkv, grid):
     sizes = np.diff(begins)
     assert (sizes >= 0).all() and sizes.max() - sizes.min() <= 1       # balanced to one tile
     nc = len(begins) - 1
-    assert nc == min(grid, max(1, -(-tiles // 8)))
+    assert nc == min(grid, max(1, -(-tiles // 16)))    # schedule.cuh kMinTilesPerCta = 16

@@ -198,3 +198,41 @@ def test_unsupported_and_invalid_raise():
     with pytest.raises(comem.ComemError) as e:
         gpu_run(b, workspace=torch.empty(1024, dtype=torch.uint8, device=DEV))
     assert e.value.status == comem.COMEM_ERR_WORKSPACE
+
+
+# ---- fused combine (S7 inside K1) vs the stand-alone K2 ---------------------------------------------------
+def test_fused_vs_two_phase_and_workspace_reuse(oracle):
+    """One workspace, initialised once for the largest shape, serves fused calls of several shapes
+    back to back (the arrival counters re-arm themselves); the two-call form SPLIT then COMBINE
+    (un-fused K1 + K2) agrees with the fused launch within rounding and with the oracle."""
+    big = W.make_batch([20000, 37, 0, 50001, 8191, 16, 300], 64, 8, 128, 16, seed=71, device=DEV)
+    small = W.make_batch([9000, 1], 8, 2, 64, 32, seed=72, device=DEV)
+    ws = comem.alloc_workspace(big.q, big.k_pages, big.block_table)
+    for rep in range(3):
+        for b in (big, small):
+            fused, lse_f = gpu_run(b, workspace=ws)
+            two = torch.full_like(b.q, float("nan"))
+            lse_t = torch.full_like(lse_f, float("nan"))
+            for ph in (comem.COMEM_PHASE_SPLIT, comem.COMEM_PHASE_COMBINE):
+                comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                                     b.softmax_scale, two, ws, lse_out=lse_t, phases=ph)
+            torch.cuda.synchronize()
+            ref, _ = oracle_rows(oracle, b, all_pairs(b))
+            assert_parity(errors(fused, ref, all_pairs(b)), f"fused rep{rep}")
+            assert_parity(errors(two, ref, all_pairs(b)), f"two-phase rep{rep}")
+            assert float((fused.float() - two.float()).abs().max()) <= 2.0 ** -7 * float(fused.float().abs().max())
+            live = torch.isfinite(lse_f)
+            assert torch.equal(live, torch.isfinite(lse_t))
+            assert float((lse_f[live] - lse_t[live]).abs().max()) < 1e-4
+
+
+def test_every_grid_size_same_answer(oracle):
+    """Sweep the persistent grid (1 CTA ... more CTAs than tiles): every cut pattern of the
+    segments goes through the fused merge and must match the oracle."""
+    b = W.make_batch([3000, 555, 16], 16, 2, 128, 16, seed=73, device=DEV, poison_unused=True)
+    try:
+        for g in (1, 2, 3, 5, 8, 13, 37, 64, 148, 296, 1024):
+            comem.comem_set_grid_ctas(g)
+            check_batch(oracle, b, what=f"grid {g}")
+    finally:
+        comem.comem_set_grid_ctas(0)
