@@ -24,12 +24,17 @@ template <int D>
 __global__ void __launch_bounds__(kCombineThreads)
 combine_kernel(const DecodeParams p)
 {
-    extern __shared__ __align__(16) float stage[];  // MergeCfg<D>::kStageBytes
+    extern __shared__ __align__(128) float stage[];  // MergeCfg<D>::kStageBytes
     __shared__ int s_before[kMaxGroup], s_total[kMaxGroup];
+    __shared__ __align__(8) uint64_t s_bar;
     const int b = blockIdx.x / p.num_kv_heads;
     const int kvh = blockIdx.x - b * p.num_kv_heads;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
+    if (tid == 0) {
+        mbar_init(smem_u32(&s_bar), 1);
+        fence_mbar_init();
+    }
     pdl_wait_prior_grid();  // seq_lens / partials come from the kernels launched just before
 
     // tiles before sequence b, and in total (block reduction over seq_lens)
@@ -70,7 +75,8 @@ combine_kernel(const DecodeParams p)
     if (i_first == i_last) return;  // one CTA owned the whole segment and wrote the rows itself
     // slot of split s: CTA i's first-segment slot (2i) unless the segment starts inside CTA i_first
     const int first_slot = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
-    merge_partials<D>(p, warp, lane, first_slot, i_first, i_last - i_first + 1, row0, stage);
+    uint32_t phase = 0;
+    merge_partials<D>(p, warp, lane, first_slot, i_first, i_last - i_first + 1, row0, stage, smem_u32(&s_bar), phase);
 }
 
 }  // namespace

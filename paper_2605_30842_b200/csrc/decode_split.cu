@@ -30,6 +30,7 @@ namespace {
 
 constexpr int kConsumerWarps = 8;
 constexpr int kConsumerThreads = kConsumerWarps * 32;
+static_assert(kConsumerWarps == kMaxGroup, "S6 and merge.cuh map warp w to query head w of the group");
 constexpr int kProducerWarps = 2;  // one elected lane each; tiles alternate between them (issue-rate bound otherwise)
 constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
 constexpr unsigned kFull = 0xffffffffu;
@@ -57,7 +58,7 @@ template <int D>
 __host__ __device__ constexpr size_t smem_bytes_for(int batch)
 {
     return 1024 /* alignment slack */ + (size_t)Cfg<D>::kStages * Cfg<D>::kStageBytes +
-           (size_t)Cfg<D>::kScratchBytes + 2 * Cfg<D>::kStages * 8 +
+           (size_t)Cfg<D>::kScratchBytes + (2 * Cfg<D>::kStages + 1) * 8 +
            ((size_t)batch + 1) * 4 + 16;
 }
 
@@ -94,9 +95,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     uint8_t *ring_ptr = smem_raw + (ring - raw);
     float *scratch = reinterpret_cast<float *>(ring_ptr + C::kStages * C::kStageBytes);
     uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(scratch) + C::kScratchBytes);
-    int *prefix = reinterpret_cast<int *>(bars + 2 * C::kStages);
+    int *prefix = reinterpret_cast<int *>(bars + 2 * C::kStages + 1);
     const uint32_t full0 = smem_u32(bars);
     const uint32_t empty0 = full0 + 8 * C::kStages;
+    const uint32_t merge_bar = empty0 + 8 * C::kStages;  // completion of merge.cuh's bulk copies
 
     __shared__ int s_merge[4];  // {this CTA merges?, first_slot, i_first, nsplit} of the segment just published
 
@@ -109,6 +111,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             mbar_init(full0 + 8 * s, 1);
             mbar_init(empty0 + 8 * s, 1);
         }
+        mbar_init(merge_bar, 1);
         fence_mbar_init();
     }
     if (warp == kConsumerWarps && lane == 0) {  // first producer warp
@@ -254,6 +257,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 
     float *my_scratch = scratch + warp * C::kScratchFloatsPerWarp;
 
+    uint32_t merge_phase = 0;
     int64_t x = c0;
     int n = 0;        // CTA-local index of the segment's first tile
     int t = warp;     // this warp's next tile (CTA-local index)
@@ -443,19 +447,17 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     *reinterpret_cast<float4 *>(part + head * D + 4 * lane) = num;
                 }
             }
-            if (lane == 0) {
-                if (whole_segment) {
-                    if (p.lse_out) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
-                } else {
-                    part[kMaxGroup * D + head] = M;
-                    part[kMaxGroup * D + kMaxGroup + head] = den;
-                    part[kMaxGroup * D + 2 * kMaxGroup + head] = den_x;
-                }
+            if (whole_segment) {
+                if (p.lse_out && lane == 0) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
+            } else if (lane < 2) {  // the head's state sector, written whole: {m, l, lx, 0} {0, 0, 0, 0}
+                *reinterpret_cast<float4 *>(part + kMaxGroup * D + 8 * head + 4 * lane) =
+                    lane == 0 ? make_float4(M, den, den_x, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
         if (!whole_segment && p.fuse_combine) {
             // S7: publish the partial, take a ticket on the segment's arrival counter; the CTA that
             // arrives last merges all of the segment's partials and re-arms the counter.
+            fence_proxy_async_smem();             // scratch (generic writes above) is the merge's TMA landing area
             named_bar_sync(1, kConsumerThreads);  // every consumer's partial stores are issued
             COMEM_STAMP(5);
             if (threadIdx.x == 0) {
@@ -476,7 +478,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             COMEM_STAMP(6);
             if (s_merge[0]) {
                 merge_partials<D>(p, warp, lane, s_merge[1], s_merge[2], s_merge[3],
-                                  (int64_t)sp.b * p.num_q_heads + head0, scratch);
+                                  (int64_t)sp.b * p.num_q_heads + head0, scratch, merge_bar, merge_phase);
             }
         }
         named_bar_sync(1, kConsumerThreads);

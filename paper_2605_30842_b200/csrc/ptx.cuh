@@ -90,6 +90,20 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
+// 1-D bulk copy global -> shared through the TMA unit, completion (bytes) on an mbarrier;
+// src, dst 16-byte aligned, bytes a multiple of 16
+__device__ __forceinline__ void bulk_load(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_global()
+{
+    // order this thread's earlier generic-proxy accesses to global memory before its later async-proxy
+    // (TMA) accesses to it; FENCE.VIEW.ASYNC.G only -- the state-space-less form adds a MEMBAR.GPU
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+}
+
 // ---- tensor-core fragments ------------------------------------------------------------------
 __device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr)
 {

@@ -29,7 +29,6 @@ constexpr int kTileTokens = 16;
 constexpr int kTileShift = 4;
 // Fewer than this many tiles per CTA is not worth a partial + combine round trip.
 constexpr int kMinTilesPerCta = 16;
-// Partial record per (CTA, slot): acc fp32 [8 heads][D] + m[8] + l[8] (rounded-p sum) + lx[8] (exact-p sum).
 constexpr int kMaxGroup = 8;
 // Largest batch the split kernel's shared-memory prefix table is sized for (== COMEM_MAX_BATCH).
 constexpr int kMaxBatch = 4096;
@@ -52,6 +51,8 @@ COMEM_HD int cta_of_tile(int64_t x, int64_t total_tiles, int nc)
     return (int)(((x + 1) * nc - 1) / total_tiles);
 }
 
-COMEM_HD int partial_stride_floats(int head_dim) { return kMaxGroup * head_dim + 3 * kMaxGroup; }
+// Partial record: acc fp32 [8 heads][D], then per head one 32-byte sector {m, l, lx, 0, 0, 0, 0, 0}
+// (a whole sector per head so that it is written by ONE store instruction and read by one load).
+COMEM_HD int partial_stride_floats(int head_dim) { return kMaxGroup * head_dim + 8 * kMaxGroup; }
 
 }  // namespace comem
