@@ -1,22 +1,32 @@
-// decode_split.cu — K1, the split-KV kernel: page-gather loader + QK^T + online softmax + PV
-// (SURVEY.md §8(a) S1..S6) for one decode step of paged GQA attention (PAPER.md L49, L61).
+// decode_split.cu — K1, the whole decode-attention step in one launch: split-KV scheduler,
+// page-gather loader, QK^T, online softmax, PV, partial write and (fused) the log-sum-exp combine
+// (SURVEY.md §8(a) S1..S8) for one decode step of paged GQA attention (PAPER.md L49, L61).
 //
 // Shape of the kernel (sm_100a):
-//   * persistent grid, one contiguous range of 16-token tiles per CTA (schedule.cuh);
-//   * warp 4 = producer: reads the block table 32 entries at a time and issues, per tile,
-//     one TMA tiled load for K and one for V ([16 tokens][D] of one kv head, 128-byte
-//     swizzle) into a kStages-deep shared-memory ring guarded by full/empty mbarriers —
-//     up to kStages * 8 KiB in flight per CTA, two CTAs per SM;
-//   * warps 0..3 = consumers: tile n of the CTA goes to warp n % 4, so four independent
+//   * persistent grid, ONE CTA per SM (10 warps, ~214 KiB of shared memory), one contiguous range
+//     of 16-token tiles per CTA (schedule.cuh);
+//   * before griddepcontrol.wait: mbarrier init, tensor-map prefetch and an L2 prefetch of the
+//     small control inputs (seq_lens, block table, q) -- they overlap the previous kernel's tail;
+//   * warps 8, 9 = producers: each reads the block table 32 entries at a time and issues, for
+//     every other tile of the CTA, one TMA tiled load for K and one for V ([16 tokens][D] of one kv
+//     head, 128-byte swizzle) into a 16-stage shared-memory ring guarded by full/empty
+//     mbarriers -- 128 KiB of K+V in flight per SM (one producer lane is issue-rate bound);
+//   * warps 0..7 = consumers: tile n of the CTA goes to warp n % 8, so eight independent
 //     online-softmax states stream concurrently.  Per tile and warp:
 //        S[G(pad 16) x 16 tok] = Q_g K^T      mma.sync m16n8k16 (Q fragments live in registers)
 //        m, p = online softmax in the log2 domain (quad shuffles for the row max)
 //        O^T[D x G] += V^T P^T                mma.sync with V^T via ldmatrix.trans; P is
 //                                             rounded to bf16 and l sums the ROUNDED p, so
 //                                             out is an exact weighted mean of V rows;
-//   * at the end of a (b, kv head) segment the four warp states are merged through shared
-//     memory in warp-index order and either written as the final bf16 row (the CTA owned the
-//     whole segment) or as an fp32 partial (acc, m, l) for the combine kernel.
+//   * S6, at the end of a (b, kv head) segment: the eight warp states are merged through shared
+//     memory in warp-index order (warp w -> query head w, lane -> one float4 of the row) and
+//     either written as the final bf16 row (the CTA owned the whole segment) or as an fp32
+//     partial record (acc[8][D], then one 32-byte state sector {m, l, lx} per head);
+//   * S7, fused: the CTA then fences, takes a ticket on the segment's arrival counter, and the
+//     CTA that arrives LAST pulls all of the segment's records with TMA bulk copies and merges
+//     them in CTA-index order (merge.cuh), re-arming the counter for the next launch.  No CTA
+//     ever waits for another one.  With fuse_combine == 0 the kernel stops after S6 and the
+//     stand-alone K2 (combine.cu) does the merge.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
 #include "decode_params.cuh"
