@@ -13,8 +13,9 @@ What the ONE JSON line on stdout holds (rank 0):
   roofline             the dominant (only) kernel: algorithmic bytes per launch / its average launch
                        duration over the timed region, against MEASURED_PEAKS.json's hbm_gbs; the un-fused
                        split phase timed alone is reported beside it as `split_only_us`
-  e2e                  the same metric through comem_decode_step_host: every step copies q and the new
-                       (k, v) rows from pinned host memory, appends, attends, copies out back
+  e2e                  the same metric through comem_decode_step_host: every step brings q and the new
+                       (k, v) rows from pinned host memory, appends, attends, and lands out in host memory
+                       (the kernels move those bytes themselves over the host link), host-synchronous
   cpu_baseline         the fp64 oracle (oracle/, test infrastructure) on this box's host cores
   parity               GPU vs oracle on the bench's own inputs (max-abs / mean-abs / rel-l2)
 
@@ -458,7 +459,7 @@ def main() -> int:
                 "e2e": {"value": e2e_total / (e2e_ms_max * 1e-3) / 1e9, "unit": UNIT,
                         "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "us_per_step": e2e_ms_max / args.steps * 1e3,
-                        "api": "comem_decode_step_host (H2D q,k,v rows -> kv_append -> fused split+combine -> D2H out, sync)"},
+                        "api": "comem_decode_step_host, pinned host buffers: K3 reads the q,k,v rows over the host link and appends -> fused split+combine stores out into host memory -> stream synchronize (2 launches, no copy engine)"},
                 "gpu_launches": args.steps,
                 "clocks": sampler.summary()}
         if cpu_base is not None:

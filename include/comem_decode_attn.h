@@ -162,8 +162,14 @@ int comem_kv_append_async(void *k_pages, void *v_pages, const int32_t *block_tab
  *   lse_host                host, fp32 [batch][num_q_heads], or NULL
  *   k_pages, v_pages, block_table, seq_lens, workspace: device, as above
  *
- * Sequence on `cuda_stream`: H2D(q, new_k, new_v) -> kv_append -> decode_attn ->
- * D2H(out[, lse]) -> cudaStreamSynchronize.  Returns execution errors too.
+ * Two paths, chosen per call with cudaPointerGetAttributes:
+ *   - every host buffer is PINNED and device-mapped (cudaHostAlloc / cudaHostRegister): the kernels
+ *     move the bytes themselves -- K3 reads q / new_k / new_v over the host link (q is staged in
+ *     the workspace), the attention kernel stores out (and lse) straight into host memory;
+ *     2 launches + cudaStreamSynchronize, no copy engine;
+ *   - otherwise (pageable memory): cudaMemcpyAsync H2D(q, new_k, new_v) -> kv_append -> decode_attn
+ *     -> cudaMemcpyAsync D2H(out[, lse]) -> cudaStreamSynchronize.
+ * Both are host-synchronous and return execution errors too.
  */
 int comem_decode_step_host(const void *q_host, const void *new_k_host, const void *new_v_host,
                            void *k_pages, void *v_pages, const int32_t *block_table,

@@ -176,6 +176,16 @@ int grid_for(int head_dim, int *grid)
 unsigned long long *g_trace = nullptr;
 #endif
 
+// Is this host pointer pinned AND mapped into the device address space?  If so return the device
+// alias (identical under UVA, but ask anyway).
+void *device_alias(const void *host_ptr)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, host_ptr) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (at.type != cudaMemoryTypeHost || at.devicePointer == nullptr) return nullptr;
+    return at.devicePointer;
+}
+
 bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 }  // namespace
@@ -380,6 +390,36 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
     char *ws = static_cast<char *>(workspace);
     const size_t q_bytes = (size_t)batch * num_q_heads * head_dim * 2;
     const size_t kv_bytes = (size_t)batch * num_kv_heads * head_dim * 2;
+    // Fast path: every host buffer is pinned and device-mapped (cudaHostAlloc / cudaHostRegister, what
+    // torch's pin_memory() gives).  The kernels then move the step's bytes themselves: K3 reads the
+    // q / k / v rows over the host link (staging q in the workspace), the attention kernel writes out
+    // (and lse) straight into host memory -- 2 launches + 1 synchronize, no cudaMemcpyAsync.
+    {
+        void *dq = device_alias(q_host), *dout = device_alias(out_host);
+        void *dk = new_k_host ? device_alias(new_k_host) : nullptr;
+        void *dv = new_v_host ? device_alias(new_v_host) : nullptr;
+        void *dlse = lse_host ? device_alias(lse_host) : nullptr;
+        const bool mapped = dq && dout && (!new_k_host || (dk && dv)) && (!lse_host || dlse) &&
+                            aligned(dq, 16) && aligned(dout, 16) && (!dk || (aligned(dk, 16) && aligned(dv, 16)));
+        if (mapped) {
+            if (!k_pages || !v_pages || !block_table || !seq_lens) return COMEM_ERR_INVALID_ARG;
+            if (launch_kv_append(static_cast<__nv_bfloat16 *>(k_pages), static_cast<__nv_bfloat16 *>(v_pages),
+                                 block_table, seq_lens, static_cast<const __nv_bfloat16 *>(dk),
+                                 static_cast<const __nv_bfloat16 *>(dv), num_kv_heads * head_dim, page_size, batch,
+                                 max_pages_per_seq, stream, static_cast<const __nv_bfloat16 *>(dq),
+                                 reinterpret_cast<__nv_bfloat16 *>(ws + wl.q), num_q_heads * head_dim) != cudaSuccess) {
+                cudaGetLastError();
+                return COMEM_ERR_CUDA;
+            }
+            st = comem_decode_attn_async(ws + wl.q, k_pages, v_pages, block_table, seq_lens, num_q_heads,
+                                         num_kv_heads, head_dim, page_size, softmax_scale, dout, batch,
+                                         max_pages_per_seq, num_pages, static_cast<float *>(dlse), workspace,
+                                         workspace_bytes, cuda_stream);
+            if (st != COMEM_OK) return st;
+            if (cudaStreamSynchronize(stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+            return COMEM_OK;
+        }
+    }
     bool ok = cudaMemcpyAsync(ws + wl.q, q_host, q_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess;
     if (ok && new_k_host) {
         ok = cudaMemcpyAsync(ws + wl.new_k, new_k_host, kv_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess &&

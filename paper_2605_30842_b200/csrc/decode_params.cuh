@@ -37,7 +37,9 @@ cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t str
 cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
                              const int32_t *block_table, int32_t *seq_lens,
                              const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v, int row_elems,
-                             int page_size, int batch, int max_pages, cudaStream_t stream);
+                             int page_size, int batch, int max_pages, cudaStream_t stream,
+                             const __nv_bfloat16 *q_src = nullptr, __nv_bfloat16 *q_dst = nullptr,
+                             int q_row_elems = 0);
 // occupancy-derived persistent grid for the split kernel on the current device
 cudaError_t split_default_grid(int head_dim, int *grid_ctas);
 size_t split_smem_bytes(int head_dim, int batch);

@@ -219,6 +219,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         constexpr int kStageShift = (C::kStages == 16) ? 4 : 5;
         static_assert((1 << kStageShift) == C::kStages, "kStageShift");
         const int pw = warp - kConsumerWarps;
+        // K/V bytes are used once per step: evict-first keeps them from displacing the L2-resident
+        // control data, partial records and whatever else the model keeps there between steps
+        const uint64_t stream_policy = l2_policy_evict_first();
         const int tiles_per_page_mask = (1 << p.page_tile_shift) - 1;
         int tl0 = 0;  // CTA-local index of the current segment's first tile
         int64_t x = c0;
@@ -244,8 +247,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                         const uint32_t dst = ring + stage * C::kStageBytes;
                         const uint32_t bar = full0 + 8 * stage;
                         mbar_arrive_expect_tx(bar, C::kStageBytes);
-                        tma_load_4d(dst, &tm_k, bar, 0, row, 0, sp.kvh);
-                        tma_load_4d(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh);
+                        tma_load_4d_hint(dst, &tm_k, bar, 0, row, 0, sp.kvh, stream_policy);
+                        tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh, stream_policy);
                     }
                 }
             }

@@ -2,6 +2,10 @@
 // corrected per DESIGN.md reading R3).  One CTA per sequence copies the new token's
 // [Hkv][D] K row and V row (contiguous in the paged layout) into slot seq_len % page_size of
 // page block_table[b][seq_len / page_size] with 16-byte stores, then bumps seq_lens[b].
+// The same CTA can also stage sequence b's query rows (q_src -> q_dst, 16-byte copies): on the
+// end-to-end path (comem_decode_step_host) new_k / new_v / q_src are device-mapped PINNED HOST
+// pointers, so this one kernel is the whole host->device leg of a step (zero-copy reads over the
+// host link) instead of three cudaMemcpyAsync calls.
 #include "decode_params.cuh"
 #include "ptx.cuh"
 
@@ -12,10 +16,17 @@ namespace {
 __global__ void __launch_bounds__(128)
 kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *block_table,
                  int32_t *seq_lens, const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v,
-                 int row_elems, int page_size, int max_pages)
+                 int row_elems, int page_size, int max_pages, const __nv_bfloat16 *q_src,
+                 __nv_bfloat16 *q_dst, int q_row_elems)
 {
     pdl_wait_prior_grid();
     const int b = blockIdx.x;
+    if (q_src != nullptr) {
+        const uint4 *s = reinterpret_cast<const uint4 *>(q_src + (int64_t)b * q_row_elems);
+        uint4 *d = reinterpret_cast<uint4 *>(q_dst + (int64_t)b * q_row_elems);
+        for (int i = threadIdx.x; i < q_row_elems / 8; i += blockDim.x) d[i] = s[i];
+    }
+    if (new_k == nullptr) return;
     const int t = seq_lens[b];
     const int page = t / page_size;
     const int slot = t - page * page_size;
@@ -38,10 +49,11 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
 
 cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *block_table,
                              int32_t *seq_lens, const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v,
-                             int row_elems, int page_size, int batch, int max_pages, cudaStream_t stream)
+                             int row_elems, int page_size, int batch, int max_pages, cudaStream_t stream,
+                             const __nv_bfloat16 *q_src, __nv_bfloat16 *q_dst, int q_row_elems)
 {
     kv_append_kernel<<<batch, 128, 0, stream>>>(k_pages, v_pages, block_table, seq_lens, new_k, new_v,
-                                               row_elems, page_size, max_pages);
+                                               row_elems, page_size, max_pages, q_src, q_dst, q_row_elems);
     return cudaGetLastError();
 }
 

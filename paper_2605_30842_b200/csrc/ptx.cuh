@@ -59,14 +59,21 @@ __device__ __forceinline__ void tma_prefetch_desc(const void *tmap)
 {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
-__device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void *tmap, uint32_t bar,
-                                            int c0, int c1, int c2, int c3)
+// L2 eviction-priority hint (createpolicy) for the load below: the KV stream is read exactly once per step
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_load_4d_hint(uint32_t dst_smem, const void *tmap, uint32_t bar,
+                                                 int c0, int c1, int c2, int c3, uint64_t policy)
 {
     asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
-        " [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
         ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1),
-        "r"(c2), "r"(c3)
+        "r"(c2), "r"(c3), "l"(policy)
         : "memory");
 }
 
@@ -78,16 +85,6 @@ __device__ __forceinline__ void prefetch_l2(const void *p)
 __device__ __forceinline__ void fence_acq_rel_gpu()
 {
     asm volatile("fence.acq_rel.gpu;" ::: "memory");
-}
-
-// 16-byte asynchronous copy global -> shared, cached in L2 only
-__device__ __forceinline__ void cp_async_16(uint32_t dst_smem, const void *src)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all()
-{
-    asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
 // 1-D bulk copy global -> shared through the TMA unit, completion (bytes) on an mbarrier;

@@ -189,6 +189,30 @@ def test_decode_step_host(oracle):
     assert np.max(np.abs(lse_h.numpy().reshape(-1) - ref_lse)) < 1e-3
 
 
+def test_decode_step_host_pageable_fallback(oracle):
+    """Pageable (un-pinned) host buffers take the cudaMemcpyAsync path; same answer as the zero-copy path."""
+    outs = []
+    for pinned in (True, False):
+        b = W.make_batch([4000, 333, 16], 32, 8, 128, 32, seed=65, device=DEV, spare_tokens=4)
+        ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+        q, nk, nv = (t.cpu() for t in W.decode_step_rows(b, 0, 6500))
+        out_h = torch.empty_like(q)
+        lse_h = torch.empty((3, 32), dtype=torch.float32)
+        if pinned:
+            q, nk, nv, out_h, lse_h = (t.pin_memory() for t in (q, nk, nv, out_h, lse_h))
+        for step in range(2):   # second call: no append (k, v = None)
+            comem.comem_decode_step_host(q, nk if step == 0 else None, nv if step == 0 else None, b.k_pages,
+                                         b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, out_h, ws,
+                                         lse_host=lse_h)
+        assert b.seq_lens.cpu().tolist() == [4001, 334, 17]
+        outs.append((out_h.clone(), lse_h.clone()))
+        b2 = W.DecodeBatch(q=q.to(DEV), k_pages=b.k_pages, v_pages=b.v_pages, block_table=b.block_table,
+                           seq_lens=b.seq_lens, softmax_scale=b.softmax_scale)
+        ref, _ = oracle_rows(oracle, b2, all_pairs(b2))
+        assert_parity(errors(out_h.to(DEV), ref, all_pairs(b2)), f"step_host pinned={pinned}")
+    assert torch.equal(bits(outs[0][0]), bits(outs[1][0])) and torch.equal(outs[0][1], outs[1][1])
+
+
 def test_unsupported_and_invalid_raise():
     b = W.make_batch([100], 16, 1, 128, 16, seed=64, device=DEV)                # group 16
     with pytest.raises(comem.ComemError) as e:
