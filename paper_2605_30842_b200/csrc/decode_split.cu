@@ -110,11 +110,20 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     const uint32_t empty0 = full0 + 8 * C::kStages;
     const uint32_t merge_bar = empty0 + 8 * C::kStages;  // completion of merge.cuh's bulk copies
 
-    __shared__ int s_merge[4];  // {this CTA merges?, first_slot, i_first, nsplit} of the segment just published
+    // A CTA cuts at most two segments: its first (slot 0) and its last (slot 1; slot 0 if it has one segment only).
+    // Per slot: {this CTA merges?, first_slot, i_first, nsplit, arrival counter index, first output row}.
+    __shared__ int s_seg[2][6];
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     COMEM_STAMP(0);
+#ifdef COMEM_TRACE
+    if (p.trace && threadIdx.x == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        p.trace[blockIdx.x * 16 + 15] = smid;
+    }
+#endif
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
@@ -271,6 +280,40 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     float *my_scratch = scratch + warp * C::kScratchFloatsPerWarp;
 
     uint32_t merge_phase = 0;
+    bool pending_first = false;  // slot 0's ticket was taken in mid-stream; its outcome is in s_seg[0][0]
+
+    // S7: publish the stored partial, take a ticket on the segment's arrival counter; the CTA that
+    // arrives LAST on a segment merges all of that segment's partials and re-arms the counter.
+    // release = fence + relaxed ticket (cumulative over a barrier: the whole CTA's partial stores
+    // happen-before the ticket); acquire = ticket + fence, paid only by a CTA that merges.
+    // `have_first`: slot 0's ticket was already taken in mid-stream (see the segment loop); if it
+    // turned out to be the last one, its merge is done here too.
+    auto publish_and_merge = [&](bool have_first, bool do_cur, int cur_slot) {
+        fence_proxy_async_smem();             // scratch (generic writes in S6) is the merge's TMA landing area
+        named_bar_sync(1, kConsumerThreads);  // every consumer's partial stores are issued
+        COMEM_STAMP(5);
+        if (threadIdx.x == 0) {
+            int last1 = 0;
+            if (do_cur) {
+                int *ctr = p.seg_counters + s_seg[cur_slot][4];
+                fence_acq_rel_gpu();
+                last1 = atomicAdd(ctr, 1) == s_seg[cur_slot][3] - 1;
+                if (last1) *ctr = 0;  // re-armed for the next launch (ordered by the kernel boundary)
+                s_seg[cur_slot][0] = last1;
+            }
+            if (last1 || (have_first && s_seg[0][0])) fence_acq_rel_gpu();
+        }
+        named_bar_sync(1, kConsumerThreads);
+        COMEM_STAMP(6);
+        if (have_first && s_seg[0][0]) {
+            merge_partials<D>(p, warp, lane, s_seg[0][1], s_seg[0][2], s_seg[0][3], (int64_t)s_seg[0][5], scratch,
+                              merge_bar, merge_phase);
+            if (do_cur) named_bar_sync(1, kConsumerThreads);  // the staging area is reused below
+        }
+        if (do_cur && s_seg[cur_slot][0])
+            merge_partials<D>(p, warp, lane, s_seg[cur_slot][1], s_seg[cur_slot][2], s_seg[cur_slot][3],
+                              (int64_t)s_seg[cur_slot][5], scratch, merge_bar, merge_phase);
+    };
     int64_t x = c0;
     int n = 0;        // CTA-local index of the segment's first tile
     int t = warp;     // this warp's next tile (CTA-local index)
@@ -286,9 +329,12 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             // which CTAs cut this segment (64-bit divisions: done now, under the streaming, not in the tail)
             const int64_t seg0 = x - sp.j, seg1 = seg0 + sp.T;
             const int i_first = cta_of_tile(seg0, total, nc);
-            s_merge[1] = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
-            s_merge[2] = i_first;
-            s_merge[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
+            int *sg = s_seg[x == c0 ? 0 : 1];
+            sg[1] = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
+            sg[2] = i_first;
+            sg[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
+            sg[4] = sp.b * p.num_kv_heads + sp.kvh;
+            sg[5] = sp.b * p.num_q_heads + sp.kvh * p.group;
         }
         const int seq_len = p.seq_lens[sp.b];
         const int head0 = sp.kvh * p.group;
@@ -467,39 +513,36 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     lane == 0 ? make_float4(M, den, den_x, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
+        bool early_ticket = false;
         if (!whole_segment && p.fuse_combine) {
-            // S7: publish the partial, take a ticket on the segment's arrival counter; the CTA that
-            // arrives last merges all of the segment's partials and re-arms the counter.
-            fence_proxy_async_smem();             // scratch (generic writes above) is the merge's TMA landing area
-            named_bar_sync(1, kConsumerThreads);  // every consumer's partial stores are issued
-            COMEM_STAMP(5);
-            if (threadIdx.x == 0) {
-                // release = fence + relaxed ticket (cumulative over the barrier above: the whole CTA's
-                // partial stores happen-before the ticket); acquire = ticket + fence, paid only by the
-                // CTA that merges.  The merge reads the partials with L2 (ld.cg) loads.
-                int *ctr = p.seg_counters + sp.b * p.num_kv_heads + sp.kvh;
-                fence_acq_rel_gpu();
-                const int ticket = atomicAdd(ctr, 1);
-                const int last = (ticket == s_merge[3] - 1);
-                if (last) {
-                    *ctr = 0;  // re-armed for the next launch (ordered by the kernel boundary)
-                    fence_acq_rel_gpu();
-                }
-                s_merge[0] = last;
-            }
-            named_bar_sync(1, kConsumerThreads);
-            COMEM_STAMP(6);
-            if (s_merge[0]) {
-                merge_partials<D>(p, warp, lane, s_merge[1], s_merge[2], s_merge[3],
-                                  (int64_t)sp.b * p.num_q_heads + head0, scratch, merge_bar, merge_phase);
+            // S7.  A cut segment that is not the CTA's last one (i.e. its first, with tiles of other
+            // segments still to stream) must not stall the stream for the fence / ticket / merge round
+            // trips (~3 us): thread 0 alone takes its ticket after the barrier below while the other
+            // warps go on with the next segment; in mid-stream this CTA is practically never the last
+            // arriver, and if it is, the merge waits until the CTA's end.
+            if (x + cnt < c1) early_ticket = true;
+            else {
+                publish_and_merge(pending_first, true, x == c0 ? 0 : 1);
+                pending_first = false;
             }
         }
         named_bar_sync(1, kConsumerThreads);
+        if (early_ticket) {
+            pending_first = true;
+            if (threadIdx.x == 0) {
+                int *ctr = p.seg_counters + s_seg[0][4];
+                fence_acq_rel_gpu();  // after the barrier: covers every consumer's partial stores
+                const int last0 = atomicAdd(ctr, 1) == s_seg[0][3] - 1;
+                if (last0) *ctr = 0;
+                s_seg[0][0] = last0;
+            }
+        }
         COMEM_STAMP(7);
 
         x += cnt;
         n += cnt;
     }
+    if (pending_first) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
 }
 
 template <int D>
