@@ -25,7 +25,7 @@ std::atomic<int> g_grid_override{0};
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct WorkspaceLayout {
-    size_t counters, partials, q, new_k, new_v, out, lse, total;
+    size_t counters, part_acc, part_state, q, new_k, new_v, out, lse, total;
 };
 
 WorkspaceLayout workspace_layout(int batch, int hq, int hkv, int d)
@@ -34,8 +34,10 @@ WorkspaceLayout workspace_layout(int batch, int hq, int hkv, int d)
     size_t off = 0;
     w.counters = off;  // first, so that a buffer initialised for a large shape is initialised for smaller ones
     off = align_up(off + (size_t)batch * hkv * sizeof(int), 256);
-    w.partials = off;
-    off = align_up(off + (size_t)2 * kMaxGridCtas * partial_stride_floats(d) * sizeof(float), 256);
+    w.part_acc = off;
+    off = align_up(off + (size_t)2 * kMaxGridCtas * record_floats(d) * sizeof(float), 256);
+    w.part_state = off;
+    off = align_up(off + (size_t)2 * kMaxGridCtas * kStateFloats * sizeof(float), 256);
     w.q = off;
     off = align_up(off + (size_t)batch * hq * d * 2, 256);
     w.new_k = off;
@@ -226,7 +228,7 @@ int comem_workspace_init_async(void *workspace, size_t workspace_bytes, int batc
     if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
     const int st = check_device();
     if (st != COMEM_OK) return st;
-    if (cudaMemsetAsync(static_cast<char *>(workspace) + wl.counters, 0, wl.partials - wl.counters,
+    if (cudaMemsetAsync(static_cast<char *>(workspace) + wl.counters, 0, wl.part_acc - wl.counters,
                         static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
@@ -297,7 +299,9 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
     p.seq_lens = seq_lens;
     p.out = static_cast<__nv_bfloat16 *>(out);
     p.lse_out = lse_out;
-    p.partials = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.partials);
+    p.part_acc = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.part_acc);
+    p.part_state = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.part_state);
+    p.part_cap = kMaxGridCtas;
     p.seg_counters = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.counters);
     const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
     p.fuse_combine = fused ? 1 : 0;

@@ -73,8 +73,8 @@ combine_kernel(const DecodeParams p)
     const int i_first = cta_of_tile(seg0, total, nc);
     const int i_last = cta_of_tile(seg1 - 1, total, nc);
     if (i_first == i_last) return;  // one CTA owned the whole segment and wrote the rows itself
-    // slot of split s: CTA i's first-segment slot (2i) unless the segment starts inside CTA i_first
-    const int first_slot = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
+    // the first split's record is CTA i_first's kind-1 record when the segment starts inside its range
+    const int first_slot = cta_begin(i_first, total, nc) < seg0 ? 1 : 0;
     uint32_t phase = 0;
     merge_partials<D>(p, warp, lane, first_slot, i_first, i_last - i_first + 1, row0, stage, smem_u32(&s_bar), phase);
 }

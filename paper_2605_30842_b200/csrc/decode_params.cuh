@@ -13,7 +13,9 @@ struct DecodeParams {
     const int32_t *seq_lens;     // [batch]
     __nv_bfloat16 *out;          // [batch][Hq][D]
     float *lse_out;              // [batch][Hq] or nullptr
-    float *partials;             // workspace: [2 * grid_ctas][partial_stride_floats(D)]
+    float *part_acc;             // workspace: [2 kinds][part_cap][8][D] (schedule.cuh)
+    float *part_state;           // workspace: [2 kinds][part_cap][8][8]
+    int part_cap;                // records per kind the workspace holds (>= grid_ctas)
     int *seg_counters;           // workspace: [batch][Hkv] arrival counters, zero between launches
     int fuse_combine;            // 1: the last CTA to finish a cut segment merges it inside K1
 #ifdef COMEM_TRACE

@@ -111,7 +111,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     const uint32_t merge_bar = empty0 + 8 * C::kStages;  // completion of merge.cuh's bulk copies
 
     // A CTA cuts at most two segments: its first (slot 0) and its last (slot 1; slot 0 if it has one segment only).
-    // Per slot: {this CTA merges?, first_slot, i_first, nsplit, arrival counter index, first output row}.
+    // Per slot: {this CTA merges?, first record's kind, i_first, nsplit, arrival counter index, first output row}.
     __shared__ int s_seg[2][6];
 
     const int warp = threadIdx.x >> 5;
@@ -330,7 +330,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const int64_t seg0 = x - sp.j, seg1 = seg0 + sp.T;
             const int i_first = cta_of_tile(seg0, total, nc);
             int *sg = s_seg[x == c0 ? 0 : 1];
-            sg[1] = 2 * i_first + (cta_begin(i_first, total, nc) < seg0 ? 1 : 0);
+            sg[1] = cta_begin(i_first, total, nc) < seg0 ? 1 : 0;  // record kind of the segment's first split
             sg[2] = i_first;
             sg[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
             sg[4] = sp.b * p.num_kv_heads + sp.kvh;
@@ -485,9 +485,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 den_x += ww[w] * scratch[w * C::kScratchFloatsPerWarp + C::kStateOff + 2 * kMaxGroup + head];
             }
             const int64_t row = (int64_t)sp.b * p.num_q_heads + head0 + head;
-            float *part = nullptr;
-            if (!whole_segment)
-                part = p.partials + (int64_t)(2 * cta + (x == c0 ? 0 : 1)) * partial_stride_floats(D);
+            const int64_t rec = (int64_t)(x == c0 ? 0 : 1) * p.part_cap + cta;  // [kind][cta]
             if (lane < D / 4) {
                 float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
@@ -503,13 +501,13 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     packed.y = pack_bf16x2(num.z * inv, num.w * inv);
                     *reinterpret_cast<uint2 *>(p.out + row * D + 4 * lane) = packed;
                 } else {
-                    *reinterpret_cast<float4 *>(part + head * D + 4 * lane) = num;
+                    *reinterpret_cast<float4 *>(p.part_acc + rec * (kMaxGroup * D) + head * D + 4 * lane) = num;
                 }
             }
             if (whole_segment) {
                 if (p.lse_out && lane == 0) p.lse_out[row] = (M + log2f(den_x)) * 0.69314718055994530942f;
             } else if (lane < 2) {  // the head's state sector, written whole: {m, l, lx, 0} {0, 0, 0, 0}
-                *reinterpret_cast<float4 *>(part + kMaxGroup * D + 8 * head + 4 * lane) =
+                *reinterpret_cast<float4 *>(p.part_state + rec * kStateFloats + 8 * head + 4 * lane) =
                     lane == 0 ? make_float4(M, den, den_x, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }

@@ -51,8 +51,13 @@ COMEM_HD int cta_of_tile(int64_t x, int64_t total_tiles, int nc)
     return (int)(((x + 1) * nc - 1) / total_tiles);
 }
 
-// Partial record: acc fp32 [8 heads][D], then per head one 32-byte sector {m, l, lx, 0, 0, 0, 0, 0}
-// (a whole sector per head so that it is written by ONE store instruction and read by one load).
-COMEM_HD int partial_stride_floats(int head_dim) { return kMaxGroup * head_dim + 8 * kMaxGroup; }
+// Split partials in the workspace.  A CTA writes at most two records: kind 0 for its FIRST segment,
+// kind 1 for its LAST segment when that is a different one.  Structure of arrays, indexed [kind][cta]:
+//   acc   fp32 [2][cap][8 heads][D]      un-normalised accumulator rows
+//   state fp32 [2][cap][8 heads][8]      per head one 32-byte sector {m, l, lx, 0, 0, 0, 0, 0}
+// A segment cut by CTAs i_first..i_last is therefore record (kind k0, i_first) followed by the
+// CONTIGUOUS run (kind 0, i_first+1 .. i_last): the merge fetches it with two bulk copies.
+constexpr int kStateFloats = 8 * kMaxGroup;
+COMEM_HD int record_floats(int head_dim) { return kMaxGroup * head_dim; }
 
 }  // namespace comem
