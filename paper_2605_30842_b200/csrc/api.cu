@@ -17,6 +17,7 @@ namespace comem {
 namespace {
 
 constexpr int kMaxGridCtas = 1024;  // workspace is sized for this many persistent CTAs
+static_assert(kMaxGridCtas == kMaxGridCtasBound, "schedule.cuh's 32-bit fast paths assume this bound");
 constexpr float kLog2e = 1.4426950408889634f;
 static_assert(kMaxBatch == COMEM_MAX_BATCH, "header and scheduler disagree on the batch limit");
 
@@ -261,9 +262,22 @@ int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_head
 {
     if (!seq_lens_host || !tile_begin || !num_ctas || batch <= 0 || num_kv_heads <= 0 || grid_ctas <= 0)
         return COMEM_ERR_INVALID_ARG;
-    int64_t tiles = 0;
-    for (int b = 0; b < batch; ++b) tiles += tiles_of(seq_lens_host[b]);
-    const int64_t total = tiles * num_kv_heads;
+    std::vector<int> prefix(batch + 1, 0);
+    for (int b = 0; b < batch; ++b) prefix[b + 1] = prefix[b] + tiles_of(seq_lens_host[b]);
+    const int64_t total = (int64_t)prefix[batch] * num_kv_heads;
+    if (total > 0 && batch * num_kv_heads <= kAlignedMaxSegs) {
+        int e[kAlignedMaxSegs + 1];
+        if (aligned_build(prefix.data(), batch, num_kv_heads, grid_ctas, e)) {  // segment-aligned variant
+            *num_ctas = grid_ctas;
+            for (int s = 0; s < batch * num_kv_heads; ++s) {
+                const int b = s / num_kv_heads, kvh = s - b * num_kv_heads, T = prefix[b + 1] - prefix[b];
+                const int64_t seg0 = (int64_t)num_kv_heads * prefix[b] + (int64_t)kvh * T;
+                for (int i = e[s]; i < e[s + 1]; ++i) tile_begin[i] = aligned_cta_begin(seg0, T, i - e[s], e[s + 1] - e[s]);
+            }
+            tile_begin[grid_ctas] = total;
+            return COMEM_OK;
+        }
+    }
     const int nc = total == 0 ? 0 : sched_num_ctas(total, grid_ctas);
     *num_ctas = nc;
     for (int i = 0; i <= nc; ++i) tile_begin[i] = nc ? cta_begin(i, total, nc) : 0;

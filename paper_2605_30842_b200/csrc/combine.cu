@@ -26,6 +26,7 @@ combine_kernel(const DecodeParams p)
 {
     extern __shared__ __align__(128) float stage[];  // MergeCfg<D>::kStageBytes
     __shared__ int s_before[kMaxGroup], s_total[kMaxGroup];
+    __shared__ int s_prefix[kAlignedMaxSegs + 1], s_e[kAlignedMaxSegs + 1], s_aligned;
     __shared__ __align__(8) uint64_t s_bar;
     const int b = blockIdx.x / p.num_kv_heads;
     const int kvh = blockIdx.x - b * p.num_kv_heads;
@@ -52,6 +53,16 @@ combine_kernel(const DecodeParams p)
             total += __shfl_xor_sync(kFullMask, total, o);
         }
         if (lane == 0) { s_before[warp] = before; s_total[warp] = total; }
+        // the segment-aligned variant of the schedule (schedule.cuh), decided exactly as K1 decides it
+        if (tid == 0) {
+            s_aligned = 0;
+            if (p.batch * p.num_kv_heads <= kAlignedMaxSegs) {
+                s_prefix[0] = 0;
+                for (int i = 0; i < p.batch; ++i) s_prefix[i + 1] = s_prefix[i] + tiles_of(__ldg(p.seq_lens + i));
+                if (s_prefix[p.batch] > 0)
+                    s_aligned = aligned_build(s_prefix, p.batch, p.num_kv_heads, p.grid_ctas, s_e) ? 1 : 0;
+            }
+        }
     }
     __syncthreads();
     pdl_launch_dependents();
@@ -64,6 +75,14 @@ combine_kernel(const DecodeParams p)
     if (T == 0) {
         for (int e = tid; e < p.group * D; e += kCombineThreads) p.out[row0 * D + e] = __float2bfloat16_rn(0.f);
         if (p.lse_out && tid < p.group) p.lse_out[row0 + tid] = -INFINITY;
+        return;
+    }
+    if (s_aligned) {
+        const int sidx = b * p.num_kv_heads + kvh;
+        const int c = s_e[sidx + 1] - s_e[sidx];
+        if (c <= 1) return;
+        uint32_t ph = 0;
+        merge_partials<D>(p, warp, lane, 0, s_e[sidx], c, row0, stage, smem_u32(&s_bar), ph);
         return;
     }
     const int64_t total = (int64_t)p.num_kv_heads * total_tiles;

@@ -113,6 +113,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     // A CTA cuts at most two segments: its first (slot 0) and its last (slot 1; slot 0 if it has one segment only).
     // Per slot: {this CTA merges?, first record's kind, i_first, nsplit, arrival counter index, first output row}.
     __shared__ int s_seg[2][6];
+    __shared__ int s_e[kAlignedMaxSegs + 1];  // segment-aligned schedule (schedule.cuh): CTAs before each segment
+    __shared__ int s_aligned, s_valid;
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -151,45 +153,114 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         if (gtid < (((int64_t)p.batch * p.num_q_heads * D * 2 + 127) >> 7))
             prefetch_l2(reinterpret_cast<const char *>(p.q) + (gtid << 7));
     }
+    // S1, the schedule: everything below is a function of seq_lens (and the launch dimensions).
+    // It is computed SPECULATIVELY before griddepcontrol.wait, from whatever seq_lens holds while the
+    // previous kernel may still be running (it may be kv_append, about to bump every length), and
+    // validated after the wait by re-reading seq_lens: a decode step changes a sequence's tile count
+    // once in 16 steps, so the guess is nearly always right and the ~2 us of cold, division-heavy
+    // schedule code run under the previous kernel's tail instead of on this launch's critical path.
+    // A wrong guess just runs the same code again.  seq_lens is read with ld.cg (L2) throughout, so
+    // no stale copy can sit in L1.
+    int64_t total = 0, c0 = 0, c1 = 0;
+    int nc = 0, al_first = 0, al_count = 0;  // aligned: first CTA and CTA count of this CTA's segment
+    bool aligned = false;
+    const int cta = blockIdx.x;
+    auto compute_schedule = [&]() {
+        // exclusive prefix of tiles per sequence (warp 0); kept small: no unrolling
+        if (warp == 0) {
+            if (p.batch <= 32) {
+                const int mine = lane < p.batch ? tiles_of(__ldcg(p.seq_lens + lane)) : 0;
+                int incl = mine;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(kFull, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                if (lane < p.batch) prefix[lane] = incl - mine;
+                if (lane == 31) prefix[p.batch] = incl;
+            } else {
+                const int per = (p.batch + 31) >> 5;
+                const int b0 = lane * per;
+                int sum = 0;
+#pragma unroll 1
+                for (int i = 0; i < per; ++i)
+                    if (b0 + i < p.batch) sum += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                int incl = sum;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(kFull, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                int run = incl - sum;
+#pragma unroll 1
+                for (int i = 0; i < per; ++i)
+                    if (b0 + i < p.batch) {
+                        prefix[b0 + i] = run;
+                        run += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                    }
+                if (lane == 31) prefix[p.batch] = incl;
+            }
+            // Few long segments?  Then deal whole CTAs to segments (schedule.cuh, "segment-aligned
+            // variant"; the same arithmetic as aligned_build, two segments per lane).
+            __syncwarp();
+            const int S = p.batch * p.num_kv_heads;
+            const int64_t tot = (int64_t)p.num_kv_heads * prefix[p.batch];
+            bool ok = S <= kAlignedMaxSegs && tot >= (int64_t)gridDim.x * kMinTilesPerCta;
+            if (ok) {  // warp-uniform
+                const int ideal = ideal_tiles_per_cta(tot, (int)gridDim.x);
+                bool mine_ok = true;
+                for (int sidx = lane; sidx < S; sidx += 32) {
+                    const int b = sidx / p.num_kv_heads, kvh = sidx - b * p.num_kv_heads;
+                    const int T = prefix[b + 1] - prefix[b];
+                    const int64_t before = (int64_t)p.num_kv_heads * prefix[b] + (int64_t)kvh * T;
+                    const int e_lo = aligned_boundary(before, tot, (int)gridDim.x);
+                    const int e_hi = aligned_boundary(before + T, tot, (int)gridDim.x);
+                    s_e[sidx + 1] = e_hi;
+                    mine_ok = mine_ok && aligned_segment_ok(T, e_hi - e_lo, ideal);
+                }
+                if (lane == 0) s_e[0] = 0;
+                ok = __all_sync(kFull, mine_ok);
+            }
+            if (lane == 0) s_aligned = ok ? 1 : 0;
+        }
+        __syncthreads();
+        // this CTA's range [c0, c1) of the linearised tile space
+        total = (int64_t)p.num_kv_heads * prefix[p.batch];
+        aligned = s_aligned != 0;
+        c0 = c1 = 0;
+        if (total == 0) return;
+        if (aligned) {
+            nc = (int)gridDim.x;
+            int lo = 0, hi = p.batch * p.num_kv_heads;  // s_e[lo] <= cta < s_e[hi]
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (s_e[mid] <= cta) lo = mid; else hi = mid;
+            }
+            const int b = lo / p.num_kv_heads, kvh = lo - b * p.num_kv_heads;
+            const int T = prefix[b + 1] - prefix[b];
+            const int64_t seg0 = (int64_t)p.num_kv_heads * prefix[b] + (int64_t)kvh * T;
+            al_first = s_e[lo];
+            al_count = s_e[lo + 1] - al_first;
+            c0 = aligned_cta_begin(seg0, T, cta - al_first, al_count);
+            c1 = aligned_cta_begin(seg0, T, cta - al_first + 1, al_count);
+        } else {
+            nc = sched_num_ctas(total, (int)gridDim.x);
+            if (cta < nc) {
+                c0 = cta_begin(cta, total, nc);
+                c1 = cta_begin(cta + 1, total, nc);
+            }
+        }
+    };
+    compute_schedule();  // speculative
     pdl_wait_prior_grid();
     COMEM_STAMP(1);
-
-    // S1: exclusive prefix of tiles per sequence (warp 0), the whole schedule follows from it.
-    // Executed once per CTA on the critical path of the launch: kept small (no unrolling; the
-    // instruction fetch of cold straight-line code costs more than the arithmetic).
-    if (warp == 0) {
-        if (p.batch <= 32) {
-            const int mine = lane < p.batch ? tiles_of(__ldg(p.seq_lens + lane)) : 0;
-            int incl = mine;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(kFull, incl, o);
-                if (lane >= o) incl += v;
-            }
-            if (lane < p.batch) prefix[lane] = incl - mine;
-            if (lane == 31) prefix[p.batch] = incl;
-        } else {
-            const int per = (p.batch + 31) >> 5;
-            const int b0 = lane * per;
-            int sum = 0;
+    if (warp == 0) {  // validate the guess against the lengths as they are now
+        bool same = true;
 #pragma unroll 1
-            for (int i = 0; i < per; ++i)
-                if (b0 + i < p.batch) sum += tiles_of(__ldg(p.seq_lens + b0 + i));
-            int incl = sum;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(kFull, incl, o);
-                if (lane >= o) incl += v;
-            }
-            int run = incl - sum;
-#pragma unroll 1
-            for (int i = 0; i < per; ++i)
-                if (b0 + i < p.batch) {
-                    prefix[b0 + i] = run;
-                    run += tiles_of(__ldg(p.seq_lens + b0 + i));
-                }
-            if (lane == 31) prefix[p.batch] = incl;
-        }
+        for (int b = lane; b < p.batch; b += 32)
+            same = same && tiles_of(__ldcg(p.seq_lens + b)) == prefix[b + 1] - prefix[b];
+        same = __all_sync(kFull, same);
+        if (lane == 0) s_valid = same ? 1 : 0;
     }
 #ifdef COMEM_TRACE
     if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
@@ -197,6 +268,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     if (p.trace && threadIdx.x == 32) p.trace[blockIdx.x * 16 + 13] = globaltimer_ns();
 #endif
     __syncthreads();
+    if (!s_valid) {
+        __syncthreads();  // everyone has read s_valid and the old tables before warp 0 rewrites them
+        compute_schedule();
+    }
     pdl_launch_dependents();
     COMEM_STAMP(2);
 
@@ -210,15 +285,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 for (int h = threadIdx.x; h < p.num_q_heads; h += kThreads) p.lse_out[row0 + h] = -INFINITY;
         }
     }
-
-    const int64_t total = (int64_t)p.num_kv_heads * prefix[p.batch];
-    if (total == 0) return;
-    const int nc = sched_num_ctas(total, (int)gridDim.x);
-    const int cta = blockIdx.x;
-    if (cta >= nc) return;
-    const int64_t c0 = cta_begin(cta, total, nc);
-    const int64_t c1 = cta_begin(cta + 1, total, nc);
-    if (c0 >= c1) return;
+    if (c0 >= c1) return;  // nothing to stream (no tiles at all, or more CTAs than the schedule uses)
 
     if (warp >= kConsumerWarps) {
         // ------------------------------ S2: page-gather producers -----------------------------
@@ -327,16 +394,22 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         const bool whole_segment = (sp.j == 0 && cnt == sp.T);
         if (!whole_segment && p.fuse_combine && threadIdx.x == 0) {
             // which CTAs cut this segment (64-bit divisions: done now, under the streaming, not in the tail)
-            const int64_t seg0 = x - sp.j, seg1 = seg0 + sp.T;
-            const int i_first = cta_of_tile(seg0, total, nc);
             int *sg = s_seg[x == c0 ? 0 : 1];
-            sg[1] = cta_begin(i_first, total, nc) < seg0 ? 1 : 0;  // record kind of the segment's first split
-            sg[2] = i_first;
-            sg[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
+            if (aligned) {
+                sg[1] = 0;
+                sg[2] = al_first;
+                sg[3] = al_count;
+            } else {
+                const int64_t seg0 = x - sp.j, seg1 = seg0 + sp.T;
+                const int i_first = cta_of_tile(seg0, total, nc);
+                sg[1] = cta_begin(i_first, total, nc) < seg0 ? 1 : 0;  // record kind of the segment's first split
+                sg[2] = i_first;
+                sg[3] = cta_of_tile(seg1 - 1, total, nc) - i_first + 1;
+            }
             sg[4] = sp.b * p.num_kv_heads + sp.kvh;
             sg[5] = sp.b * p.num_q_heads + sp.kvh * p.group;
         }
-        const int seq_len = p.seq_lens[sp.b];
+        const int seq_len = __ldcg(p.seq_lens + sp.b);
         const int head0 = sp.kvh * p.group;
 
         // Q fragments (A operand of S = Q K^T): row = head `quad`, rows 8..15 are zero padding.

@@ -51,6 +51,65 @@ COMEM_HD int cta_of_tile(int64_t x, int64_t total_tiles, int nc)
     return (int)(((x + 1) * nc - 1) / total_tiles);
 }
 
+// ---- segment-aligned variant -----------------------------------------------------------------
+// A CTA whose linear range straddles a segment boundary pays for a second epilogue (S6) in
+// mid-stream -- about 2 us, which a short step (one 32K sequence: ~18 us of streaming) cannot
+// amortise, and which lands on the critical path because that CTA is then the last to arrive on
+// its second segment.  When the step has FEW LONG segments the CTAs are therefore dealt to the
+// segments instead: segment s (s = b * Hkv + kv head, in linear order) owns the CTAs
+// [e[s], e[s+1]) with e[s+1] = round(tiles up to the end of s * grid / total tiles), and CTA j of
+// its c owns tiles [j*T/c, (j+1)*T/c) of it.  No CTA sees two segments; the price is that c is the
+// ideal share rounded, i.e. up to T/c - total/grid extra tiles on the slowest CTA.  The variant
+// is used iff every non-empty segment gets a CTA and that price is below kAlignedMaxLossTiles
+// (same decision, same integer arithmetic, in K1, K2 and comem_schedule_host).
+constexpr int kAlignedMaxSegs = 64;
+constexpr int kMaxGridCtasBound = 1024;  // j <= c <= grid <= 1024 (api.cu's kMaxGridCtas)
+constexpr int kAlignedMaxLossTiles = 6;
+
+COMEM_HD int aligned_boundary(int64_t tiles_to_end, int64_t total_tiles, int grid_ctas)
+{
+    // same value either way; the 32-bit form keeps 64-bit divisions off the launch's critical path
+    if (total_tiles <= (int64_t)(0x7fffffff / 2) / grid_ctas)
+        return (int)(((uint32_t)tiles_to_end * (uint32_t)grid_ctas + (uint32_t)total_tiles / 2u) / (uint32_t)total_tiles);
+    return (int)((tiles_to_end * grid_ctas + total_tiles / 2) / total_tiles);
+}
+// tiles on the busiest CTA if the work were cut evenly
+COMEM_HD int ideal_tiles_per_cta(int64_t total_tiles, int grid_ctas)
+{
+    return (int)((total_tiles + grid_ctas - 1) / grid_ctas);
+}
+// is a segment of T tiles that was dealt c CTAs acceptable?
+COMEM_HD bool aligned_segment_ok(int T, int c, int ideal)
+{
+    if (T == 0) return true;
+    if (c < 1) return false;
+    return (T + c - 1) / c - ideal <= kAlignedMaxLossTiles;
+}
+// Serial builder (host, K2): prefix[b] = tiles of sequences < b (batch + 1 entries).  Fills
+// e[0 .. batch*hkv] and returns true iff the aligned variant applies.
+COMEM_HD bool aligned_build(const int *prefix, int batch, int hkv, int grid_ctas, int *e)
+{
+    const int S = batch * hkv;
+    const int64_t total = (int64_t)hkv * prefix[batch];
+    if (S > kAlignedMaxSegs || total < (int64_t)grid_ctas * kMinTilesPerCta) return false;
+    const int ideal = ideal_tiles_per_cta(total, grid_ctas);
+    bool ok = true;
+    e[0] = 0;
+    for (int s = 0; s < S; ++s) {
+        const int b = s / hkv, kvh = s - b * hkv;
+        const int T = prefix[b + 1] - prefix[b];
+        e[s + 1] = aligned_boundary((int64_t)hkv * prefix[b] + (int64_t)(kvh + 1) * T, total, grid_ctas);
+        ok = ok && aligned_segment_ok(T, e[s + 1] - e[s], ideal);
+    }
+    return ok;
+}
+// first tile (linear coordinates) of CTA j of the c CTAs of a segment that starts at seg0 with T tiles
+COMEM_HD int64_t aligned_cta_begin(int64_t seg0, int T, int j, int c)
+{
+    if (T <= 0x7fffffff / kMaxGridCtasBound) return seg0 + (int)((uint32_t)(j * T) / (uint32_t)c);
+    return seg0 + ((int64_t)j * T) / c;
+}
+
 // Split partials in the workspace.  A CTA writes at most two records: kind 0 for its FIRST segment,
 // kind 1 for its LAST segment when that is a different one.  Structure of arrays, indexed [kind][cta]:
 //   acc   fp32 [2][cap][8 heads][D]      un-normalised accumulator rows

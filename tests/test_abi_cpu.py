@@ -106,3 +106,25 @@ def test_schedule_partitions_tile_space(lib, lens, hkv, grid):
     assert (sizes >= 0).all() and sizes.max() - sizes.min() <= 1       # balanced to one tile
     nc = len(begins) - 1
     assert nc == min(grid, max(1, -(-tiles // 16)))    # schedule.cuh kMinTilesPerCta = 16
+
+
+def test_schedule_segment_aligned_variant(lib):
+    """Few long segments (C2: 8 segments of 2048 tiles on 148 CTAs): whole CTAs are dealt to segments,
+    so no CTA straddles a segment boundary, at the price of 18 vs 19 CTAs per segment; many
+    segments (C3-like) keep the linear cut, balanced to one tile."""
+    begins = comem.comem_schedule_host([32768], 8, 148)
+    assert len(begins) == 149 and begins[0] == 0 and begins[-1] == 8 * 2048
+    sizes = np.diff(begins)
+    assert sizes.min() >= 107 and sizes.max() <= 114
+    for i in range(148):
+        assert begins[i] // 2048 == (begins[i + 1] - 1) // 2048, i      # one segment per CTA
+    per_seg = np.bincount(np.asarray(begins[:-1]) // 2048, minlength=8)
+    assert sorted(set(per_seg.tolist())) == [18, 19] and per_seg.sum() == 148
+    # the price is capped: 2 sequences x 8 heads of 65536 tokens would cost 12 tiles -> linear cut
+    begins = comem.comem_schedule_host([65536, 65536], 8, 148)
+    sizes = np.diff(begins)
+    assert sizes.max() - sizes.min() <= 1
+    # more segments than kAlignedMaxSegs -> linear cut
+    begins = comem.comem_schedule_host([20000] * 32, 8, 148)
+    sizes = np.diff(begins)
+    assert sizes.max() - sizes.min() <= 1
