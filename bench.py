@@ -45,8 +45,8 @@ FALLBACK_PEAK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES_NOMINAL = 126e6
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE split-KV launch from the committed
-# `ncu --set full` capture (profiles/README.md names the command); None until captured.
-NCU_TRAFFIC_BYTES = {"c2": None, "c3": None, "c4": None}
+# `ncu --set full` capture (profiles/r1_b_fused.md names the command).
+NCU_TRAFFIC_BYTES = {"c2": 137_632_512, "c3": 4_838_226_768, "c4": 8_595_141_560}  # profiles/r1_b_fused.md
 
 
 def parse_args():
