@@ -29,6 +29,9 @@
 //     stand-alone K2 (combine.cu) does the merge.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
+#ifndef COMEM_PREFETCH_TILES
+#define COMEM_PREFETCH_TILES 16
+#endif
 #include "decode_params.cuh"
 #include "ptx.cuh"
 #include "schedule.cuh"
@@ -41,6 +44,7 @@ namespace {
 constexpr int kConsumerWarps = 8;
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 static_assert(kConsumerWarps == kMaxGroup, "S6 and merge.cuh map warp w to query head w of the group");
+constexpr int kPrefetchTiles = COMEM_PREFETCH_TILES;  // per CTA, L2-prefetched before the PDL wait (<= 32: one per lane)
 constexpr int kProducerWarps = 2;  // one elected lane each; tiles alternate between them (issue-rate bound otherwise)
 constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
 constexpr unsigned kFull = 0xffffffffu;
@@ -140,10 +144,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         tma_prefetch_desc(&tm_v);
     }
     // Nothing above touched global data.  The inputs may still be written by the kernel running
-    // before this one (kv_append bumps seq_lens), so they are only READ after the wait -- but an L2
-    // prefetch is a hint on a coherent cache and may run now: the small control inputs (seq_lens,
-    // block table, q) are pulled from DRAM while the previous grid drains, and the dependent
-    // chain seq_lens -> block table -> first TMA below then runs at L2 latency.
+    // before this one (kv_append bumps seq_lens), so nothing read before the wait is trusted -- but
+    // an L2 prefetch is a hint on a coherent cache and may run now: the small control inputs
+    // (seq_lens, block table, q) are pulled from DRAM while the previous grid drains, and the
+    // dependent chain seq_lens -> block table -> first TMA after the wait then runs at L2 latency.
     {
         const int64_t gtid = (int64_t)blockIdx.x * kThreads + threadIdx.x;
         if (gtid < (((int64_t)p.batch * 4 + 127) >> 7))
@@ -252,6 +256,26 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         }
     };
     compute_schedule();  // speculative
+    // Still before the wait: ask the TMA unit to pull this CTA's first tiles into L2.  Cached KV rows
+    // of old tokens are immutable, so a prefetch from the guessed schedule and the block table as it
+    // reads now is at worst useless (the page index is clamped to the table row, a bad page id is an
+    // out-of-range tensor coordinate: both harmless for a hint).  HBM is idle while the previous
+    // kernel drains its tail; the first real loads after the wait then hit L2.
+    if (warp == kConsumerWarps && c0 < c1) {
+        const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
+        const int64_t rem = c1 - c0;
+        int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
+        cnt = cnt < kPrefetchTiles ? cnt : kPrefetchTiles;
+        if (lane < cnt) {
+            const int jj = sp.j + lane;
+            int page = jj >> p.page_tile_shift;
+            page = page < p.max_pages ? page : p.max_pages - 1;
+            const int pid = __ldcg(p.block_table + (int64_t)sp.b * p.max_pages + page);
+            const int row = pid * p.page_size + ((jj & ((1 << p.page_tile_shift) - 1)) << kTileShift);
+            tma_prefetch_tile_4d(&tm_k, 0, row, 0, sp.kvh);
+            tma_prefetch_tile_4d(&tm_v, 0, row, 0, sp.kvh);
+        }
+    }
     pdl_wait_prior_grid();
     COMEM_STAMP(1);
     if (warp == 0) {  // validate the guess against the lengths as they are now

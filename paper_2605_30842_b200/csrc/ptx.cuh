@@ -59,6 +59,12 @@ __device__ __forceinline__ void tma_prefetch_desc(const void *tmap)
 {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
+// L2 prefetch of one tile (a hint: nothing is written, out-of-range coordinates are harmless)
+__device__ __forceinline__ void tma_prefetch_tile_4d(const void *tmap, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 // L2 eviction-priority hint (createpolicy) for the load below: the KV stream is read exactly once per step
 __device__ __forceinline__ uint64_t l2_policy_evict_first()
 {
