@@ -5,8 +5,10 @@
 // Shape of the kernel (sm_100a):
 //   * persistent grid, ONE CTA per SM (10 warps, ~214 KiB of shared memory), one contiguous range
 //     of 16-token tiles per CTA (schedule.cuh);
-//   * before griddepcontrol.wait: mbarrier init, tensor-map prefetch and an L2 prefetch of the
-//     small control inputs (seq_lens, block table, q) -- they overlap the previous kernel's tail;
+//   * before griddepcontrol.wait (i.e. under the previous kernel's tail): mbarrier init, tensor-map
+//     prefetch, an L2 prefetch of the small control inputs (seq_lens, block table, q), the whole
+//     schedule computed SPECULATIVELY from seq_lens as it reads now (validated after the wait),
+//     and a TMA L2 prefetch of the CTA's first 16 tiles;
 //   * warps 8, 9 = producers: each reads the block table 32 entries at a time and issues, for
 //     every other tile of the CTA, one TMA tiled load for K and one for V ([16 tokens][D] of one kv
 //     head, 128-byte swizzle) into a 16-stage shared-memory ring guarded by full/empty
