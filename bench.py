@@ -54,8 +54,10 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=8192)
     ap.add_argument("--warmup", type=int, default=64)
-    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--affine", action="store_true",
+                    help="P:L184 check: sweep the context at batch 16 and fit t = a + b*L (extra, not the bench line)")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
@@ -332,6 +334,8 @@ def run_reference(args, rank: int) -> int:
 
     oracle.build()
     cores = oracle.max_threads()
+    if args.workload == "c5":
+        args.workload = "c3"  # C5's agent batch is C3; the oracle arm has no streams to overlap
     desc = workload_desc(args.workload)
     # The sample is a prefix of sequence 0's context, all query heads: T tokens chosen from a
     # calibration pass so that (warmup + steps) passes fit the budget.
@@ -370,11 +374,153 @@ def run_reference(args, rank: int) -> int:
     return 0
 
 
+def run_c5(args) -> int:
+    """BASELINE.json configs[4]: the agent batch (C3) and the memory-model batch on two CUDA streams,
+    64 successive decode steps each (append one token per sequence, then attend).  Reports each stream
+    alone, both overlapped, and the aggregate GB/s over the overlapped window.  1 GPU only."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    n_steps = 64
+    agent = W.config3_agent_ragged(device, spare_tokens=n_steps)
+    memory = W.config5_memory_ragged(device, spare_tokens=n_steps)
+    sa, sm = torch.cuda.Stream(device), torch.cuda.Stream(device)
+    jobs = []
+    for b, st, seed in ((agent, sa, 1005_000), (memory, sm, 1005_500)):
+        jobs.append({"b": b, "stream": st, "len0": b.seq_lens.clone(),
+                     "rows": [W.decode_step_rows(b, i, seed) for i in range(n_steps)],
+                     "out": torch.empty_like(b.q),
+                     "ws": comem.alloc_workspace(b.q, b.k_pages, b.block_table, stream=st)})
+    torch.cuda.synchronize(device)
+
+    def nbytes(j):  # algorithmic bytes of the 64 steps: the context grows by one token per step
+        b = j["b"]
+        l0 = int(j["len0"].sum().item())
+        per_tok = b.num_kv_heads * b.head_dim * 4
+        return sum((l0 + (i + 1) * b.batch) * per_tok + b.batch * b.num_q_heads * b.head_dim * 2
+                   for i in range(n_steps))
+
+    def enqueue(j, i):
+        b, st = j["b"], j["stream"]
+        q, nk, nv = j["rows"][i]
+        comem.comem_kv_append_async(b.k_pages, b.v_pages, b.block_table, b.seq_lens, nk, nv, stream=st)
+        comem.comem_decode_attn_async(q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale,
+                                      j["out"], j["ws"], stream=st)
+
+    def run(which):
+        for j in jobs:
+            j["b"].seq_lens.copy_(j["len0"])
+        torch.cuda.synchronize(device)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in jobs]
+        t0 = torch.cuda.Event(enable_timing=True)
+        t0.record(torch.cuda.current_stream(device))
+        for k in which:
+            jobs[k]["stream"].wait_event(t0)
+            ev[k][0].record(jobs[k]["stream"])
+        for i in range(n_steps):
+            for k in which:
+                enqueue(jobs[k], i)
+        for k in which:
+            ev[k][1].record(jobs[k]["stream"])
+        torch.cuda.synchronize(device)
+        return {k: (t0.elapsed_time(ev[k][1]), ev[k][0].elapsed_time(ev[k][1])) for k in which}
+
+    run([0, 1])  # warm-up
+    reps = max(1, min(5, args.steps // n_steps if args.steps >= n_steps else 1))
+    alone_a = min(run([0])[0][1] for _ in range(reps))
+    alone_m = min(run([1])[1][1] for _ in range(reps))
+    both = [run([0, 1]) for _ in range(reps)]
+    best = min(both, key=lambda r: max(r[0][0], r[1][0]))
+    window = max(best[0][0], best[1][0])
+    by_a, by_m = nbytes(jobs[0]), nbytes(jobs[1])
+    line = {"metric": METRIC, "value": (by_a + by_m) / (window * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": n_steps, "warmup": n_steps, "ms_per_step": window / n_steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": "C5 k-step-off overlap: C3 agent batch + memory batch (8 x U[65536,131072], 32q/8kv) "
+                                   "on two streams, 64 append+attend steps each",
+                       "l2": "cold: each step reads 4.5 + 3.0 GiB of KV >> L2", "launch": "host launches, 2 kernels per step per stream"},
+            "c5": {"agent_alone_us_per_step": alone_a / n_steps * 1e3, "memory_alone_us_per_step": alone_m / n_steps * 1e3,
+                   "overlapped_window_us_per_step": window / n_steps * 1e3,
+                   "agent_overlapped_us_per_step": best[0][1] / n_steps * 1e3,
+                   "memory_overlapped_us_per_step": best[1][1] / n_steps * 1e3,
+                   "agent_slowdown": best[0][1] / alone_a, "memory_slowdown": best[1][1] / alone_m,
+                   "agent_alone_gbs": by_a / (alone_a * 1e-3) / 1e9, "memory_alone_gbs": by_m / (alone_m * 1e-3) / 1e9,
+                   "serial_sum_us_per_step": (alone_a + alone_m) / n_steps * 1e3},
+            "gpu_launches": 4 * n_steps}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_affine(args) -> int:
+    """SURVEY.md §8(d) affine check of eq. 5 (t = L*S/W): batch 16, 64q/8kv, D 128, page 16,
+    context L in {4K .. 128K}; least-squares fit t = a + b*L.  16 * 4096 B / b is the streaming rate,
+    a the fixed cost per step.  One JSON line; an extra, not the driver's bench line."""
+    import numpy as np
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    stream = torch.cuda.Stream(device)
+    B, pts = 16, []
+    for L in (4096, 8192, 16384, 32768, 65536, 131072):
+        R = max(1, min(8, (1 << 30) // (B * L * 4096)))          # rotate pools while one step is < 1 GiB (L2-cold)
+        pools = [W.make_batch([L] * B, 64, 8, 128, 16, 7000 + i, device) for i in range(R)]
+        outs = [torch.empty_like(b.q) for b in pools]
+        ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream)
+        with torch.cuda.stream(stream):
+            def enq():
+                for b, o in zip(pools, outs):
+                    comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                                  b.softmax_scale, o, ws, stream=stream)
+            enq()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                enq()
+            for _ in range(3):
+                g.replay()
+            n = max(2, int(20e-3 / (B * L * 4096 / 7e12) / R))     # ~20 ms of streaming per point
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            e0.record(stream)
+            for _ in range(n):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+        us = e0.elapsed_time(e1) / (n * R) * 1e3
+        pts.append((L, us, pools[0].algorithmic_bytes() / us / 1e3))
+        del pools, outs, ws, g
+        torch.cuda.empty_cache()
+    Ls, ts = np.array([p[0] for p in pts], float), np.array([p[1] for p in pts], float)
+    b_fit, a_fit = np.polyfit(Ls, ts, 1)
+    print(json.dumps({"affine_check": "t_us = a + b * L at batch 16, 64q/8kv, D128, page 16 (PAPER.md eq. 5)",
+                      "points": [{"L": int(l), "us_per_step": round(u, 2), "gbs": round(gb, 1)} for l, u, gb in pts],
+                      "a_us": a_fit, "b_us_per_token": b_fit, "slope_gbs": B * 4096 / b_fit / 1e3,
+                      "max_rel_residual": float(np.max(np.abs(a_fit + b_fit * Ls - ts) / ts))}), flush=True)
+    return 0
+
+
 def main() -> int:
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
     if args.impl == "reference":
         return run_reference(args, rank)
+    if args.affine:
+        return run_affine(args) if rank == 0 else 0
+    if args.workload == "c5":
+        return run_c5(args) if rank == 0 else 0
 
     import torch
     import paper_2605_30842_b200 as comem
