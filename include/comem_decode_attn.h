@@ -188,6 +188,19 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
 int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_heads, int grid_ctas,
                         int64_t *tile_begin, int *num_ctas);
 
+/*
+ * comem_validate_inputs — debug aid for the one thing the hot path trusts (see "Device-side DATA"
+ * above): checks on the device that 0 <= seq_lens[b] <= max_pages_per_seq * page_size and that every
+ * USED block-table entry is a page id in [0, num_pages).  Host-synchronous (1 kernel, a 4-byte
+ * read-back through `workspace`, which may be the attention workspace).  Returns COMEM_OK or
+ * COMEM_ERR_INVALID_ARG.  With the environment variable COMEM_DEBUG_VALIDATE=1 the synchronous
+ * entry points (comem_decode_attn, comem_decode_step_host) run it first and return its verdict
+ * instead of computing on bad data; the *_async entry points never validate.
+ */
+int comem_validate_inputs(const int32_t *block_table, const int32_t *seq_lens, int batch,
+                          int max_pages_per_seq, int page_size, int64_t num_pages, void *workspace,
+                          size_t workspace_bytes, void *cuda_stream);
+
 /* Persistent-grid size (CTAs) the split kernel uses on the current device, or a
  * negative COMEM_ERR_* value.  comem_set_grid_ctas(n > 0) overrides it for later
  * calls from this process (n <= 0 restores the default); used to give each of two

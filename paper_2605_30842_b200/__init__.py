@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     comem_kv_append_async,
     comem_schedule_host,
     comem_set_grid_ctas,
+    comem_validate_inputs,
     comem_status_string,
     comem_version,
     comem_workspace_init_async,

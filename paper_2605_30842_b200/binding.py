@@ -59,6 +59,8 @@ def load_library():
     lib.comem_decode_attn_workspace_bytes.restype = sz
     lib.comem_workspace_init_async.argtypes = [vp, sz, i32, i32, i32, i32, vp]
     lib.comem_workspace_init_async.restype = i32
+    lib.comem_validate_inputs.argtypes = [vp, vp, i32, i32, i32, i64, vp, sz, vp]
+    lib.comem_validate_inputs.restype = i32
     lib.comem_kv_append_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
     lib.comem_kv_append_async.restype = i32
     lib.comem_decode_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
@@ -209,6 +211,13 @@ def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale:
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn")
     return out
+
+
+def comem_validate_inputs(block_table, seq_lens, page_size: int, num_pages: int, workspace, stream=None) -> int:
+    """Debug aid: COMEM_OK or COMEM_ERR_INVALID_ARG (returned, not raised) for the device-side data."""
+    return int(load_library().comem_validate_inputs(
+        _ptr(block_table), _ptr(seq_lens), block_table.shape[0], block_table.shape[1], int(page_size),
+        int(num_pages), _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
 
 
 def comem_kv_append_async(k_pages, v_pages, block_table, seq_lens, new_k, new_v, stream=None) -> None:

@@ -6,6 +6,7 @@
 
 #include <atomic>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <vector>
@@ -26,14 +27,16 @@ std::atomic<int> g_grid_override{0};
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct WorkspaceLayout {
-    size_t counters, part_acc, part_state, q, new_k, new_v, out, lse, total;
+    size_t counters, flag, part_acc, part_state, q, new_k, new_v, out, lse, total;
 };
 
 WorkspaceLayout workspace_layout(int batch, int hq, int hkv, int d)
 {
     WorkspaceLayout w;
     size_t off = 0;
-    w.counters = off;  // first, so that a buffer initialised for a large shape is initialised for smaller ones
+    w.flag = off;      // comem_validate_inputs' verdict word: offset 0 whatever the shape
+    off = align_up(off + sizeof(int), 256);
+    w.counters = off;  // next, so that a buffer initialised for a large shape is initialised for smaller ones
     off = align_up(off + (size_t)batch * hkv * sizeof(int), 256);
     w.part_acc = off;
     off = align_up(off + (size_t)2 * kMaxGridCtas * record_floats(d) * sizeof(float), 256);
@@ -189,6 +192,12 @@ void *device_alias(const void *host_ptr)
     return at.devicePointer;
 }
 
+bool debug_validate()
+{
+    static const bool on = [] { const char *e = std::getenv("COMEM_DEBUG_VALIDATE"); return e && e[0] == '1'; }();
+    return on;
+}
+
 bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 }  // namespace
@@ -229,7 +238,7 @@ int comem_workspace_init_async(void *workspace, size_t workspace_bytes, int batc
     if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
     const int st = check_device();
     if (st != COMEM_OK) return st;
-    if (cudaMemsetAsync(static_cast<char *>(workspace) + wl.counters, 0, wl.part_acc - wl.counters,
+    if (cudaMemsetAsync(static_cast<char *>(workspace) + wl.flag, 0, wl.part_acc - wl.flag,
                         static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
@@ -240,6 +249,36 @@ int comem_workspace_init_async(void *workspace, size_t workspace_bytes, int batc
 #ifdef COMEM_TRACE
 int comem_set_trace(void *buf) { g_trace = static_cast<unsigned long long *>(buf); return COMEM_OK; }
 #endif
+
+static int validate_impl(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages_per_seq,
+                         int page_size, int64_t num_pages, void *workspace, size_t workspace_bytes,
+                         void *cuda_stream, int extra_tokens)
+{
+    if (!block_table || !seq_lens || batch <= 0 || max_pages_per_seq <= 0 || page_size <= 0 || num_pages <= 0)
+        return COMEM_ERR_INVALID_ARG;
+    const WorkspaceLayout wl = workspace_layout(batch, 1, 1, 64);
+    if (!workspace || workspace_bytes < wl.counters || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
+    const int st = check_device();
+    if (st != COMEM_OK) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int *flag = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.flag);
+    int verdict = 0;
+    if (launch_validate(block_table, seq_lens, batch, max_pages_per_seq, page_size, num_pages, flag, stream, extra_tokens) != cudaSuccess ||
+        cudaMemcpyAsync(&verdict, flag, sizeof(int), cudaMemcpyDeviceToHost, stream) != cudaSuccess ||
+        cudaMemsetAsync(flag, 0, sizeof(int), stream) != cudaSuccess || cudaStreamSynchronize(stream) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return verdict == 0 ? COMEM_OK : COMEM_ERR_INVALID_ARG;
+}
+
+int comem_validate_inputs(const int32_t *block_table, const int32_t *seq_lens, int batch,
+                          int max_pages_per_seq, int page_size, int64_t num_pages, void *workspace,
+                          size_t workspace_bytes, void *cuda_stream)
+{
+    return validate_impl(block_table, seq_lens, batch, max_pages_per_seq, page_size, num_pages, workspace,
+                         workspace_bytes, cuda_stream, 0);
+}
 
 int comem_set_grid_ctas(int n)
 {
@@ -361,6 +400,11 @@ int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages, c
                       int page_size, float softmax_scale, void *out, int batch, int max_pages_per_seq,
                       int64_t num_pages, float *lse_out, void *workspace, size_t workspace_bytes)
 {
+    if (debug_validate()) {
+        const int v = comem_validate_inputs(block_table, seq_lens, batch, max_pages_per_seq, page_size, num_pages,
+                                            workspace, workspace_bytes, nullptr);
+        if (v != COMEM_OK) return v;
+    }
     const int st = comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, num_q_heads,
                                            num_kv_heads, head_dim, page_size, softmax_scale, out, batch,
                                            max_pages_per_seq, num_pages, lse_out, workspace,
@@ -404,6 +448,12 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
     const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
     if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
     if ((st = check_device()) != COMEM_OK) return st;
+    if (debug_validate()) {
+        if (!block_table || !seq_lens) return COMEM_ERR_INVALID_ARG;
+        st = validate_impl(block_table, seq_lens, batch, max_pages_per_seq, page_size, num_pages, workspace,
+                           workspace_bytes, cuda_stream, new_k_host ? 1 : 0);
+        if (st != COMEM_OK) return st;
+    }
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     char *ws = static_cast<char *>(workspace);
     const size_t q_bytes = (size_t)batch * num_q_heads * head_dim * 2;

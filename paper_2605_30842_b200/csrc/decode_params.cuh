@@ -42,6 +42,8 @@ cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
                              int page_size, int batch, int max_pages, cudaStream_t stream,
                              const __nv_bfloat16 *q_src = nullptr, __nv_bfloat16 *q_dst = nullptr,
                              int q_row_elems = 0);
+cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,
+                            int page_size, int64_t num_pages, int *flag, cudaStream_t stream, int extra_tokens = 0);
 // occupancy-derived persistent grid for the split kernel on the current device
 cudaError_t split_default_grid(int head_dim, int *grid_ctas);
 size_t split_smem_bytes(int head_dim, int batch);

@@ -45,7 +45,36 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
     if (threadIdx.x == 0) seq_lens[b] = t + 1;
 }
 
+// Debug aid (comem_validate_inputs): one CTA per sequence checks what the hot path trusts --
+// seq_len within the table row's reach and every USED table entry a page id inside the pool.
+// flag: 0 = fine; otherwise 1 + index of the first offending sequence seen.
+__global__ void __launch_bounds__(128)
+validate_kernel(const int32_t *block_table, const int32_t *seq_lens, int max_pages, int page_size,
+                long long num_pages, int *flag, int extra_tokens)
+{
+    const int b = blockIdx.x;
+    const int len = seq_lens[b] + extra_tokens;  // extra_tokens = 1: the state after the append about to run
+    bool bad = seq_lens[b] < 0 || (long long)len > (long long)max_pages * page_size;
+    if (!bad) {
+        const int used = (len + page_size - 1) / page_size;
+        for (int j = threadIdx.x; j < used; j += blockDim.x) {
+            const int pid = block_table[(long long)b * max_pages + j];
+            bad = bad || pid < 0 || pid >= num_pages;
+        }
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicCAS(flag, 0, b + 1);
+}
+
 }  // namespace
+
+cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,
+                            int page_size, int64_t num_pages, int *flag, cudaStream_t stream, int extra_tokens)
+{
+    cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), stream);
+    if (e != cudaSuccess) return e;
+    validate_kernel<<<batch, 128, 0, stream>>>(block_table, seq_lens, max_pages, page_size, (long long)num_pages, flag, extra_tokens);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *block_table,
                              int32_t *seq_lens, const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v,

@@ -260,3 +260,23 @@ def test_every_grid_size_same_answer(oracle):
             check_batch(oracle, b, what=f"grid {g}")
     finally:
         comem.comem_set_grid_ctas(0)
+
+
+def test_validate_inputs_debug_aid():
+    """comem_validate_inputs flags exactly the two things the hot path trusts; the workspace it borrows
+    stays usable (its counters are re-zeroed)."""
+    b = W.make_batch([100, 37, 0, 5000], 8, 2, 64, 16, seed=81, device=DEV, poison_unused=True)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    ok = lambda bt, sl: comem.comem_validate_inputs(bt, sl, 16, b.num_pages, ws)  # noqa: E731
+    assert ok(b.block_table, b.seq_lens) == comem.COMEM_OK            # -1 in IGNORED entries is fine
+    bad = b.block_table.clone()
+    bad[3, 7] = b.num_pages                                           # a used entry outside the pool
+    assert ok(bad, b.seq_lens) == comem.COMEM_ERR_INVALID_ARG
+    bad[3, 7] = -5
+    assert ok(bad, b.seq_lens) == comem.COMEM_ERR_INVALID_ARG
+    long = b.seq_lens.clone()
+    long[1] = b.block_table.shape[1] * 16 + 1                         # longer than the table row reaches
+    assert ok(b.block_table, long) == comem.COMEM_ERR_INVALID_ARG
+    out, _ = gpu_run(b, workspace=ws)                                 # the borrowed workspace still works
+    out2, _ = gpu_run(b)
+    assert torch.equal(bits(out), bits(out2))
