@@ -280,3 +280,31 @@ def test_validate_inputs_debug_aid():
     out, _ = gpu_run(b, workspace=ws)                                 # the borrowed workspace still works
     out2, _ = gpu_run(b)
     assert torch.equal(bits(out), bits(out2))
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_randomised_shapes(oracle, case):
+    """Seeded random draws over everything the ABI accepts: batch, kv heads, group, head_dim, page size,
+    ragged lengths with zeros and tile/page-boundary values mixed in, and the persistent grid size
+    (so that linear and segment-aligned schedules, whole and cut segments, one- and multi-round
+    merges all occur)."""
+    rng = np.random.default_rng(9000 + case)
+    G = int(rng.choice([1, 2, 4, 8]))
+    hkv = int(rng.integers(1, 9))
+    D = int(rng.choice([64, 128]))
+    ps = int(rng.choice([16, 32]))
+    batch = int(rng.integers(1, 13))
+    special = [0, 1, 15, 16, 17, ps - 1, ps, ps + 1, 255, 256, 257]
+    lens = [int(rng.choice(special)) if rng.random() < 0.3 else int(rng.integers(1, 6000)) for _ in range(batch)]
+    if case % 6 == 0:
+        lens[0] = int(rng.integers(20000, 60000))          # one long sequence: many splits per segment
+    grid = int(rng.choice([0, 0, 3, 17, 61, 148, 211, 600]))
+    pool = max(1, sum(W.pages_needed(l, ps) for l in lens)) + int(rng.integers(0, 9))   # an all-empty batch still has a pool
+    b = W.make_batch(lens, G * hkv, hkv, D, ps, seed=9100 + case, device=DEV, poison_unused=True, num_pages=pool)
+    try:
+        comem.comem_set_grid_ctas(grid)
+        out, lse, _ = check_batch(oracle, b, what=f"case {case}: G{G} hkv{hkv} D{D} ps{ps} lens{lens} grid{grid}")
+        out2, lse2 = gpu_run(W.permute_pages(b, seed=case))
+        assert torch.equal(bits(out), bits(out2)) and torch.equal(lse.nan_to_num(neginf=-1e30), lse2.nan_to_num(neginf=-1e30))
+    finally:
+        comem.comem_set_grid_ctas(0)
