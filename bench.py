@@ -205,6 +205,25 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
     return e0.elapsed_time(e1)
 
 
+def step_distribution(torch, comem, pools, outs, ws, stream, n, phases):
+    """Each of n single steps timed on its own with a CUDA-event pair (host launches, the stream idle
+    before each step, so launch latency is inside): min / median / p95 in microseconds.  The headline
+    number is the back-to-back one; this is the spread SURVEY.md §8(d) asks for."""
+    R = len(pools)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    with torch.cuda.stream(stream):
+        for i in range(n):
+            b = pools[i % R]
+            stream.synchronize()
+            ev[i][0].record(stream)
+            comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                                 b.softmax_scale, outs[i % R], ws, stream=stream, phases=phases)
+            ev[i][1].record(stream)
+        stream.synchronize()
+    us = sorted(a.elapsed_time(b) * 1e3 for a, b in ev)
+    return {"n": n, "min": us[0], "median": us[n // 2], "p95": us[min(n - 1, int(0.95 * n))]}
+
+
 def timed_e2e(torch, comem, replicas, pools, ws, stream, steps, warmup, sampler, device, seed_base):
     """End to end through comem_decode_step_host: per step H2D(q, new k, new v) from pinned host
     memory -> append -> attention -> D2H(out), host-synchronous.  Returns (ms, bytes, h2d, d2h)."""
@@ -316,7 +335,13 @@ def cpu_baseline_and_parity(batch, gpu_out, budget_s=20.0):
               "rel_l2": float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)),
               "tol": {"max_abs": 2e-2, "mean_abs": 2e-3, "rel_l2": 5e-3}}
     parity["ok"] = bool(parity["max_abs"] <= 2e-2 and parity["mean_abs"] <= 2e-3 and parity["rel_l2"] <= 5e-3)
+    # one thread, on one query head of the first sampled sequence (scaled to bytes of KV consumed)
+    t0 = time.perf_counter()
+    oracle.decode_attn(q, kp, vp, bt, sl, batch.softmax_scale, pairs=[(0, 0)], num_threads=1)
+    one = time.perf_counter() - t0
+    one_gbs = lens[seqs[0]] * batch.head_dim * 4 / g / one / 1e9   # a head reads 1/G of its kv head's K+V
     base = {"value": nbytes / best / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "single_thread_value": one_gbs,
             "sample": f"{len(seqs)} of {len(lens)} sequences, all {hq} query heads, full context "
                       f"({toks} tokens), best of {reps}; {best:.3f} s per pass",
             "seconds": best}
@@ -561,6 +586,7 @@ def main() -> int:
                      not args.no_graph, sampler, device)
     ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, args.steps, args.warmup,
                            comem.COMEM_PHASE_SPLIT, not args.no_graph, sampler, device)
+    dist = step_distribution(torch, comem, pools, outs, ws, stream, 200 if args.workload == "c2" else 20, both)
     bytes_k_steps = sum(step_bytes[i % R] for i in range(args.steps))
     ms_max = replicas.max_over_ranks(ms, device)
     ms_split_max = replicas.max_over_ranks(ms_split, device)
@@ -606,6 +632,7 @@ def main() -> int:
                         "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "us_per_step": e2e_ms_max / args.steps * 1e3,
                         "api": "comem_decode_step_host, pinned host buffers: K3 reads the q,k,v rows over the host link and appends -> fused split+combine stores out into host memory -> stream synchronize (2 launches, no copy engine)"},
+                "isolated_step_us": dist, "input_checksums": pools[0].checksums(),
                 "gpu_launches": args.steps,
                 "clocks": sampler.summary()}
         if cpu_base is not None:
