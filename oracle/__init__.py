@@ -42,6 +42,9 @@ def _load():
         lib.oracle_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, vp,
                                            i32, i32, vp, i64, i32]
         lib.oracle_decode_attn.restype = i32
+        lib.oracle_decode_attn_window.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, vp, vp,
+                                                  i32, i32, i32]
+        lib.oracle_decode_attn_window.restype = i32
         lib.oracle_decode_attn_partial.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32,
                                                    i32, i32, i64, i64, i32, vp, vp, vp]
         lib.oracle_decode_attn_partial.restype = i32
@@ -113,6 +116,24 @@ def decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale, pairs
                                 _p(pr), npairs, int(num_threads))
     if rc != 0:
         raise ValueError(f"oracle_decode_attn: invalid argument (rc={rc})")
+    return out, lse
+
+
+def decode_attn_window(q, k_pages, v_pages, block_table, seq_lens, softmax_scale, window: int,
+                       sink_tokens: int, num_threads: int = 0):
+    """Sliding-window + attention-sink variant: the query (position L-1) attends t < sink_tokens or
+    t >= L - window.  Returns (out [batch, Hq, D], lse [batch, Hq]) as numpy float64."""
+    lib = _load()
+    qb, kb, vb = as_bits(q), as_bits(k_pages), as_bits(v_pages)
+    bt, sl = _as_i32(block_table), _as_i32(seq_lens)
+    batch, hq, hkv, d, ps, maxp, _ = _dims(qb, kb, bt)
+    out = np.empty((batch, hq, d), np.float64)
+    lse = np.empty((batch, hq), np.float64)
+    rc = lib.oracle_decode_attn_window(_p(qb), _p(kb), _p(vb), _p(bt), _p(sl), hq, hkv, d, ps,
+                                       ctypes.c_float(float(np.float32(softmax_scale))), int(window),
+                                       int(sink_tokens), _p(out), _p(lse), batch, maxp, int(num_threads))
+    if rc != 0:
+        raise ValueError(f"oracle_decode_attn_window: invalid argument (rc={rc})")
     return out, lse
 
 

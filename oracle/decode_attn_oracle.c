@@ -32,6 +32,9 @@
  * permutation bit-identity; GQA convention; split/LSE-merge invariance (pins
  * oracle_lse_merge and oracle_decode_attn_partial); tail-poison independence;
  * brute-force dense numpy fp64; torch CPU fp64 SDPA; lse closed form.
+ * oracle_decode_attn_window: W1..W5 (window >= L is the full result bit for bit; window 1 returns
+ * the last V; equals full attention over a cache compacted to the kept tokens; masked tokens'
+ * contents are irrelevant; brute-force dense masked softmax).
  */
 #include <math.h>
 #include <stdint.h>
@@ -133,6 +136,74 @@ int oracle_decode_attn(const uint16_t *q,           /* bf16 [batch][Hq][D] */
         /* pass 2: normaliser and weighted sum of values */
         double Z = 0.0;
         for (int64_t t = 0; t < L; ++t) {
+            const double w = exp(s[t] - m);
+            const uint16_t *vrow = paged_row(v_pages, bt, t, kvh, num_kv_heads, D, page_size);
+            Z += w;
+            for (int d = 0; d < D; ++d) o[d] += w * bf16_to_double(vrow[d]);
+        }
+        for (int d = 0; d < D; ++d) o[d] /= Z;
+        if (lse) lse[r] = m + log(Z);
+        free(s);
+        free(qd);
+    }
+    return 0;
+}
+
+/*
+ * Sliding-window + attention-sink variant (the paper names sliding windows and
+ * attention sinks as orthogonal byte-reducing approaches; it gives no formula, so the
+ * reading is DESIGN.md R17): the one query, which sits at position L-1, attends the kept set
+ *     K = { t in [0, L) : t < sink_tokens  or  t >= L - window }
+ * and out = softmax over K only.  window >= L (or window <= 0, "no window") keeps everything and is
+ * oracle_decode_attn.  Same two-pass fp64 statement, masked positions simply absent.
+ */
+int oracle_decode_attn_window(const uint16_t *q, const uint16_t *k_pages, const uint16_t *v_pages,
+                              const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                              int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                              int window, int sink_tokens, double *out, double *lse, int batch,
+                              int max_pages_per_seq, int num_threads)
+{
+    if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return 1;
+    if (num_q_heads <= 0 || num_kv_heads <= 0 || num_q_heads % num_kv_heads != 0) return 1;
+    if (head_dim <= 0 || page_size <= 0 || batch <= 0 || sink_tokens < 0) return 1;
+    const int G = num_q_heads / num_kv_heads;
+    const int D = head_dim;
+    const int64_t rows = (int64_t)batch * num_q_heads;
+    const double scale = (double)softmax_scale;
+#ifdef _OPENMP
+    if (num_threads <= 0) num_threads = omp_get_max_threads();
+#else
+    (void)num_threads;
+#endif
+#pragma omp parallel for schedule(dynamic, 1) num_threads(num_threads)
+    for (int64_t r = 0; r < rows; ++r) {
+        const int b = (int)(r / num_q_heads), h = (int)(r % num_q_heads);
+        const int kvh = h / G;
+        const int64_t L = seq_lens[b];
+        const int64_t first_in_window = (window <= 0 || window >= L) ? 0 : L - window;
+        const int32_t *bt = block_table + (int64_t)b * max_pages_per_seq;
+        double *o = out + r * D;
+        for (int d = 0; d < D; ++d) o[d] = 0.0;
+        if (L <= 0) {
+            if (lse) lse[r] = -INFINITY;
+            continue;
+        }
+        double *qd = (double *)malloc(sizeof(double) * D);
+        double *s = (double *)malloc(sizeof(double) * (size_t)L);
+        const uint16_t *qrow = q + ((int64_t)b * num_q_heads + h) * D;
+        for (int d = 0; d < D; ++d) qd[d] = bf16_to_double(qrow[d]);
+        double m = -INFINITY;
+        for (int64_t t = 0; t < L; ++t) {
+            if (!(t < sink_tokens || t >= first_in_window)) continue; /* not in the kept set */
+            const uint16_t *krow = paged_row(k_pages, bt, t, kvh, num_kv_heads, D, page_size);
+            double dot = 0.0;
+            for (int d = 0; d < D; ++d) dot += qd[d] * bf16_to_double(krow[d]);
+            s[t] = scale * dot;
+            if (s[t] > m) m = s[t];
+        }
+        double Z = 0.0;
+        for (int64_t t = 0; t < L; ++t) {
+            if (!(t < sink_tokens || t >= first_in_window)) continue;
             const double w = exp(s[t] - m);
             const uint16_t *vrow = paged_row(v_pages, bt, t, kvh, num_kv_heads, D, page_size);
             Z += w;
