@@ -58,6 +58,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--affine", action="store_true",
                     help="P:L184 check: sweep the context at batch 16 and fit t = a + b*L (extra, not the bench line)")
+    ap.add_argument("--window", type=int, default=0,
+                    help="extra: time comem_decode_attn_window_async on the C4 batch with this sliding window")
+    ap.add_argument("--sinks", type=int, default=64, help="attention-sink tokens for --window")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
@@ -537,11 +540,60 @@ def run_affine(args) -> int:
     return 0
 
 
+def run_window(args) -> int:
+    """Extra: the sliding-window + attention-sink variant on the C4 batch
+    (16 x 131072 tokens, 32q/8kv, page 32).  Algorithmic bytes = K+V of the KEPT tokens + Q; the same
+    HBM roofline applies to them.  One JSON line; not the driver's bench line."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    b = W.config4_memory_long(device)
+    kept = sum(min(L, min(args.sinks, max(L - args.window, 0)) + min(args.window, L)) for L in b.seq_lens.cpu().tolist())
+    nbytes = kept * b.num_kv_heads * b.head_dim * 4 + b.batch * b.num_q_heads * b.head_dim * 2
+    R = max(1, min(8, (1 << 30) // max(nbytes, 1)))              # rotate q/out only: the pool is 17 GiB, L2-cold anyway
+    stream = torch.cuda.Stream(device)
+    out = torch.empty_like(b.q)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table, stream=stream)
+    with torch.cuda.stream(stream):
+        f = lambda: comem.comem_decode_attn_window_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,  # noqa: E731
+                                                         b.softmax_scale, out, ws, args.window, args.sinks, stream=stream)
+        f()
+        stream.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            f()
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > L2: written between timed steps
+        n, tot = max(3, min(args.steps, 50)), 0.0
+        for i in range(n + 3):
+            flush.fill_(i & 0xff)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            if i >= 3:
+                tot += e0.elapsed_time(e1)
+    us = tot / n * 1e3
+    print(json.dumps({"extra": "sliding window + sinks on the C4 batch", "window": args.window, "sinks": args.sinks,
+                      "kept_tokens": kept, "algorithmic_bytes_per_step": nbytes, "us_per_step": us,
+                      "value": nbytes / us / 1e3, "unit": UNIT, "l2": "flushed (512 MiB written) before every timed step",
+                      "full_attention_bytes": b.algorithmic_bytes()}), flush=True)
+    return 0
+
+
 def main() -> int:
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
     if args.impl == "reference":
         return run_reference(args, rank)
+    if args.window > 0:
+        return run_window(args) if rank == 0 else 0
     if args.affine:
         return run_affine(args) if rank == 0 else 0
     if args.workload == "c5":

@@ -123,6 +123,23 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
                                    void *workspace, size_t workspace_bytes, void *cuda_stream,
                                    int phases);
 
+/*
+ * comem_decode_attn_window_async — the byte-reducing variant the paper calls orthogonal (sliding
+ * window + attention sinks; reading R17): the query, which sits at
+ * position seq_lens[b] - 1, attends only the positions t < sink_tokens and t >= seq_lens[b] - window,
+ * and only the 16-token tiles holding such a position are scheduled and read.  window <= 0 (or
+ * >= seq_lens[b]) means no window: the call is then comem_decode_attn_async.  sink_tokens >= 0.
+ * Everything else (arguments, workspace, determinism, one fused launch) as comem_decode_attn_async;
+ * the contents of positions outside the kept set never matter (NaN / Inf included).
+ */
+int comem_decode_attn_window_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens,
+                                   int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                                   float softmax_scale, void *out, int batch,
+                                   int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream,
+                                   int window, int sink_tokens);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,
@@ -183,7 +200,7 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
  * scheduler; used by tests and DESIGN.md).  Given host copies of seq_lens,
  * writes for each CTA i in [0, *num_ctas) its half-open range of 16-token tiles
  * [tile_begin[i], tile_begin[i+1]) in the linearised (b, kv_head, tile) order.
- * tile_begin must hold grid_ctas + 1 entries.  Returns COMEM_OK.
+ * tile_begin must hold grid_ctas + 1 entries.  Returns COMEM_OK.  (Full attention only: no window.)
  */
 int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_heads, int grid_ctas,
                         int64_t *tile_begin, int *num_ctas);

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     comem_decode_attn,
     comem_decode_attn_async,
     comem_decode_attn_phases_async,
+    comem_decode_attn_window_async,
     COMEM_PHASE_SPLIT,
     COMEM_PHASE_COMBINE,
     comem_decode_attn_workspace_bytes,

@@ -52,6 +52,9 @@ def load_library():
     lib.comem_decode_attn_phases_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                                    i32, i64, vp, vp, sz, vp, i32]
     lib.comem_decode_attn_phases_async.restype = i32
+    lib.comem_decode_attn_window_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
+                                                   i32, i64, vp, vp, sz, vp, i32, i32]
+    lib.comem_decode_attn_window_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
     lib.comem_decode_attn.restype = i32
@@ -192,6 +195,20 @@ def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_
         workspace.numel() * workspace.element_size(), _stream(stream))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_async")
+
+
+def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
+                                   workspace, window: int, sink_tokens: int, lse_out=None, stream=None) -> None:
+    """Sliding-window + attention-sink decode attention (one fused launch on ``stream``)."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_window_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_window_async")
 
 
 def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out=None,

@@ -323,13 +323,14 @@ int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_head
     return COMEM_OK;
 }
 
-int comem_decode_attn_phases_async(const void *q, const void *k_pages, const void *v_pages,
-                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
-                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale,
-                                   void *out, int batch, int max_pages_per_seq, int64_t num_pages,
-                                   float *lse_out, void *workspace, size_t workspace_bytes,
-                                   void *cuda_stream, int phases)
+static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pages,
+                            const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                            int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                            void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                            float *lse_out, void *workspace, size_t workspace_bytes,
+                            void *cuda_stream, int phases, int window, int sink_tokens)
 {
+    if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
     if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;
     int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
@@ -369,6 +370,8 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
     p.page_size = page_size;
     p.page_tile_shift = page_size == 32 ? 1 : 0;
     p.scale_log2 = softmax_scale * kLog2e;
+    p.window = window > 0 ? window : 0;
+    p.sinks = window > 0 ? sink_tokens : 0;
     if ((st = grid_for(head_dim, &p.grid_ctas)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -381,6 +384,31 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
         return COMEM_ERR_CUDA;
     }
     return COMEM_OK;
+}
+
+int comem_decode_attn_phases_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                                   void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                                   float *lse_out, void *workspace, size_t workspace_bytes,
+                                   void *cuda_stream, int phases)
+{
+    return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
+                            page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
+                            workspace, workspace_bytes, cuda_stream, phases, 0, 0);
+}
+
+int comem_decode_attn_window_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                                   void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                                   float *lse_out, void *workspace, size_t workspace_bytes,
+                                   void *cuda_stream, int window, int sink_tokens)
+{
+    return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
+                            page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
+                            workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
+                            window, sink_tokens);
 }
 
 int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,

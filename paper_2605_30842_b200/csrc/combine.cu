@@ -43,7 +43,7 @@ combine_kernel(const DecodeParams p)
         int before = 0, total = 0;
 #pragma unroll 1
         for (int i = tid; i < p.batch; i += kCombineThreads) {
-            const int ti = tiles_of(__ldg(p.seq_lens + i));
+            const int ti = seq_tiles(__ldg(p.seq_lens + i), p.window, p.sinks);
             total += ti;
             if (i < b) before += ti;
         }
@@ -58,7 +58,7 @@ combine_kernel(const DecodeParams p)
             s_aligned = 0;
             if (p.batch * p.num_kv_heads <= kAlignedMaxSegs) {
                 s_prefix[0] = 0;
-                for (int i = 0; i < p.batch; ++i) s_prefix[i + 1] = s_prefix[i] + tiles_of(__ldg(p.seq_lens + i));
+                for (int i = 0; i < p.batch; ++i) s_prefix[i + 1] = s_prefix[i] + seq_tiles(__ldg(p.seq_lens + i), p.window, p.sinks);
                 if (s_prefix[p.batch] > 0)
                     s_aligned = aligned_build(s_prefix, p.batch, p.num_kv_heads, p.grid_ctas, s_e) ? 1 : 0;
             }
@@ -70,7 +70,7 @@ combine_kernel(const DecodeParams p)
 #pragma unroll
     for (int w = 0; w < kMaxGroup; ++w) { before += s_before[w]; total_tiles += s_total[w]; }
 
-    const int T = tiles_of(__ldg(p.seq_lens + b));
+    const int T = seq_tiles(__ldg(p.seq_lens + b), p.window, p.sinks);
     const int64_t row0 = (int64_t)b * p.num_q_heads + kvh * p.group;
     if (T == 0) {
         for (int e = tid; e < p.group * D; e += kCombineThreads) p.out[row0 * D + e] = __float2bfloat16_rn(0.f);

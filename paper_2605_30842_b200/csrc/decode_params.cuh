@@ -30,6 +30,8 @@ struct DecodeParams {
     int page_tile_shift;         // log2(page_size / 16): tiles per page
     int grid_ctas;               // persistent grid size the schedule was sized for
     float scale_log2;            // softmax_scale * log2(e)
+    int window;                  // sliding window in tokens (<= 0: none), schedule.cuh win_tiles
+    int sinks;                   // attention-sink tokens kept at the start of every sequence
 };
 
 // launchers (defined in decode_split.cu / combine.cu / kv_append.cu)

@@ -175,7 +175,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // exclusive prefix of tiles per sequence (warp 0); kept small: no unrolling
         if (warp == 0) {
             if (p.batch <= 32) {
-                const int mine = lane < p.batch ? tiles_of(__ldcg(p.seq_lens + lane)) : 0;
+                const int mine = lane < p.batch ? seq_tiles(__ldcg(p.seq_lens + lane), p.window, p.sinks) : 0;
                 int incl = mine;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -190,7 +190,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 int sum = 0;
 #pragma unroll 1
                 for (int i = 0; i < per; ++i)
-                    if (b0 + i < p.batch) sum += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                    if (b0 + i < p.batch) sum += seq_tiles(__ldcg(p.seq_lens + b0 + i), p.window, p.sinks);
                 int incl = sum;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -202,7 +202,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 for (int i = 0; i < per; ++i)
                     if (b0 + i < p.batch) {
                         prefix[b0 + i] = run;
-                        run += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                        run += seq_tiles(__ldcg(p.seq_lens + b0 + i), p.window, p.sinks);
                     }
                 if (lane == 31) prefix[p.batch] = incl;
             }
@@ -263,7 +263,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     // reads now is at worst useless (the page index is clamped to the table row, a bad page id is an
     // out-of-range tensor coordinate: both harmless for a hint).  HBM is idle while the previous
     // kernel drains its tail; the first real loads after the wait then hit L2.
-    if (warp == kConsumerWarps && c0 < c1) {
+    if (warp == kConsumerWarps && c0 < c1 && p.window <= 0) {  // (identity tile map only)
         const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
         const int64_t rem = c1 - c0;
         int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
@@ -284,7 +284,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         bool same = true;
 #pragma unroll 1
         for (int b = lane; b < p.batch; b += 32)
-            same = same && tiles_of(__ldcg(p.seq_lens + b)) == prefix[b + 1] - prefix[b];
+            same = same && seq_tiles(__ldcg(p.seq_lens + b), p.window, p.sinks) == prefix[b + 1] - prefix[b];
         same = __all_sync(kFull, same);
         if (lane == 0) s_valid = same ? 1 : 0;
     }
@@ -332,8 +332,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const int64_t rem = c1 - x;
             const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
             const int32_t *bt = p.block_table + (int64_t)sp.b * p.max_pages;
+            // sequence tile index -> logical tile (identity unless a sliding window is set)
+            const WinTiles wt = win_tiles(p.window > 0 ? __ldcg(p.seq_lens + sp.b) : 0, p.window, p.sinks);
             for (int base = 0; base < cnt; base += 32) {
-                const int jj = sp.j + base + lane;
+                const int jj = win_logical_tile(wt, sp.j + base + lane);
                 int pid = 0;
                 if (base + lane < cnt) pid = __ldg(bt + (jj >> p.page_tile_shift));
                 const int m = cnt - base < 32 ? cnt - base : 32;
@@ -343,9 +345,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     const uint32_t phase = (uint32_t)(tl >> kStageShift) & 1u;
                     mbar_wait(empty0 + 8 * stage, phase ^ 1u);
                     const int pid_i = __shfl_sync(kFull, pid, i);
+                    const int jj_i = __shfl_sync(kFull, jj, i);
                     if (lane == 0) {
-                        const int row = pid_i * p.page_size +
-                                        (((sp.j + base + i) & tiles_per_page_mask) << kTileShift);
+                        const int row = pid_i * p.page_size + ((jj_i & tiles_per_page_mask) << kTileShift);
                         const uint32_t dst = ring + stage * C::kStageBytes;
                         const uint32_t bar = full0 + 8 * stage;
                         mbar_arrive_expect_tx(bar, C::kStageBytes);
@@ -436,6 +438,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             sg[5] = sp.b * p.num_q_heads + sp.kvh * p.group;
         }
         const int seq_len = __ldcg(p.seq_lens + sp.b);
+        const WinTiles wt = win_tiles(seq_len, p.window, p.sinks);
         const int head0 = sp.kvh * p.group;
 
         // Q fragments (A operand of S = Q K^T): row = head `quad`, rows 8..15 are zero padding.
@@ -465,7 +468,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 #endif
             const uint32_t k_base = ring + stage * C::kStageBytes;
             const uint32_t v_base = k_base + C::kTileBytes;
-            const int valid = seq_len - ((sp.j + (t - n)) << kTileShift);  // >= 1; < 16 only on the last tile
+            // which of the tile's 16 tokens count: all but the ones past seq_len (last tile) and, under a
+            // sliding window, the ones in the gap between the sinks and the window
+            const unsigned alive = win_alive_mask(wt, seq_len, win_logical_tile(wt, sp.j + (t - n)));
 
             // S3: scores for 2 n-tiles of 8 tokens
             float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
@@ -479,18 +484,18 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             }
             float s0 = s[0][0] * p.scale_log2, s1 = s[0][1] * p.scale_log2;
             float s2 = s[1][0] * p.scale_log2, s3 = s[1][1] * p.scale_log2;
-            if (valid < kTileTokens) {
-                // ragged tail: mask by index (never by arithmetic) and zero the dead V rows so
-                // that NaN/Inf garbage past seq_len cannot reach the accumulators (0 * NaN).
+            if (alive != 0xffffu) {
+                // edge tile: mask by index (never by arithmetic) and zero the dead V rows so that
+                // NaN/Inf garbage in tokens that do not count cannot reach the accumulators (0 * NaN).
                 const int tok = 2 * qlane;
-                if (tok >= valid) s0 = -INFINITY;
-                if (tok + 1 >= valid) s1 = -INFINITY;
-                if (tok + 8 >= valid) s2 = -INFINITY;
-                if (tok + 9 >= valid) s3 = -INFINITY;
+                if (!((alive >> tok) & 1u)) s0 = -INFINITY;
+                if (!((alive >> (tok + 1)) & 1u)) s1 = -INFINITY;
+                if (!((alive >> (tok + 8)) & 1u)) s2 = -INFINITY;
+                if (!((alive >> (tok + 9)) & 1u)) s3 = -INFINITY;
                 constexpr int kChunksPerRow = D / 8;  // 16-byte chunks per V row
-                const int dead = (kTileTokens - valid) * kChunksPerRow;
-                for (int idx = lane; idx < dead; idx += 32) {
-                    const int row = valid + idx / kChunksPerRow;
+                for (int idx = lane; idx < kTileTokens * kChunksPerRow; idx += 32) {
+                    const int row = idx / kChunksPerRow;
+                    if ((alive >> row) & 1u) continue;
                     const int ch = idx % kChunksPerRow;
                     const uint32_t a = v_base + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
                     asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");

@@ -35,6 +35,37 @@ constexpr int kMaxBatch = 4096;
 
 COMEM_HD int tiles_of(int seq_len) { return seq_len <= 0 ? 0 : (seq_len + kTileTokens - 1) >> kTileShift; }
 
+// ---- sliding window + attention sinks (reading R17) ---------------------------------
+// The query sits at position L-1 and attends t < sinks or t >= L - window.  Only the tiles that
+// hold a kept token are scheduled and read: the sink tiles [0, sink_tiles) and the window tiles
+// [win_first, tiles_of(L)); a sequence's tile index j (0 <= j < total) maps to a logical tile through
+// win_logical_tile.  window <= 0 or >= L: everything is kept and the map is the identity.
+struct WinTiles {
+    int sink_tiles, win_first, total;
+    int lo, sk;  // kept tokens: t < sk or t >= lo (sk = min(sinks, lo))
+};
+COMEM_HD WinTiles win_tiles(int L, int window, int sinks)
+{
+    WinTiles w;
+    const int all = tiles_of(L);
+    w.lo = (window <= 0 || window >= L) ? 0 : L - window;
+    w.sk = sinks < w.lo ? (sinks > 0 ? sinks : 0) : w.lo;
+    w.win_first = w.lo >> kTileShift;
+    const int st = (w.sk + kTileTokens - 1) >> kTileShift;
+    w.sink_tiles = st < w.win_first ? st : w.win_first;
+    w.total = L <= 0 ? 0 : w.sink_tiles + (all - w.win_first);
+    return w;
+}
+COMEM_HD int seq_tiles(int L, int window, int sinks) { return window <= 0 ? tiles_of(L) : win_tiles(L, window, sinks).total; }
+COMEM_HD int win_logical_tile(const WinTiles &w, int j) { return j < w.sink_tiles ? j : j - w.sink_tiles + w.win_first; }
+// bit i set <=> token 16*tile + i is kept and < L
+COMEM_HD unsigned win_alive_mask(const WinTiles &w, int L, int tile)
+{
+    const int base = tile << kTileShift;
+    auto low = [](int n) -> unsigned { return n <= 0 ? 0u : (n >= kTileTokens ? 0xffffu : (1u << n) - 1u); };
+    return low(L - base) & (low(w.sk - base) | (~low(w.lo - base) & 0xffffu));
+}
+
 COMEM_HD int sched_num_ctas(int64_t total_tiles, int grid_ctas)
 {
     int64_t want = (total_tiles + kMinTilesPerCta - 1) / kMinTilesPerCta;
