@@ -50,7 +50,7 @@ extern "C" {
 enum {
     COMEM_OK = 0,
     COMEM_ERR_INVALID_ARG = 1, /* null required pointer, batch <= 0, Hq % Hkv != 0, bad scale, misaligned */
-    COMEM_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}; page_size not in {16,32}; G not in {1,2,4,8};
+    COMEM_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}; page_size not in {16,32}; G = Hq/Hkv not in 1..8;
                                   batch > COMEM_MAX_BATCH; device is not sm_100 */
     COMEM_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than comem_decode_attn_workspace_bytes() */
     COMEM_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (no device, launch error, ...) */

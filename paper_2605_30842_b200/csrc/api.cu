@@ -63,7 +63,7 @@ int check_shape(int hq, int hkv, int d, int ps, int batch, int max_pages, int64_
     const int g = hq / hkv;
     if (d != 64 && d != 128) return COMEM_ERR_UNSUPPORTED;
     if (ps != 16 && ps != 32) return COMEM_ERR_UNSUPPORTED;
-    if (g != 1 && g != 2 && g != 4 && g != 8) return COMEM_ERR_UNSUPPORTED;
+    if (g < 1 || g > kMaxGroup) return COMEM_ERR_UNSUPPORTED;  // the group is packed into one 8-wide MMA dimension
     if (batch > COMEM_MAX_BATCH) return COMEM_ERR_UNSUPPORTED;
     // TMA row coordinate (page * page_size) and the linear tile count must fit in int32
     if (num_pages * ps >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
@@ -214,7 +214,7 @@ const char *comem_status_string(int status)
     switch (status) {
         case COMEM_OK: return "ok";
         case COMEM_ERR_INVALID_ARG: return "invalid argument";
-        case COMEM_ERR_UNSUPPORTED: return "unsupported shape or device (needs sm_100; head_dim 64/128; page_size 16/32; group 1/2/4/8)";
+        case COMEM_ERR_UNSUPPORTED: return "unsupported shape or device (needs sm_100; head_dim 64/128; page_size 16/32; group 1..8)";
         case COMEM_ERR_WORKSPACE: return "workspace missing or too small";
         case COMEM_ERR_CUDA: return "CUDA error (no device, driver entry point missing, or launch/execution failure)";
         default: return "unknown status";

@@ -26,6 +26,15 @@ def test_small_grid(oracle, G, D, ps):
     check_batch(oracle, b, what=f"G{G} D{D} ps{ps}")
 
 
+@pytest.mark.parametrize("G", [3, 5, 6, 7])
+def test_odd_group_sizes(oracle, G):
+    """Any group size up to 8 is packed into the 8-wide MMA dimension (e.g. 40q/8kv models: G = 5)."""
+    b = W.make_batch([9000, 33, 0, 2500, 17], G * 2, 2, 128, 16, seed=90 + G, device=DEV, poison_unused=True)
+    check_batch(oracle, b, what=f"G{G}")
+    b = W.make_batch([700, 64], G * 3, 3, 64, 32, seed=95 + G, device=DEV, poison_unused=True)
+    check_batch(oracle, b, what=f"G{G} D64 ps32")
+
+
 @pytest.mark.parametrize("hkv", [1, 3, 8])
 def test_kv_head_counts(oracle, hkv):
     b = W.make_batch([700, 33, 4097], 4 * hkv, hkv, 128, 16, seed=7 + hkv, device=DEV, poison_unused=True)
