@@ -45,6 +45,11 @@ def _load():
         lib.oracle_decode_attn_window.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, vp, vp,
                                                   i32, i32, i32]
         lib.oracle_decode_attn_window.restype = i32
+        lib.oracle_decode_attn_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, vp, vp,
+                                               i32, i32, i32]
+        lib.oracle_decode_attn_fp8.restype = i32
+        lib.oracle_e4m3_decode.argtypes = [i32]
+        lib.oracle_e4m3_decode.restype = c.c_double
         lib.oracle_decode_attn_partial.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32,
                                                    i32, i32, i64, i64, i32, vp, vp, vp]
         lib.oracle_decode_attn_partial.restype = i32
@@ -134,6 +139,44 @@ def decode_attn_window(q, k_pages, v_pages, block_table, seq_lens, softmax_scale
                                        int(sink_tokens), _p(out), _p(lse), batch, maxp, int(num_threads))
     if rc != 0:
         raise ValueError(f"oracle_decode_attn_window: invalid argument (rc={rc})")
+    return out, lse
+
+
+def _as_u8(x) -> np.ndarray:
+    """torch uint8 / float8_e4m3fn CPU tensor or numpy uint8 array -> C-contiguous numpy uint8 (raw bytes)."""
+    if isinstance(x, np.ndarray):
+        assert x.dtype == np.uint8, x.dtype
+        return np.ascontiguousarray(x)
+    import torch  # plumbing only
+
+    assert x.device.type == "cpu" and x.element_size() == 1, (x.dtype, x.device)
+    return np.ascontiguousarray(x.contiguous().view(torch.uint8).numpy())
+
+
+def e4m3_decode(byte: int) -> float:
+    """Value of one OCP FP8 E4M3 byte as the oracle reads it (NaN for 0x7f / 0xff)."""
+    return float(_load().oracle_e4m3_decode(int(byte)))
+
+
+def decode_attn_fp8(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, softmax_scale,
+                    window: int = 0, sink_tokens: int = 0, num_threads: int = 0):
+    """FP8 (E4M3 + one fp32 scale per physical page and kv head) KV-cache variant, reading R18.
+    k_pages / v_pages: raw bytes [P, page_size, Hkv, D]; k_scale / v_scale: fp32 [P, Hkv].
+    Returns (out [batch, Hq, D], lse [batch, Hq]) as numpy float64."""
+    lib = _load()
+    qb, kb, vb = as_bits(q), _as_u8(k_pages), _as_u8(v_pages)
+    bt, sl = _as_i32(block_table), _as_i32(seq_lens)
+    batch, hq, hkv, d, ps, maxp, npages = _dims(qb, kb, bt)
+    ks = np.ascontiguousarray(np.asarray(k_scale.cpu().numpy() if hasattr(k_scale, "cpu") else k_scale, np.float32))
+    vs = np.ascontiguousarray(np.asarray(v_scale.cpu().numpy() if hasattr(v_scale, "cpu") else v_scale, np.float32))
+    assert vb.shape == kb.shape and ks.shape == (npages, hkv) and vs.shape == (npages, hkv)
+    out = np.empty((batch, hq, d), np.float64)
+    lse = np.empty((batch, hq), np.float64)
+    rc = lib.oracle_decode_attn_fp8(_p(qb), _p(kb), _p(vb), _p(ks), _p(vs), _p(bt), _p(sl), hq, hkv, d, ps,
+                                    ctypes.c_float(float(np.float32(softmax_scale))), int(window),
+                                    int(sink_tokens), _p(out), _p(lse), batch, maxp, int(num_threads))
+    if rc != 0:
+        raise ValueError(f"oracle_decode_attn_fp8: invalid argument (rc={rc})")
     return out, lse
 
 

@@ -35,6 +35,10 @@
  * oracle_decode_attn_window: W1..W5 (window >= L is the full result bit for bit; window 1 returns
  * the last V; equals full attention over a cache compacted to the kept tokens; masked tokens'
  * contents are irrelevant; brute-force dense masked softmax).
+ * oracle_decode_attn_fp8 / oracle_e4m3_decode: F1..F6 (tests/test_oracle_fp8_pins.py: the 256-entry
+ * decode table vs the format's published values and vs torch's float8_e4m3fn cast; equals the pinned
+ * bf16 oracle on a cache whose values both formats hold exactly; L = 1 closed form; scale
+ * linearity; tail / unused-page poison independence; brute-force dense numpy fp64).
  */
 #include <math.h>
 #include <stdint.h>
@@ -208,6 +212,99 @@ int oracle_decode_attn_window(const uint16_t *q, const uint16_t *k_pages, const 
             const uint16_t *vrow = paged_row(v_pages, bt, t, kvh, num_kv_heads, D, page_size);
             Z += w;
             for (int d = 0; d < D; ++d) o[d] += w * bf16_to_double(vrow[d]);
+        }
+        for (int d = 0; d < D; ++d) o[d] /= Z;
+        if (lse) lse[r] = m + log(Z);
+        free(s);
+        free(qd);
+    }
+    return 0;
+}
+
+/*
+ * FP8 (E4M3) KV-cache variant (the paper names "KV Cache Quantization (Hooper et
+ * al., 2024)" as an orthogonal byte-reducing technique, and gives no format, so the reading is
+ * DESIGN.md R18): K and V are stored one byte per element in the OCP FP8 E4M3 ("fn") encoding
+ *     byte = s eeee mmm :  e = 0      -> (-1)^s * (m / 8) * 2^-6          (subnormal, incl. +-0)
+ *                          e = 1..15  -> (-1)^s * (1 + m / 8) * 2^(e - 7)  (max 0x7e = 448)
+ *                          0x7f, 0xff -> NaN (there is no infinity)
+ * with one fp32 scale per (physical page, kv head) and per pool:
+ *     k_t[d] = k_scale[pid][kvh] * e4m3(K8[pid][slot][kvh][d]),   v_t likewise with v_scale.
+ * Attention over the dequantised cache is then exactly oracle_decode_attn_window (and, with
+ * window <= 0, oracle_decode_attn): same two-pass fp64 statement.  q stays bf16.
+ */
+static double e4m3_to_double(uint8_t byte)
+{
+    const int sign = byte >> 7, e = (byte >> 3) & 15, m = byte & 7;
+    double mag;
+    if (e == 15 && m == 7) return NAN;
+    if (e == 0) mag = ldexp((double)m / 8.0, -6);
+    else mag = ldexp(1.0 + (double)m / 8.0, e - 7);
+    return sign ? -mag : mag;
+}
+
+/* exported so that the decode table itself can be pinned against the format's published values */
+double oracle_e4m3_decode(int byte) { return e4m3_to_double((uint8_t)byte); }
+
+int oracle_decode_attn_fp8(const uint16_t *q,          /* bf16 [batch][Hq][D] */
+                           const uint8_t *k_pages,     /* e4m3 [P][ps][Hkv][D] */
+                           const uint8_t *v_pages,     /* e4m3 [P][ps][Hkv][D] */
+                           const float *k_scale,       /* fp32 [P][Hkv] */
+                           const float *v_scale,       /* fp32 [P][Hkv] */
+                           const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                           int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                           int window, int sink_tokens, double *out, double *lse, int batch,
+                           int max_pages_per_seq, int num_threads)
+{
+    if (!q || !k_pages || !v_pages || !k_scale || !v_scale || !block_table || !seq_lens || !out) return 1;
+    if (num_q_heads <= 0 || num_kv_heads <= 0 || num_q_heads % num_kv_heads != 0) return 1;
+    if (head_dim <= 0 || page_size <= 0 || batch <= 0 || sink_tokens < 0) return 1;
+    const int G = num_q_heads / num_kv_heads;
+    const int D = head_dim;
+    const int64_t rows = (int64_t)batch * num_q_heads;
+    const double scale = (double)softmax_scale;
+#ifdef _OPENMP
+    if (num_threads <= 0) num_threads = omp_get_max_threads();
+#else
+    (void)num_threads;
+#endif
+#pragma omp parallel for schedule(dynamic, 1) num_threads(num_threads)
+    for (int64_t r = 0; r < rows; ++r) {
+        const int b = (int)(r / num_q_heads), h = (int)(r % num_q_heads);
+        const int kvh = h / G;
+        const int64_t L = seq_lens[b];
+        const int64_t first_in_window = (window <= 0 || window >= L) ? 0 : L - window;
+        const int32_t *bt = block_table + (int64_t)b * max_pages_per_seq;
+        double *o = out + r * D;
+        for (int d = 0; d < D; ++d) o[d] = 0.0;
+        if (L <= 0) {
+            if (lse) lse[r] = -INFINITY;
+            continue;
+        }
+        double *qd = (double *)malloc(sizeof(double) * D);
+        double *s = (double *)malloc(sizeof(double) * (size_t)L);
+        const uint16_t *qrow = q + ((int64_t)b * num_q_heads + h) * D;
+        for (int d = 0; d < D; ++d) qd[d] = bf16_to_double(qrow[d]);
+        double m = -INFINITY;
+        for (int64_t t = 0; t < L; ++t) {
+            if (!(t < sink_tokens || t >= first_in_window)) continue;
+            const int64_t pid = bt[t / page_size], slot = t % page_size;
+            const uint8_t *krow = k_pages + ((pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
+            const double ks = (double)k_scale[pid * num_kv_heads + kvh];
+            double dot = 0.0;
+            for (int d = 0; d < D; ++d) dot += qd[d] * (ks * e4m3_to_double(krow[d]));
+            s[t] = scale * dot;
+            if (s[t] > m) m = s[t];
+        }
+        double Z = 0.0;
+        for (int64_t t = 0; t < L; ++t) {
+            if (!(t < sink_tokens || t >= first_in_window)) continue;
+            const int64_t pid = bt[t / page_size], slot = t % page_size;
+            const uint8_t *vrow = v_pages + ((pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
+            const double vs = (double)v_scale[pid * num_kv_heads + kvh];
+            const double w = exp(s[t] - m);
+            Z += w;
+            for (int d = 0; d < D; ++d) o[d] += w * (vs * e4m3_to_double(vrow[d]));
         }
         for (int d = 0; d < D; ++d) o[d] /= Z;
         if (lse) lse[r] = m + log(Z);

@@ -91,6 +91,96 @@ class DecodeBatch:
         return {"q": cs(self.q), "block_table": cs(self.block_table), "seq_lens": cs(self.seq_lens)}
 
 
+@dataclasses.dataclass
+class Fp8DecodeBatch:
+    """A decode batch whose KV cache is stored as FP8 E4M3 bytes with one fp32 scale per
+    (physical page, kv head) and per pool (reading R18)."""
+
+    q: torch.Tensor            # bf16 [batch, Hq, D]
+    k_pages: torch.Tensor      # uint8 (E4M3 bytes) [P, page_size, Hkv, D]
+    v_pages: torch.Tensor      # uint8 (E4M3 bytes) [P, page_size, Hkv, D]
+    k_scale: torch.Tensor      # fp32 [P, Hkv]
+    v_scale: torch.Tensor      # fp32 [P, Hkv]
+    block_table: torch.Tensor  # int32 [batch, max_pages_per_seq]
+    seq_lens: torch.Tensor     # int32 [batch]
+    softmax_scale: float
+    name: str = ""
+    seed: int = 0
+
+    batch = property(lambda self: self.q.shape[0])
+    num_q_heads = property(lambda self: self.q.shape[1])
+    num_kv_heads = property(lambda self: self.k_pages.shape[2])
+    head_dim = property(lambda self: self.q.shape[2])
+    page_size = property(lambda self: self.k_pages.shape[1])
+    num_pages = property(lambda self: self.k_pages.shape[0])
+    max_pages_per_seq = property(lambda self: self.block_table.shape[1])
+
+    def algorithmic_bytes(self, kept_tokens: Optional[int] = None) -> int:
+        """K and V bytes (1 B per element) of the tokens read, their page scales (2 x 4 B per page and
+        kv head) and Q."""
+        ps = self.page_size
+        lens = self.seq_lens.to(torch.int64)
+        tokens = int(lens.sum().item()) if kept_tokens is None else int(kept_tokens)
+        pages = int(((lens + ps - 1) // ps).sum().item()) if kept_tokens is None else (int(kept_tokens) + ps - 1) // ps
+        return (tokens * self.num_kv_heads * self.head_dim * 2 + pages * self.num_kv_heads * 8 +
+                self.batch * self.num_q_heads * self.head_dim * 2)
+
+    def to(self, device) -> "Fp8DecodeBatch":
+        mv = lambda t: t.to(device)
+        return dataclasses.replace(self, q=mv(self.q), k_pages=mv(self.k_pages), v_pages=mv(self.v_pages),
+                                   k_scale=mv(self.k_scale), v_scale=mv(self.v_scale),
+                                   block_table=mv(self.block_table), seq_lens=mv(self.seq_lens))
+
+
+E4M3_MAX = 448.0
+
+
+def _quantize_pool_e4m3(pages: torch.Tensor, chunk_pages: int = 4096):
+    """[P, ps, Hkv, D] bf16 -> (uint8 E4M3 bytes, fp32 scale [P, Hkv]).  Input recipe, not the method:
+    scale = amax over the (page, kv head) block / 448 (1 where the block is all zero, NaN where it holds
+    nothing but NaN poison); byte = torch's round-to-nearest float8_e4m3fn cast of x / scale.  NaN
+    poison stays NaN (0x7f)."""
+    P, ps, hkv, d = pages.shape
+    out = torch.empty((P, ps, hkv, d), dtype=torch.uint8, device=pages.device)
+    scale = torch.empty((P, hkv), dtype=torch.float32, device=pages.device)
+    for i in range(0, P, chunk_pages):
+        x = pages[i:i + chunk_pages].float()
+        isnan = torch.isnan(x)
+        amax = torch.where(isnan, torch.zeros_like(x), x.abs()).amax(dim=(1, 3))
+        sc = torch.where(amax > 0, amax / E4M3_MAX, torch.ones_like(amax))
+        sc = torch.where(isnan.all(dim=3).all(dim=1), torch.full_like(sc, float("nan")), sc)
+        y = x / torch.where(torch.isnan(sc), torch.ones_like(sc), sc).view(-1, 1, hkv, 1)
+        out[i:i + chunk_pages] = y.to(torch.float8_e4m3fn).view(torch.uint8)
+        scale[i:i + chunk_pages] = sc
+    return out, scale
+
+
+def quantize_batch_fp8(batch: "DecodeBatch") -> Fp8DecodeBatch:
+    """The same seeded batch with its cache stored as E4M3 + per-(page, kv head) scales."""
+    k8, ks = _quantize_pool_e4m3(batch.k_pages)
+    v8, vs = _quantize_pool_e4m3(batch.v_pages)
+    return Fp8DecodeBatch(q=batch.q, k_pages=k8, v_pages=v8, k_scale=ks, v_scale=vs,
+                          block_table=batch.block_table, seq_lens=batch.seq_lens,
+                          softmax_scale=batch.softmax_scale, name=(batch.name + "+fp8kv") if batch.name else "fp8kv",
+                          seed=batch.seed)
+
+
+def permute_pages_fp8(batch: Fp8DecodeBatch, seed: int) -> Fp8DecodeBatch:
+    """permute_pages for the FP8 cache: pages and their scale rows move together."""
+    g = torch.Generator(device="cpu")
+    g.manual_seed(seed)
+    perm = torch.randperm(batch.num_pages, generator=g)          # new_id = perm[old_id]
+    inv = torch.empty_like(perm)
+    inv[perm] = torch.arange(batch.num_pages)
+    dev = batch.k_pages.device
+    invd = inv.to(dev)
+    bt = batch.block_table.cpu().to(torch.int64)
+    bt2 = torch.where(bt >= 0, perm[bt.clamp_min(0)], bt).to(torch.int32)
+    return dataclasses.replace(batch, k_pages=batch.k_pages[invd], v_pages=batch.v_pages[invd],
+                               k_scale=batch.k_scale[invd], v_scale=batch.v_scale[invd],
+                               block_table=bt2.to(dev))
+
+
 def f32(x: float) -> float:
     """Round a python float to fp32 (the ABI's softmax_scale is a C float)."""
     return float(np.float32(x))
