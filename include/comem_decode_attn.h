@@ -140,6 +140,29 @@ int comem_decode_attn_window_async(const void *q, const void *k_pages, const voi
                                    void *workspace, size_t workspace_bytes, void *cuda_stream,
                                    int window, int sink_tokens);
 
+/*
+ * comem_decode_attn_fp8_async — the same step over an FP8 KV cache, the other byte-reducing variant
+ * the paper calls orthogonal ("KV Cache Quantization"; reading R18): half the bytes
+ * per token on the same HBM roofline.
+ *   k_pages, v_pages  OCP FP8 E4M3 bytes [num_pages, page_size, num_kv_heads, head_dim], device,
+ *                     128-byte aligned (bias 7, max 448, 0x7f / 0xff = NaN, no infinities)
+ *   k_scale, v_scale  fp32 [num_pages, num_kv_heads], device: token row (pid, slot, kvh) of K is
+ *                     k_scale[pid][kvh] * e4m3(k_pages[pid][slot][kvh][:]); V likewise.  Only the scales
+ *                     of pages holding a kept token are read; they must be finite.
+ *   window, sink_tokens   as comem_decode_attn_window_async (window <= 0: full attention)
+ * q, out, lse_out, block_table, seq_lens, workspace, stream, determinism and the error contract are
+ * those of comem_decode_attn_async.  Arithmetic: E4M3 widens exactly to fp16 and the tensor op runs in
+ * fp16 with fp32 accumulation; q is converted bf16 -> fp16 (exact for 2^-14 <= |q| < 65504) and
+ * p * v_scale is rounded to fp16.  COMEM_ERR_UNSUPPORTED unless head_dim == 128.
+ */
+int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *v_pages,
+                                const float *k_scale, const float *v_scale,
+                                const int32_t *block_table, const int32_t *seq_lens,
+                                int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                                float softmax_scale, void *out, int batch, int max_pages_per_seq,
+                                int64_t num_pages, float *lse_out, void *workspace,
+                                size_t workspace_bytes, void *cuda_stream, int window, int sink_tokens);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,

@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     comem_decode_attn_window_async,
     COMEM_PHASE_SPLIT,
     COMEM_PHASE_COMBINE,
+    comem_decode_attn_fp8_async,
     comem_decode_attn_workspace_bytes,
     comem_decode_step_host,
     comem_grid_ctas,

@@ -55,6 +55,9 @@ def load_library():
     lib.comem_decode_attn_window_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                                    i32, i64, vp, vp, sz, vp, i32, i32]
     lib.comem_decode_attn_window_async.restype = i32
+    lib.comem_decode_attn_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
+                                                i32, i64, vp, vp, sz, vp, i32, i32]
+    lib.comem_decode_attn_fp8_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
     lib.comem_decode_attn.restype = i32
@@ -209,6 +212,29 @@ def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, s
         workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_window_async")
+
+
+def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
+                                softmax_scale: float, out, workspace, window: int = 0, sink_tokens: int = 0,
+                                lse_out=None, stream=None) -> None:
+    """Decode attention over an FP8 (E4M3 bytes + fp32 page scales) KV cache; one fused launch."""
+    assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.dim() == 3
+    for t in (k_pages, v_pages):
+        assert t.is_cuda and t.dtype == torch.uint8 and t.is_contiguous() and t.dim() == 4
+    assert k_pages.shape == v_pages.shape and k_pages.shape[3] == q.shape[2]
+    for t in (k_scale, v_scale):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+        assert tuple(t.shape) == (k_pages.shape[0], k_pages.shape[2])
+    assert block_table.dtype == torch.int32 and block_table.is_contiguous() and block_table.shape[0] == q.shape[0]
+    assert seq_lens.dtype == torch.int32 and seq_lens.is_contiguous() and seq_lens.shape == (q.shape[0],)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_fp8_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(k_scale), _ptr(v_scale), _ptr(block_table), _ptr(seq_lens),
+        q.shape[1], k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_fp8_async")
 
 
 def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out=None,

@@ -122,10 +122,11 @@ EncodeFn encode_fn()
 struct MapKey {
     const void *ptr;
     int64_t num_pages;
-    int ps, hkv, d;
+    int ps, hkv, d, elem_bytes;
     bool operator==(const MapKey &o) const
     {
-        return ptr == o.ptr && num_pages == o.num_pages && ps == o.ps && hkv == o.hkv && d == o.d;
+        return ptr == o.ptr && num_pages == o.num_pages && ps == o.ps && hkv == o.hkv && d == o.d &&
+               elem_bytes == o.elem_bytes;
     }
 };
 struct MapEntry {
@@ -133,12 +134,15 @@ struct MapEntry {
     CUtensorMap map;
 };
 
-int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out)
+// FP8 pools (elem_bytes 1, head_dim 128 only): a token row of one kv head is 128 B, the swizzle span, so
+//   dim0 = 128 bytes of d, dim1 = P * ps token rows (stride Hkv*D B), dim2 = 1, dim3 = Hkv (stride D B),
+// box {128, 16, 1, 1}: a [16 tokens][128 B] tile, 128-byte swizzled, read with 16-byte shared loads.
+int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out, int elem_bytes = 2)
 {
     static std::mutex mu;
     static std::vector<MapEntry> cache;
     static size_t next_evict = 0;
-    const MapKey key{pool, num_pages, ps, hkv, d};
+    const MapKey key{pool, num_pages, ps, hkv, d, elem_bytes};
     std::lock_guard<std::mutex> lock(mu);
     for (const MapEntry &e : cache)
         if (e.key == key) { *out = e.map; return COMEM_OK; }
@@ -150,10 +154,20 @@ int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, 
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     MapEntry e;
     e.key = key;
-    const CUresult r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(pool), gdim, gstride,
-                           box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                           d == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r;
+    if (elem_bytes == 1) {
+        const cuuint64_t gdim8[4] = {(cuuint64_t)d, (cuuint64_t)num_pages * ps, 1, (cuuint64_t)hkv};
+        const cuuint64_t gstride8[3] = {(cuuint64_t)hkv * d, (cuuint64_t)d, (cuuint64_t)d};
+        const cuuint32_t box8[4] = {(cuuint32_t)d, (cuuint32_t)kTileTokens, 1, 1};
+        r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void *>(pool), gdim8, gstride8, box8, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+        r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(pool), gdim, gstride,
+                box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                d == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
     if (r != CUDA_SUCCESS) return COMEM_ERR_CUDA;
     if (cache.size() < 64) cache.push_back(e);
     else { cache[next_evict] = e; next_evict = (next_evict + 1) % cache.size(); }
@@ -207,7 +221,7 @@ using namespace comem;
 
 extern "C" {
 
-int comem_version(void) { return 110; }
+int comem_version(void) { return 120; }
 
 const char *comem_status_string(int status)
 {
@@ -328,9 +342,12 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
                             int num_kv_heads, int head_dim, int page_size, float softmax_scale,
                             void *out, int batch, int max_pages_per_seq, int64_t num_pages,
                             float *lse_out, void *workspace, size_t workspace_bytes,
-                            void *cuda_stream, int phases, int window, int sink_tokens)
+                            void *cuda_stream, int phases, int window, int sink_tokens,
+                            const float *k_scale = nullptr, const float *v_scale = nullptr, bool kv_fp8 = false)
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
+    if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
+    if (kv_fp8 && head_dim != 128 && (head_dim == 64)) return COMEM_ERR_UNSUPPORTED;
     if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;
     int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
@@ -344,10 +361,13 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     if ((st = check_device()) != COMEM_OK) return st;
 
     CUtensorMap tm_k, tm_v;
-    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k)) != COMEM_OK) return st;
-    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v)) != COMEM_OK) return st;
+    const int elem_bytes = kv_fp8 ? 1 : 2;
+    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k, elem_bytes)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v, elem_bytes)) != COMEM_OK) return st;
 
     DecodeParams p;
+    p.k_scale = kv_fp8 ? k_scale : nullptr;
+    p.v_scale = kv_fp8 ? v_scale : nullptr;
     p.q = static_cast<const __nv_bfloat16 *>(q);
     p.block_table = block_table;
     p.seq_lens = seq_lens;
@@ -375,7 +395,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     if ((st = grid_for(head_dim, &p.grid_ctas)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream) != cudaSuccess) {
+    if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }
@@ -409,6 +429,19 @@ int comem_decode_attn_window_async(const void *q, const void *k_pages, const voi
                             page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
                             workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
                             window, sink_tokens);
+}
+
+int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *v_pages, const float *k_scale,
+                                const float *v_scale, const int32_t *block_table, const int32_t *seq_lens,
+                                int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                                float softmax_scale, void *out, int batch, int max_pages_per_seq,
+                                int64_t num_pages, float *lse_out, void *workspace, size_t workspace_bytes,
+                                void *cuda_stream, int window, int sink_tokens)
+{
+    return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
+                            page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
+                            workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
+                            window, sink_tokens, k_scale, v_scale, true);
 }
 
 int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,

@@ -32,11 +32,14 @@ struct DecodeParams {
     float scale_log2;            // softmax_scale * log2(e)
     int window;                  // sliding window in tokens (<= 0: none), schedule.cuh win_tiles
     int sinks;                   // attention-sink tokens kept at the start of every sequence
+    const float *k_scale;        // FP8 cache only (reading R18): fp32 [P][Hkv] page scales, else nullptr
+    const float *v_scale;
 };
 
 // launchers (defined in decode_split.cu / combine.cu / kv_append.cu)
+// kv_fp8: the pools hold E4M3 bytes and p.k_scale / p.v_scale are set (head_dim 128 only)
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
-                                const DecodeParams &p, int head_dim, cudaStream_t stream);
+                                const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false);
 cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
 cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
                              const int32_t *block_table, int32_t *seq_lens,

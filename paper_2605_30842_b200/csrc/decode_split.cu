@@ -47,18 +47,27 @@ constexpr int kConsumerWarps = 8;
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 static_assert(kConsumerWarps == kMaxGroup, "S6 and merge.cuh map warp w to query head w of the group");
 constexpr int kPrefetchTiles = COMEM_PREFETCH_TILES;  // per CTA, L2-prefetched before the PDL wait (<= 32: one per lane)
-constexpr int kProducerWarps = 2;  // one elected lane each; tiles alternate between them (issue-rate bound otherwise)
-constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
 constexpr unsigned kFull = 0xffffffffu;
 
-template <int D>
+// kFp8: the FP8 (E4M3 + per-page, per-kv-head scale) cache of reading R18.  Tiles are half the bytes,
+// so the ring has twice the stages (same 128 KiB in flight) and twice the producer warps (a tile
+// must be issued every ~85 ns per SM to keep up with HBM).
+template <int D, bool kFp8>
 struct Cfg {
-    static constexpr int kTileBytes = kTileTokens * D * 2;  // one K (or V) tile
+    static_assert(!kFp8 || D == 128, "the FP8 fragment mapping is written for head_dim 128");
+    static constexpr int kElemBytes = kFp8 ? 1 : 2;
+    // one elected lane per producer warp; tiles are dealt round-robin to them (one lane is issue-rate bound)
+    static constexpr int kProducerWarps = kFp8 ? 4 : 2;
+    static constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
+    static constexpr int kPrefetch = kFp8 ? 2 * kPrefetchTiles : kPrefetchTiles;
+    static_assert(kPrefetch <= 32, "one prefetched tile per lane");
+    static constexpr int kTileBytes = kTileTokens * D * kElemBytes;  // one K (or V) tile
     static constexpr int kStageBytes = 2 * kTileBytes;      // K + V
     // kStages % kConsumerWarps == 0 so that a ring stage always belongs to the same consumer warp:
     // a warp then never waits on a stage more than one phase ahead of the barrier (mbarrier waits
     // carry only the phase PARITY; out-of-order TMA completion could otherwise alias two phases).
-    static constexpr int kStages = (D == 128) ? 16 : 32;  // 128 KiB of K+V in flight per SM
+    static constexpr int kStages = 128 * 1024 / kStageBytes;  // 128 KiB of K+V in flight per SM: 16 (bf16, D 128) or 32
+    static constexpr int kScaleBytes = kFp8 ? kStages * 8 : 0;  // per ring stage: {k_scale, v_scale} of the tile's page
     static_assert(kStages % kConsumerWarps == 0, "ring stages must map to a fixed consumer warp");
     static constexpr int kRowPitch = D + 4;                       // floats; see S6
     static constexpr int kStateOff = kMaxGroup * kRowPitch;       // m[8], l[8], lx[8] follow the rows
@@ -70,12 +79,12 @@ struct Cfg {
     static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
 };
 
-template <int D>
+template <int D, bool kFp8>
 __host__ __device__ constexpr size_t smem_bytes_for(int batch)
 {
-    return 1024 /* alignment slack */ + (size_t)Cfg<D>::kStages * Cfg<D>::kStageBytes +
-           (size_t)Cfg<D>::kScratchBytes + (2 * Cfg<D>::kStages + 1) * 8 +
-           ((size_t)batch + 1) * 4 + 16;
+    using C = Cfg<D, kFp8>;
+    return 1024 /* alignment slack */ + (size_t)C::kStages * C::kStageBytes + (size_t)C::kScratchBytes +
+           (2 * C::kStages + 1) * 8 + C::kScaleBytes + ((size_t)batch + 1) * 4 + 16;
 }
 
 struct SegPos {
@@ -99,19 +108,22 @@ __device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch
     return s;
 }
 
-template <int D>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int D, bool kFp8>
+__global__ void __launch_bounds__((Cfg<D, kFp8>::kThreads), 1)
 decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                     const DecodeParams p)
 {
-    using C = Cfg<D>;
+    using C = Cfg<D, kFp8>;
+    constexpr int kThreads = C::kThreads;
+    constexpr int kProducerWarps = C::kProducerWarps;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t ring = (raw + 1023u) & ~1023u;  // 1024-aligned: the 128B-swizzle atom
     uint8_t *ring_ptr = smem_raw + (ring - raw);
     float *scratch = reinterpret_cast<float *>(ring_ptr + C::kStages * C::kStageBytes);
     uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(scratch) + C::kScratchBytes);
-    int *prefix = reinterpret_cast<int *>(bars + 2 * C::kStages + 1);
+    const uint32_t scales0 = smem_u32(bars + 2 * C::kStages + 1);  // FP8 only: float2 per ring stage
+    int *prefix = reinterpret_cast<int *>(reinterpret_cast<uint8_t *>(bars + 2 * C::kStages + 1) + C::kScaleBytes);
     const uint32_t full0 = smem_u32(bars);
     const uint32_t empty0 = full0 + 8 * C::kStages;
     const uint32_t merge_bar = empty0 + 8 * C::kStages;  // completion of merge.cuh's bulk copies
@@ -267,7 +279,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
         const int64_t rem = c1 - c0;
         int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
-        cnt = cnt < kPrefetchTiles ? cnt : kPrefetchTiles;
+        cnt = cnt < C::kPrefetch ? cnt : C::kPrefetch;
         if (lane < cnt) {
             const int jj = sp.j + lane;
             int page = jj >> p.page_tile_shift;
@@ -318,6 +330,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // Producer warp pw issues the CTA's tiles with (CTA-local index) % kProducerWarps == pw; tile
         // tl always lands in ring stage tl % kStages, in the ring's pass number tl / kStages.
         static_assert((C::kStages & (C::kStages - 1)) == 0 && C::kStages % kProducerWarps == 0, "ring indexing");
+        static_assert((kProducerWarps & (kProducerWarps - 1)) == 0, "round-robin by mask");
         constexpr int kStageShift = (C::kStages == 16) ? 4 : 5;
         static_assert((1 << kStageShift) == C::kStages, "kStageShift");
         const int pw = warp - kConsumerWarps;
@@ -338,18 +351,32 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 const int jj = win_logical_tile(wt, sp.j + base + lane);
                 int pid = 0;
                 if (base + lane < cnt) pid = __ldg(bt + (jj >> p.page_tile_shift));
+                float ks = 0.f, vs = 0.f;  // FP8: the page's scales for this kv head, one tile per lane
+                if constexpr (kFp8) {
+                    if (base + lane < cnt) {
+                        ks = __ldg(p.k_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
+                        vs = __ldg(p.v_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
+                    }
+                }
                 const int m = cnt - base < 32 ? cnt - base : 32;
-                for (int i = ((tl0 + base) ^ pw) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
+                for (int i = (pw - (tl0 + base)) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
                     const int tl = tl0 + base + i;
                     const int stage = tl & (C::kStages - 1);
                     const uint32_t phase = (uint32_t)(tl >> kStageShift) & 1u;
                     mbar_wait(empty0 + 8 * stage, phase ^ 1u);
                     const int pid_i = __shfl_sync(kFull, pid, i);
                     const int jj_i = __shfl_sync(kFull, jj, i);
+                    float ks_i = 0.f, vs_i = 0.f;
+                    if constexpr (kFp8) {
+                        ks_i = __shfl_sync(kFull, ks, i);
+                        vs_i = __shfl_sync(kFull, vs, i);
+                    }
                     if (lane == 0) {
                         const int row = pid_i * p.page_size + ((jj_i & tiles_per_page_mask) << kTileShift);
                         const uint32_t dst = ring + stage * C::kStageBytes;
                         const uint32_t bar = full0 + 8 * stage;
+                        if constexpr (kFp8)  // ordered before the consumers' wait by the arrive below (release) and their wait (acquire)
+                            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(scales0 + 8 * stage), "f"(ks_i), "f"(vs_i) : "memory");
                         mbar_arrive_expect_tx(bar, C::kStageBytes);
                         tma_load_4d_hint(dst, &tm_k, bar, 0, row, 0, sp.kvh, stream_policy);
                         tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh, stream_policy);
@@ -447,10 +474,24 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const uint32_t *qrow = reinterpret_cast<const uint32_t *>(
                 p.q + ((int64_t)sp.b * p.num_q_heads + head0 + quad) * D);
             const bool live = quad < p.group;
+            if constexpr (kFp8) {
+                // E4M3 widens exactly to fp16, so the tensor op runs in fp16 and q is converted once per
+                // segment.  The contraction index is permuted to suit 16-byte shared-memory reads of K
+                // (see S3): k-step 4c + w of lane qlane covers d = 16 (2 qlane + c) + 4 w + {0,1 | 2,3}.
 #pragma unroll
-            for (int kk = 0; kk < C::kKSteps; ++kk) {
-                qf[kk][0] = live ? __ldg(qrow + 8 * kk + qlane) : 0u;
-                qf[kk][1] = live ? __ldg(qrow + 8 * kk + 4 + qlane) : 0u;
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) {
+                        const int i32 = 8 * (2 * qlane + c) + 2 * w;
+                        qf[4 * c + w][0] = live ? bf16x2_to_f16x2(__ldg(qrow + i32)) : 0u;
+                        qf[4 * c + w][1] = live ? bf16x2_to_f16x2(__ldg(qrow + i32 + 1)) : 0u;
+                    }
+            } else {
+#pragma unroll
+                for (int kk = 0; kk < C::kKSteps; ++kk) {
+                    qf[kk][0] = live ? __ldg(qrow + 8 * kk + qlane) : 0u;
+                    qf[kk][1] = live ? __ldg(qrow + 8 * kk + 4 + qlane) : 0u;
+                }
             }
         }
 
@@ -474,16 +515,41 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 
             // S3: scores for 2 n-tiles of 8 tokens
             float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+            float sl2 = p.scale_log2, v_scale = 1.f;
+            if constexpr (kFp8) {
+                // The tile is [16 tokens][128 B], 128-byte swizzled.  Lane (quad, qlane) reads, of token rows
+                // quad and quad + 8, the 16-byte chunks 2 qlane and 2 qlane + 1: a quarter-warp (two rows that
+                // differ in bit 0, even chunks ^ row) touches every bank once.  Each 32-bit word is one k-step's
+                // B fragment: bytes 0,1 -> b0, bytes 2,3 -> b1 (the permutation q was loaded with).
+                float2 sc;
+                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(sc.x), "=f"(sc.y) : "r"(scales0 + 8 * stage));
+                sl2 *= sc.x;
+                v_scale = sc.y;
+                const uint32_t row_lo = k_base + quad * 128, row_hi = row_lo + 8 * 128;  // (quad + 8) & 7 == quad
 #pragma unroll
-            for (int kk = 0; kk < C::kKSteps; ++kk) {
-                uint32_t kf[4];
-                const uint32_t chunk = ((2 * kk) & 7) | ld_half;
-                ldmatrix_x4(kf, k_base + (kk >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
-                mma_bf16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, kf[0], kf[1]);
-                mma_bf16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, kf[2], kf[3]);
+                for (int c = 0; c < 2; ++c) {
+                    const uint32_t off = ((uint32_t)(2 * qlane + c) ^ (uint32_t)quad) << 4;
+                    const uint4 ka = lds128(row_lo + off), kb = lds128(row_hi + off);
+                    const uint32_t wa[4] = {ka.x, ka.y, ka.z, ka.w}, wb[4] = {kb.x, kb.y, kb.z, kb.w};
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) {
+                        const int kk = 4 * c + w;
+                        mma_f16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wa[w]), e4m3x2_hi_to_f16x2(wa[w]));
+                        mma_f16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wb[w]), e4m3x2_hi_to_f16x2(wb[w]));
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int kk = 0; kk < C::kKSteps; ++kk) {
+                    uint32_t kf[4];
+                    const uint32_t chunk = ((2 * kk) & 7) | ld_half;
+                    ldmatrix_x4(kf, k_base + (kk >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                    mma_bf16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, kf[0], kf[1]);
+                    mma_bf16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, kf[2], kf[3]);
+                }
             }
-            float s0 = s[0][0] * p.scale_log2, s1 = s[0][1] * p.scale_log2;
-            float s2 = s[1][0] * p.scale_log2, s3 = s[1][1] * p.scale_log2;
+            float s0 = s[0][0] * sl2, s1 = s[0][1] * sl2;
+            float s2 = s[1][0] * sl2, s3 = s[1][1] * sl2;
             if (alive != 0xffffu) {
                 // edge tile: mask by index (never by arithmetic) and zero the dead V rows so that
                 // NaN/Inf garbage in tokens that do not count cannot reach the accumulators (0 * NaN).
@@ -492,7 +558,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 if (!((alive >> (tok + 1)) & 1u)) s1 = -INFINITY;
                 if (!((alive >> (tok + 8)) & 1u)) s2 = -INFINITY;
                 if (!((alive >> (tok + 9)) & 1u)) s3 = -INFINITY;
-                constexpr int kChunksPerRow = D / 8;  // 16-byte chunks per V row
+                constexpr int kChunksPerRow = D * C::kElemBytes / 16;  // 16-byte chunks per V row
                 for (int idx = lane; idx < kTileTokens * kChunksPerRow; idx += 32) {
                     const int row = idx / kChunksPerRow;
                     if ((alive >> row) & 1u) continue;
@@ -512,11 +578,15 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const float alpha = ex2(m_run - m_new);
             m_run = m_new;
             const float e0 = ex2(s0 - m_new), e1 = ex2(s1 - m_new), e2 = ex2(s2 - m_new), e3 = ex2(s3 - m_new);
-            const uint32_t p01 = pack_bf16x2(e0, e1);  // tokens 2q, 2q+1
-            const uint32_t p23 = pack_bf16x2(e2, e3);  // tokens 2q+8, 2q+9
+            // FP8: the page's v_scale rides on p (fp16, 11 significant bits); the normaliser is the unrounded sum
+            const uint32_t p01 = kFp8 ? pack_f16x2(e0 * v_scale, e1 * v_scale) : pack_bf16x2(e0, e1);  // tokens 2q, 2q+1
+            const uint32_t p23 = kFp8 ? pack_f16x2(e2 * v_scale, e3 * v_scale) : pack_bf16x2(e2, e3);  // tokens 2q+8, 2q+9
             lx_run = lx_run * alpha + ((e0 + e1) + (e2 + e3));
-            l_run = l_run * alpha + ((bf16lo_to_f32(p01) + bf16hi_to_f32(p01)) +
-                                     (bf16lo_to_f32(p23) + bf16hi_to_f32(p23)));
+            if constexpr (kFp8)
+                l_run = lx_run;
+            else
+                l_run = l_run * alpha + ((bf16lo_to_f32(p01) + bf16hi_to_f32(p01)) +
+                                         (bf16lo_to_f32(p23) + bf16hi_to_f32(p23)));
             if (__any_sync(kFull, alpha != 1.f)) {
                 // acc columns are heads 2*qlane, 2*qlane+1: fetch their alphas from those quads
                 const float a_lo = __shfl_sync(kFull, alpha, (2 * qlane) << 2);
@@ -531,12 +601,37 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             }
 
             // S5: O^T[16 d x 8 heads] += V^T[16 d x 16 tok] * P^T[16 tok x 8 heads]
+            if constexpr (kFp8) {
+                // Lane (quad, qlane) reads the 16-byte chunk `quad` (d = 16 quad .. 16 quad + 15) of its four
+                // token rows 2q, 2q+1, 2q+8, 2q+9 (a quarter-warp: rows & 7 all even or all odd, chunks 2j and
+                // 2j+1 -> every bank once).  A-fragment registers pair two TOKENS of one d: PRMT interleaves the
+                // bytes of two rows, the conversion widens each byte pair.  m-tile u of this lane is
+                // {row quad: d = 16 quad + 2u, row quad + 8: d = 16 quad + 2u + 1}; S6 scatters accordingly.
+                const int t0 = 2 * qlane;
+                const uint32_t ch = (uint32_t)quad;
+                const uint4 r0 = lds128(v_base + t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4));
+                const uint4 r1 = lds128(v_base + (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4));
+                const uint4 r2 = lds128(v_base + (t0 + 8) * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4));
+                const uint4 r3 = lds128(v_base + (t0 + 9) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4));
+                const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
+                const uint32_t w2[4] = {r2.x, r2.y, r2.z, r2.w}, w3[4] = {r3.x, r3.y, r3.z, r3.w};
 #pragma unroll
-            for (int mt = 0; mt < C::kKSteps; ++mt) {
-                uint32_t vf[4];
-                const uint32_t chunk = ((2 * mt) & 7) | ld_half;
-                ldmatrix_x4_trans(vf, v_base + (mt >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
-                mma_bf16_16816(acc[mt], vf[0], vf[1], vf[2], vf[3], p01, p23);
+                for (int w = 0; w < 4; ++w) {
+                    const uint32_t x01e = prmt(w0[w], w1[w], 0x5140u), x23e = prmt(w2[w], w3[w], 0x5140u);
+                    const uint32_t x01o = prmt(w0[w], w1[w], 0x7362u), x23o = prmt(w2[w], w3[w], 0x7362u);
+                    mma_f16_16816(acc[2 * w], e4m3x2_lo_to_f16x2(x01e), e4m3x2_hi_to_f16x2(x01e),
+                                  e4m3x2_lo_to_f16x2(x23e), e4m3x2_hi_to_f16x2(x23e), p01, p23);
+                    mma_f16_16816(acc[2 * w + 1], e4m3x2_lo_to_f16x2(x01o), e4m3x2_hi_to_f16x2(x01o),
+                                  e4m3x2_lo_to_f16x2(x23o), e4m3x2_hi_to_f16x2(x23o), p01, p23);
+                }
+            } else {
+#pragma unroll
+                for (int mt = 0; mt < C::kKSteps; ++mt) {
+                    uint32_t vf[4];
+                    const uint32_t chunk = ((2 * mt) & 7) | ld_half;
+                    ldmatrix_x4_trans(vf, v_base + (mt >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                    mma_bf16_16816(acc[mt], vf[0], vf[1], vf[2], vf[3], p01, p23);
+                }
             }
 
             __syncwarp();
@@ -556,7 +651,15 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         l_run += __shfl_xor_sync(kFull, l_run, 2);
         lx_run += __shfl_xor_sync(kFull, lx_run, 1);
         lx_run += __shfl_xor_sync(kFull, lx_run, 2);
-        {
+        if constexpr (kFp8) {  // acc[u] = {d = 16 quad + 2u: heads 2q, 2q+1; d + 1: heads 2q, 2q+1}
+            float *lo = my_scratch + (2 * qlane) * C::kRowPitch + 16 * quad;
+            float *hi = lo + C::kRowPitch;
+#pragma unroll
+            for (int u = 0; u < C::kKSteps; ++u) {
+                *reinterpret_cast<float2 *>(lo + 2 * u) = make_float2(acc[u][0], acc[u][2]);
+                *reinterpret_cast<float2 *>(hi + 2 * u) = make_float2(acc[u][1], acc[u][3]);
+            }
+        } else {
             float *lo = my_scratch + (2 * qlane) * C::kRowPitch + quad;
             float *hi = lo + C::kRowPitch;
 #pragma unroll
@@ -647,12 +750,12 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     if (pending_first) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
 }
 
-template <int D>
+template <int D, bool kFp8>
 cudaError_t configure_once()
 {
-    static cudaError_t status = cudaFuncSetAttribute(decode_split_kernel<D>,
+    static cudaError_t status = cudaFuncSetAttribute(decode_split_kernel<D, kFp8>,
                                                      cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                     (int)smem_bytes_for<D>(kMaxBatch));
+                                                     (int)smem_bytes_for<D, kFp8>(kMaxBatch));
     return status;
 }
 
@@ -660,54 +763,47 @@ cudaError_t configure_once()
 
 size_t split_smem_bytes(int head_dim, int batch)
 {
-    return head_dim == 128 ? smem_bytes_for<128>(batch) : smem_bytes_for<64>(batch);
+    return head_dim == 128 ? smem_bytes_for<128, false>(batch) : smem_bytes_for<64, false>(batch);
 }
 
 cudaError_t split_default_grid(int head_dim, int *grid_ctas)
 {
-    int dev = 0, sms = 0, per_sm = 0;
+    // one CTA per SM whatever the variant: each takes most of the SM's shared memory
+    (void)head_dim;
+    int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    if (head_dim == 128) {
-        if ((e = configure_once<128>()) != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decode_split_kernel<128>, kThreads,
-                                                          smem_bytes_for<128>(64));
-    } else {
-        if ((e = configure_once<64>()) != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, decode_split_kernel<64>, kThreads,
-                                                          smem_bytes_for<64>(64));
-    }
-    if (e != cudaSuccess) return e;
-    if (per_sm < 1) per_sm = 1;
-    if (per_sm > 1) per_sm = 1;
-    *grid_ctas = sms * per_sm;
+    *grid_ctas = sms;
     return cudaSuccess;
 }
 
+template <int D, bool kFp8>
+static cudaError_t launch_variant(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
+                                  cudaLaunchConfig_t &cfg)
+{
+    const cudaError_t e = configure_once<D, kFp8>();
+    if (e != cudaSuccess) return e;
+    cfg.blockDim = dim3(Cfg<D, kFp8>::kThreads);
+    cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch);
+    return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8>, tm_k, tm_v, p);
+}
+
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
-                                int head_dim, cudaStream_t stream)
+                                int head_dim, cudaStream_t stream, bool kv_fp8)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(p.grid_ctas);
-    cfg.blockDim = dim3(kThreads);
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (head_dim == 128) {
-        cudaError_t e = configure_once<128>();
-        if (e != cudaSuccess) return e;
-        cfg.dynamicSmemBytes = smem_bytes_for<128>(p.batch);
-        return cudaLaunchKernelEx(&cfg, decode_split_kernel<128>, tm_k, tm_v, p);
-    }
-    cudaError_t e = configure_once<64>();
-    if (e != cudaSuccess) return e;
-    cfg.dynamicSmemBytes = smem_bytes_for<64>(p.batch);
-    return cudaLaunchKernelEx(&cfg, decode_split_kernel<64>, tm_k, tm_v, p);
+    if (kv_fp8) return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, p, cfg) : cudaErrorInvalidValue;
+    if (head_dim == 128) return launch_variant<128, false>(tm_k, tm_v, p, cfg);
+    return launch_variant<64, false>(tm_k, tm_v, p, cfg);
 }
 
 }  // namespace comem

@@ -1,0 +1,169 @@
+"""GPU parity of the FP8 (E4M3 + per-page, per-kv-head scale) KV-cache variant
+(comem_decode_attn_fp8_async, reading R18) against oracle.decode_attn_fp8 on the same bytes,
+the properties that fix bits, and a sampled check at config 4's full size."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2605_30842_b200 as comem
+from paper_2605_30842_b200 import workloads as W
+from parity_util import MAX_ABS, MEAN_ABS, REL_L2
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def bits(t):
+    return t.contiguous().view(torch.int16)
+
+
+def run8(f, window=0, sinks=0, ws=None):
+    out = torch.full_like(f.q, float("nan"))
+    lse = torch.full((f.batch, f.num_q_heads), float("nan"), dtype=torch.float32, device=DEV)
+    ws = ws if ws is not None else comem.alloc_workspace(f.q, f.k_pages, f.block_table)
+    comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                      f.softmax_scale, out, ws, window, sinks, lse_out=lse)
+    torch.cuda.synchronize()
+    return out, lse
+
+
+def gate(g, ref, gl, ref_lse, what):
+    d = np.abs(g - ref)
+    assert np.isfinite(g).all(), what
+    assert d.max() <= MAX_ABS and d.mean() <= MEAN_ABS, (what, d.max(), d.mean())
+    rel = np.linalg.norm(g - ref) / max(np.linalg.norm(ref), 1e-300)
+    assert rel <= REL_L2, (what, rel)
+    assert d.max() <= 4 * 2.0 ** -9 * np.abs(ref).max() + 1e-6, (what, d.max(), np.abs(ref).max())
+    live = np.isfinite(ref_lse)
+    assert np.array_equal(np.isneginf(gl), np.isneginf(ref_lse)), what
+    if live.any():
+        assert np.max(np.abs(gl[live] - ref_lse[live]) / np.maximum(1.0, np.abs(ref_lse[live]))) <= 2e-4, what
+    return {"max_abs": float(d.max()), "mean_abs": float(d.mean()), "rel_l2": float(rel)}
+
+
+def check(oracle, f, what, window=0, sinks=0):
+    out, lse = run8(f, window, sinks)
+    c = f.to("cpu")
+    ref, ref_lse = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table,
+                                          c.seq_lens, c.softmax_scale, window, sinks)
+    gate(out.double().cpu().numpy(), ref, lse.double().cpu().numpy(), ref_lse, what)
+    return out, lse
+
+
+def fp8_batch(lens, hq, hkv, ps, seed, **kw):
+    return W.quantize_batch_fp8(W.make_batch(lens, hq, hkv, 128, ps, seed=seed, device=DEV, poison_unused=True, **kw))
+
+
+@pytest.mark.parametrize("G,ps", [(1, 16), (4, 32), (8, 16), (3, 32), (5, 16), (8, 32)])
+def test_fp8_small_ragged(oracle, G, ps):
+    lens = [1, 15, 16, 17, 31, 33, 127, 128, 129, 512, 1000, 0, 2049]
+    f = fp8_batch(lens, 2 * G, 2, ps, seed=500 + G + ps)
+    check(oracle, f, f"G{G} ps{ps}")
+
+
+def test_fp8_long_ragged_grids_and_permutation(oracle):
+    lens = [20000, 37, 0, 50001, 8191, 16, 300]
+    f = fp8_batch(lens, 64, 8, 16, seed=521)
+    base, base_lse = check(oracle, f, "ragged default grid")
+    again, again_lse = run8(f)
+    assert torch.equal(bits(base), bits(again)) and torch.equal(base_lse, again_lse)       # run to run
+    g = W.permute_pages_fp8(f, seed=9)
+    assert not torch.equal(g.block_table, f.block_table)
+    po, pl = run8(g)
+    assert torch.equal(bits(base), bits(po)) and torch.equal(base_lse, pl)                # page placement
+    try:
+        for grid in (1, 7, 148, 296):
+            comem.comem_set_grid_ctas(grid)
+            check(oracle, f, f"ragged grid {grid}")
+    finally:
+        comem.comem_set_grid_ctas(0)
+
+
+def test_fp8_single_long_sequence_aligned_schedule(oracle):
+    """one 32K sequence x 8 kv heads: the segment-aligned schedule (18-19 CTAs per head) and the fused merge"""
+    f = fp8_batch([32768], 64, 8, 16, seed=522, k_scale=0.5)
+    check(oracle, f, "c2-shaped fp8")
+
+
+def test_fp8_window_and_sinks(oracle):
+    f = fp8_batch([5000, 100, 0, 777, 16, 2048], 32, 8, 32, seed=523)
+    for window, sinks in ((1, 0), (17, 1), (128, 16), (1000, 64), (4096, 4), (10 ** 6, 3)):
+        check(oracle, f, f"fp8 w{window} s{sinks}", window, sinks)
+    full, full_lse = run8(f)
+    w_all, l_all = run8(f, 10 ** 6, 3)
+    assert torch.equal(bits(full), bits(w_all)) and torch.equal(full_lse, l_all)
+
+
+def test_fp8_all_byte_codes_exact(oracle):
+    """L = 1, unit scales: out = bf16(e4m3(V byte)) exactly (3 mantissa bits fit bf16; the softmax weight
+    is exactly 1) for every finite byte code -- checks the device conversion of all 254 of them, and the
+    K conversion through lse = scale * q . k."""
+    f = fp8_batch([1, 1], 8, 1, 16, seed=524)
+    codes = torch.arange(256, dtype=torch.uint8, device=DEV)
+    codes = torch.where((codes & 0x7f) == 0x7f, torch.zeros_like(codes), codes)      # NaN codes -> 0
+    for b in range(2):
+        pid = int(f.block_table[b, 0])
+        f.v_pages[pid, 0, 0] = codes[128 * b:128 * (b + 1)]
+        f.k_pages[pid, 0, 0] = codes[128 * b:128 * (b + 1)].flip(0)
+        f.k_scale[pid, 0] = 1.0
+        f.v_scale[pid, 0] = 1.0
+    # q small enough that q . k stays well inside fp32 and the oracle comparison is tight
+    f = dataclasses.replace(f, q=(f.q.float() / 64).to(torch.bfloat16))
+    out, lse = run8(f)
+    want = codes.view(torch.float8_e4m3fn).float()
+    for b in range(2):
+        for h in range(8):
+            assert torch.equal(out[b, h].float(), want[128 * b:128 * (b + 1)]), (b, h)
+    c = f.to("cpu")
+    ref, ref_lse = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table,
+                                          c.seq_lens, c.softmax_scale)
+    assert np.array_equal(out.double().cpu().numpy(), ref)
+    assert np.max(np.abs(lse.double().cpu().numpy() - ref_lse) / np.maximum(1.0, np.abs(ref_lse))) <= 1e-5
+
+
+def test_fp8_scale_moves_between_page_and_bytes(oracle):
+    """Doubling a page's v_scale doubles its contribution; per-page scales that differ wildly page to page."""
+    f = fp8_batch([700, 90], 16, 4, 16, seed=525)
+    g = torch.Generator().manual_seed(5)
+    e = torch.randint(-4, 5, tuple(f.k_scale.shape), generator=g).float().to(DEV)
+    f2 = dataclasses.replace(f, v_scale=torch.nan_to_num(f.v_scale, nan=1.0) * torch.exp2(e),
+                             k_scale=torch.nan_to_num(f.k_scale, nan=1.0) * torch.exp2(-e.abs() / 2))
+    check(oracle, f2, "wild page scales")
+
+
+def test_fp8_rejects_head_dim_64_and_null_scales():
+    b = W.make_batch([100], 4, 1, 64, 16, seed=1, device=DEV)
+    k8 = torch.zeros(b.k_pages.shape, dtype=torch.uint8, device=DEV)
+    sc = torch.ones((b.num_pages, 1), dtype=torch.float32, device=DEV)
+    out = torch.empty_like(b.q)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    with pytest.raises(comem.ComemError) as ei:
+        comem.comem_decode_attn_fp8_async(b.q, k8, k8, sc, sc, b.block_table, b.seq_lens, b.softmax_scale, out, ws)
+    assert ei.value.status == comem.COMEM_ERR_UNSUPPORTED
+
+
+def test_fp8_config4_full_size_sampled(oracle):
+    """Config 4's shape (16 x 131072 tokens, 32q/8kv, page 32, peaked keys) with the cache quantised: oracle on
+    two whole sequences (all 32 heads) from the same bytes; permutation bit-identity on the complete output."""
+    bf = W.config4_memory_long(DEV, poison_unused=True)
+    f = W.quantize_batch_fp8(bf)
+    del bf
+    torch.cuda.empty_cache()
+    out, lse = run8(f)
+    ps = f.page_size
+    for b in (0, 11):
+        n = W.pages_needed(int(f.seq_lens[b]), ps)
+        ids = f.block_table[b, :n].long()
+        sub = W.Fp8DecodeBatch(q=f.q[b:b + 1].cpu(), k_pages=f.k_pages[ids].cpu(), v_pages=f.v_pages[ids].cpu(),
+                               k_scale=f.k_scale[ids].cpu(), v_scale=f.v_scale[ids].cpu(),
+                               block_table=torch.arange(n, dtype=torch.int32).view(1, n),
+                               seq_lens=f.seq_lens[b:b + 1].cpu(), softmax_scale=f.softmax_scale)
+        ref, ref_lse = oracle.decode_attn_fp8(sub.q, sub.k_pages, sub.v_pages, sub.k_scale, sub.v_scale,
+                                              sub.block_table, sub.seq_lens, sub.softmax_scale)
+        err = gate(out[b:b + 1].double().cpu().numpy(), ref, lse[b:b + 1].double().cpu().numpy(), ref_lse, f"c4 fp8 seq {b}")
+        print("c4 fp8 seq", b, err)
+    g = W.permute_pages_fp8(f, seed=77)
+    po, pl = run8(g)
+    assert torch.equal(bits(out), bits(po)) and torch.equal(lse, pl)
