@@ -61,6 +61,10 @@ def parse_args():
     ap.add_argument("--window", type=int, default=0,
                     help="extra: time comem_decode_attn_window_async on the C4 batch with this sliding window")
     ap.add_argument("--sinks", type=int, default=64, help="attention-sink tokens for --window")
+    ap.add_argument("--kv-fp8", action="store_true",
+                    help="extra: time comem_decode_attn_fp8_async (E4M3 cache + page scales) on --workload c2|c3|c4")
+    ap.add_argument("--kv-layout", default="nhd", choices=["nhd", "hnd"],
+                    help="for --kv-fp8: pools [P, page, Hkv, D] (nhd) or [P, Hkv, page, D] (hnd)")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
@@ -587,6 +591,78 @@ def run_window(args) -> int:
     return 0
 
 
+def run_fp8(args) -> int:
+    """Extra: the FP8 (E4M3 + per-page, per-kv-head scale) KV-cache variant on the
+    C2 / C3 / C4 batch, quantised by the input recipe (workloads.quantize_batch_fp8).  Algorithmic bytes =
+    1 B per K and V element of every token + 8 B of scales per (page, kv head) + Q; the same HBM roofline
+    applies.  Steps rotate over enough pools to exceed L2 and are replayed from one CUDA graph.
+    One JSON line; not the driver's bench line."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    pools = []
+    for bf in make_pools(args.workload, device, 0, 0):
+        f8 = W.quantize_batch_fp8(bf)
+        del bf
+        pools.append(W.to_hnd(f8) if args.kv_layout == "hnd" else f8)
+        del f8
+    torch.cuda.empty_cache()
+    nbytes = pools[0].algorithmic_bytes()
+    bf16_bytes = int(pools[0].seq_lens.to(torch.int64).sum().item()) * pools[0].num_kv_heads * pools[0].head_dim * 4
+    stream = torch.cuda.Stream(device)
+    outs = [torch.empty_like(b.q) for b in pools]
+    ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream,
+                               kv_layout=pools[0].kv_layout)
+    peaks = {"hbm_gbs": FALLBACK_PEAK_GBS}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peaks["hbm_gbs"] = float(json.load(fh)["hbm_gbs"])
+    except Exception:  # noqa: BLE001
+        pass
+    with torch.cuda.stream(stream):
+        def step(i):
+            b = pools[i % len(pools)]
+            comem.comem_decode_attn_fp8_async(b.q, b.k_pages, b.v_pages, b.k_scale, b.v_scale, b.block_table,
+                                              b.seq_lens, b.softmax_scale, outs[i % len(pools)], ws, stream=stream,
+                                              kv_layout=b.kv_layout)
+        for i in range(len(pools)):
+            step(i)
+        stream.synchronize()
+        per_graph = max(len(pools), 4)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            for i in range(per_graph):
+                step(i)
+        est_us = nbytes / 5e6 + 8
+        replays = max(4, min(int(2e6 / (est_us * per_graph)), max(1, args.steps // per_graph)))
+        for _ in range(3):
+            g.replay()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(replays):
+            g.replay()
+        e1.record(stream)
+        stream.synchronize()
+    us = e0.elapsed_time(e1) * 1e3 / (replays * per_graph)
+    gbs = nbytes / us / 1e3
+    print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload),
+                      "kv_layout": pools[0].kv_layout,
+                      "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
+                      "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
+                      "frac_of_measured_peak": gbs / peaks["hbm_gbs"], "peak": peaks["hbm_gbs"],
+                      "bf16_cache_bytes_same_tokens": bf16_bytes,
+                      "equivalent_bf16_gbs": bf16_bytes / us / 1e3,
+                      "l2": "cold: steps rotate over %d pools (%.2f GiB)" % (len(pools), len(pools) * nbytes / 2 ** 30)}),
+          flush=True)
+    return 0
+
+
 def main() -> int:
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -594,6 +670,8 @@ def main() -> int:
         return run_reference(args, rank)
     if args.window > 0:
         return run_window(args) if rank == 0 else 0
+    if args.kv_fp8:
+        return run_fp8(args) if rank == 0 else 0
     if args.affine:
         return run_affine(args) if rank == 0 else 0
     if args.workload == "c5":

@@ -45,7 +45,7 @@ def _load():
         lib.oracle_decode_attn_window.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, vp, vp,
                                                   i32, i32, i32]
         lib.oracle_decode_attn_window.restype = i32
-        lib.oracle_decode_attn_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, vp, vp,
+        lib.oracle_decode_attn_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, i32, i32, i32, vp, vp,
                                                i32, i32, i32]
         lib.oracle_decode_attn_fp8.restype = i32
         lib.oracle_e4m3_decode.argtypes = [i32]
@@ -159,14 +159,18 @@ def e4m3_decode(byte: int) -> float:
 
 
 def decode_attn_fp8(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, softmax_scale,
-                    window: int = 0, sink_tokens: int = 0, num_threads: int = 0):
+                    window: int = 0, sink_tokens: int = 0, num_threads: int = 0, kv_layout: str = "NHD"):
     """FP8 (E4M3 + one fp32 scale per physical page and kv head) KV-cache variant, reading R18.
-    k_pages / v_pages: raw bytes [P, page_size, Hkv, D]; k_scale / v_scale: fp32 [P, Hkv].
+    k_pages / v_pages: raw bytes [P, page_size, Hkv, D] (kv_layout "NHD") or [P, Hkv, page_size, D] ("HND");
+    k_scale / v_scale: fp32 [P, Hkv].
     Returns (out [batch, Hq, D], lse [batch, Hq]) as numpy float64."""
     lib = _load()
     qb, kb, vb = as_bits(q), _as_u8(k_pages), _as_u8(v_pages)
     bt, sl = _as_i32(block_table), _as_i32(seq_lens)
+    assert kv_layout in ("NHD", "HND")
     batch, hq, hkv, d, ps, maxp, npages = _dims(qb, kb, bt)
+    if kv_layout == "HND":
+        hkv, ps = ps, hkv
     ks = np.ascontiguousarray(np.asarray(k_scale.cpu().numpy() if hasattr(k_scale, "cpu") else k_scale, np.float32))
     vs = np.ascontiguousarray(np.asarray(v_scale.cpu().numpy() if hasattr(v_scale, "cpu") else v_scale, np.float32))
     assert vb.shape == kb.shape and ks.shape == (npages, hkv) and vs.shape == (npages, hkv)
@@ -174,7 +178,8 @@ def decode_attn_fp8(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens
     lse = np.empty((batch, hq), np.float64)
     rc = lib.oracle_decode_attn_fp8(_p(qb), _p(kb), _p(vb), _p(ks), _p(vs), _p(bt), _p(sl), hq, hkv, d, ps,
                                     ctypes.c_float(float(np.float32(softmax_scale))), int(window),
-                                    int(sink_tokens), _p(out), _p(lse), batch, maxp, int(num_threads))
+                                    int(sink_tokens), 1 if kv_layout == "HND" else 0, _p(out), _p(lse), batch, maxp,
+                                    int(num_threads))
     if rc != 0:
         raise ValueError(f"oracle_decode_attn_fp8: invalid argument (rc={rc})")
     return out, lse

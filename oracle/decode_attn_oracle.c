@@ -232,6 +232,8 @@ int oracle_decode_attn_window(const uint16_t *q, const uint16_t *k_pages, const 
  *     k_t[d] = k_scale[pid][kvh] * e4m3(K8[pid][slot][kvh][d]),   v_t likewise with v_scale.
  * Attention over the dequantised cache is then exactly oracle_decode_attn_window (and, with
  * window <= 0, oracle_decode_attn): same two-pass fp64 statement.  q stays bf16.
+ * kv_hnd != 0: the pools are laid out [P][Hkv][ps][D] ("HND") instead of [P][ps][Hkv][D]; only the
+ * address of a token row changes.
  */
 static double e4m3_to_double(uint8_t byte)
 {
@@ -253,7 +255,7 @@ int oracle_decode_attn_fp8(const uint16_t *q,          /* bf16 [batch][Hq][D] */
                            const float *v_scale,       /* fp32 [P][Hkv] */
                            const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
                            int num_kv_heads, int head_dim, int page_size, float softmax_scale,
-                           int window, int sink_tokens, double *out, double *lse, int batch,
+                           int window, int sink_tokens, int kv_hnd, double *out, double *lse, int batch,
                            int max_pages_per_seq, int num_threads)
 {
     if (!q || !k_pages || !v_pages || !k_scale || !v_scale || !block_table || !seq_lens || !out) return 1;
@@ -289,7 +291,8 @@ int oracle_decode_attn_fp8(const uint16_t *q,          /* bf16 [batch][Hq][D] */
         for (int64_t t = 0; t < L; ++t) {
             if (!(t < sink_tokens || t >= first_in_window)) continue;
             const int64_t pid = bt[t / page_size], slot = t % page_size;
-            const uint8_t *krow = k_pages + ((pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
+            const uint8_t *krow = k_pages + (kv_hnd ? (pid * num_kv_heads + kvh) * page_size + slot
+                                                    : (pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
             const double ks = (double)k_scale[pid * num_kv_heads + kvh];
             double dot = 0.0;
             for (int d = 0; d < D; ++d) dot += qd[d] * (ks * e4m3_to_double(krow[d]));
@@ -300,7 +303,8 @@ int oracle_decode_attn_fp8(const uint16_t *q,          /* bf16 [batch][Hq][D] */
         for (int64_t t = 0; t < L; ++t) {
             if (!(t < sink_tokens || t >= first_in_window)) continue;
             const int64_t pid = bt[t / page_size], slot = t % page_size;
-            const uint8_t *vrow = v_pages + ((pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
+            const uint8_t *vrow = v_pages + (kv_hnd ? (pid * num_kv_heads + kvh) * page_size + slot
+                                                    : (pid * page_size + slot) * num_kv_heads + kvh) * (int64_t)D;
             const double vs = (double)v_scale[pid * num_kv_heads + kvh];
             const double w = exp(s[t] - m);
             Z += w;

@@ -56,7 +56,7 @@ def load_library():
                                                    i32, i64, vp, vp, sz, vp, i32, i32]
     lib.comem_decode_attn_window_async.restype = i32
     lib.comem_decode_attn_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
-                                                i32, i64, vp, vp, sz, vp, i32, i32]
+                                                i32, i64, vp, vp, sz, vp, i32, i32, i32]
     lib.comem_decode_attn_fp8_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
@@ -134,14 +134,15 @@ def comem_workspace_init_async(workspace: torch.Tensor, batch: int, num_q_heads:
         raise ComemError(st, "comem_workspace_init_async")
 
 
-def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.Tensor, stream=None) -> torch.Tensor:
+def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.Tensor, stream=None,
+                    kv_layout: str = "NHD") -> torch.Tensor:
     """torch.empty of the size the library asks for (device memory is torch's job), then the
     library's one-time comem_workspace_init_async on it (on `stream` or the current stream)."""
-    n = comem_decode_attn_workspace_bytes(q.shape[0], q.shape[1], k_pages.shape[2], q.shape[2],
-                                          k_pages.shape[1], block_table.shape[1])
+    ps, hkv = (k_pages.shape[2], k_pages.shape[1]) if kv_layout == "HND" else (k_pages.shape[1], k_pages.shape[2])
+    n = comem_decode_attn_workspace_bytes(q.shape[0], q.shape[1], hkv, q.shape[2], ps, block_table.shape[1])
     ws = torch.empty(n, dtype=torch.uint8, device=q.device)
     with torch.cuda.device(q.device):
-        comem_workspace_init_async(ws, q.shape[0], q.shape[1], k_pages.shape[2], q.shape[2], stream)
+        comem_workspace_init_async(ws, q.shape[0], q.shape[1], hkv, q.shape[2], stream)
     return ws
 
 
@@ -216,23 +217,27 @@ def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, s
 
 def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
                                 softmax_scale: float, out, workspace, window: int = 0, sink_tokens: int = 0,
-                                lse_out=None, stream=None) -> None:
-    """Decode attention over an FP8 (E4M3 bytes + fp32 page scales) KV cache; one fused launch."""
+                                lse_out=None, stream=None, kv_layout: str = "NHD") -> None:
+    """Decode attention over an FP8 (E4M3 bytes + fp32 page scales) KV cache; one fused launch.
+    kv_layout "NHD": pools [P, page_size, Hkv, D]; "HND": pools [P, Hkv, page_size, D]."""
+    assert kv_layout in ("NHD", "HND")
+    hnd = kv_layout == "HND"
     assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.dim() == 3
     for t in (k_pages, v_pages):
         assert t.is_cuda and t.dtype == torch.uint8 and t.is_contiguous() and t.dim() == 4
     assert k_pages.shape == v_pages.shape and k_pages.shape[3] == q.shape[2]
+    page_size, hkv = (k_pages.shape[2], k_pages.shape[1]) if hnd else (k_pages.shape[1], k_pages.shape[2])
     for t in (k_scale, v_scale):
         assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
-        assert tuple(t.shape) == (k_pages.shape[0], k_pages.shape[2])
+        assert tuple(t.shape) == (k_pages.shape[0], hkv)
     assert block_table.dtype == torch.int32 and block_table.is_contiguous() and block_table.shape[0] == q.shape[0]
     assert seq_lens.dtype == torch.int32 and seq_lens.is_contiguous() and seq_lens.shape == (q.shape[0],)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
     st = load_library().comem_decode_attn_fp8_async(
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(k_scale), _ptr(v_scale), _ptr(block_table), _ptr(seq_lens),
-        q.shape[1], k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[1], hkv, q.shape[2], page_size, ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens))
+        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens), 1 if hnd else 0)
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_fp8_async")
 

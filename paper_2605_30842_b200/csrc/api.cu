@@ -122,11 +122,11 @@ EncodeFn encode_fn()
 struct MapKey {
     const void *ptr;
     int64_t num_pages;
-    int ps, hkv, d, elem_bytes;
+    int ps, hkv, d, elem_bytes, hnd;
     bool operator==(const MapKey &o) const
     {
         return ptr == o.ptr && num_pages == o.num_pages && ps == o.ps && hkv == o.hkv && d == o.d &&
-               elem_bytes == o.elem_bytes;
+               elem_bytes == o.elem_bytes && hnd == o.hnd;
     }
 };
 struct MapEntry {
@@ -137,12 +137,14 @@ struct MapEntry {
 // FP8 pools (elem_bytes 1, head_dim 128 only): a token row of one kv head is 128 B, the swizzle span, so
 //   dim0 = 128 bytes of d, dim1 = P * ps token rows (stride Hkv*D B), dim2 = 1, dim3 = Hkv (stride D B),
 // box {128, 16, 1, 1}: a [16 tokens][128 B] tile, 128-byte swizzled, read with 16-byte shared loads.
-int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out, int elem_bytes = 2)
+// HND layout [P][Hkv][ps][D]: dim1 = ps slots (stride D B), dim2 = Hkv (stride ps*D B), dim3 = P (stride Hkv*ps*D B).
+int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out, int elem_bytes = 2,
+                   int hnd = 0)
 {
     static std::mutex mu;
     static std::vector<MapEntry> cache;
     static size_t next_evict = 0;
-    const MapKey key{pool, num_pages, ps, hkv, d, elem_bytes};
+    const MapKey key{pool, num_pages, ps, hkv, d, elem_bytes, hnd};
     std::lock_guard<std::mutex> lock(mu);
     for (const MapEntry &e : cache)
         if (e.key == key) { *out = e.map; return COMEM_OK; }
@@ -156,8 +158,12 @@ int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, 
     e.key = key;
     CUresult r;
     if (elem_bytes == 1) {
-        const cuuint64_t gdim8[4] = {(cuuint64_t)d, (cuuint64_t)num_pages * ps, 1, (cuuint64_t)hkv};
-        const cuuint64_t gstride8[3] = {(cuuint64_t)hkv * d, (cuuint64_t)d, (cuuint64_t)d};
+        cuuint64_t gdim8[4] = {(cuuint64_t)d, (cuuint64_t)num_pages * ps, 1, (cuuint64_t)hkv};
+        cuuint64_t gstride8[3] = {(cuuint64_t)hkv * d, (cuuint64_t)d, (cuuint64_t)d};
+        if (hnd) {
+            gdim8[1] = (cuuint64_t)ps; gdim8[2] = (cuuint64_t)hkv; gdim8[3] = (cuuint64_t)num_pages;
+            gstride8[0] = (cuuint64_t)d; gstride8[1] = (cuuint64_t)ps * d; gstride8[2] = (cuuint64_t)hkv * ps * d;
+        }
         const cuuint32_t box8[4] = {(cuuint32_t)d, (cuuint32_t)kTileTokens, 1, 1};
         r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void *>(pool), gdim8, gstride8, box8, estr,
                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -343,11 +349,13 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
                             void *out, int batch, int max_pages_per_seq, int64_t num_pages,
                             float *lse_out, void *workspace, size_t workspace_bytes,
                             void *cuda_stream, int phases, int window, int sink_tokens,
-                            const float *k_scale = nullptr, const float *v_scale = nullptr, bool kv_fp8 = false)
+                            const float *k_scale = nullptr, const float *v_scale = nullptr, bool kv_fp8 = false,
+                            int kv_layout = COMEM_KV_LAYOUT_NHD)
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
     if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
-    if (kv_fp8 && head_dim != 128 && (head_dim == 64)) return COMEM_ERR_UNSUPPORTED;
+    if (kv_fp8 && head_dim == 64) return COMEM_ERR_UNSUPPORTED;
+    if (kv_layout != COMEM_KV_LAYOUT_NHD && !(kv_fp8 && kv_layout == COMEM_KV_LAYOUT_HND)) return COMEM_ERR_INVALID_ARG;
     if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;
     int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
@@ -362,12 +370,14 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
 
     CUtensorMap tm_k, tm_v;
     const int elem_bytes = kv_fp8 ? 1 : 2;
-    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k, elem_bytes)) != COMEM_OK) return st;
-    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v, elem_bytes)) != COMEM_OK) return st;
+    const int hnd = kv_layout == COMEM_KV_LAYOUT_HND ? 1 : 0;
+    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k, elem_bytes, hnd)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v, elem_bytes, hnd)) != COMEM_OK) return st;
 
     DecodeParams p;
     p.k_scale = kv_fp8 ? k_scale : nullptr;
     p.v_scale = kv_fp8 ? v_scale : nullptr;
+    p.kv_hnd = hnd;
     p.q = static_cast<const __nv_bfloat16 *>(q);
     p.block_table = block_table;
     p.seq_lens = seq_lens;
@@ -436,12 +446,12 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 int num_q_heads, int num_kv_heads, int head_dim, int page_size,
                                 float softmax_scale, void *out, int batch, int max_pages_per_seq,
                                 int64_t num_pages, float *lse_out, void *workspace, size_t workspace_bytes,
-                                void *cuda_stream, int window, int sink_tokens)
+                                void *cuda_stream, int window, int sink_tokens, int kv_layout)
 {
     return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
                             page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
                             workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
-                            window, sink_tokens, k_scale, v_scale, true);
+                            window, sink_tokens, k_scale, v_scale, true, kv_layout);
 }
 
 int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,

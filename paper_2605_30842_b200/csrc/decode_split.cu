@@ -31,6 +31,9 @@
 //     stand-alone K2 (combine.cu) does the merge.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
+#ifndef COMEM_FP8_TILES_PER_PASS
+#define COMEM_FP8_TILES_PER_PASS 1
+#endif
 #ifndef COMEM_PREFETCH_TILES
 #define COMEM_PREFETCH_TILES 16
 #endif
@@ -38,6 +41,7 @@
 #include "ptx.cuh"
 #include "schedule.cuh"
 #include "merge.cuh"
+#include <type_traits>
 
 namespace comem {
 
@@ -77,6 +81,7 @@ struct Cfg {
         kConsumerWarps * kScratchFloatsPerWarp * 4 > MergeCfg<D>::kStageBytes
             ? kConsumerWarps * kScratchFloatsPerWarp * 4 : MergeCfg<D>::kStageBytes;
     static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
+    static constexpr int kTilesPerPass = kFp8 ? COMEM_FP8_TILES_PER_PASS : 1;  // tiles a consumer warp takes per online-softmax update
 };
 
 template <int D, bool kFp8>
@@ -285,9 +290,12 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             int page = jj >> p.page_tile_shift;
             page = page < p.max_pages ? page : p.max_pages - 1;
             const int pid = __ldcg(p.block_table + (int64_t)sp.b * p.max_pages + page);
-            const int row = pid * p.page_size + ((jj & ((1 << p.page_tile_shift) - 1)) << kTileShift);
-            tma_prefetch_tile_4d(&tm_k, 0, row, 0, sp.kvh);
-            tma_prefetch_tile_4d(&tm_v, 0, row, 0, sp.kvh);
+            const int slot0 = (jj & ((1 << p.page_tile_shift) - 1)) << kTileShift;
+            // tensor coordinates of the tile: {d, token row, -, kv head}, or {d, slot, kv head, page} for the HND layout
+            const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid * p.page_size + slot0;
+            const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid : sp.kvh;
+            tma_prefetch_tile_4d(&tm_k, 0, c1, c2, c3);
+            tma_prefetch_tile_4d(&tm_v, 0, c1, c2, c3);
         }
     }
     pdl_wait_prior_grid();
@@ -347,17 +355,39 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             const int32_t *bt = p.block_table + (int64_t)sp.b * p.max_pages;
             // sequence tile index -> logical tile (identity unless a sliding window is set)
             const WinTiles wt = win_tiles(p.window > 0 ? __ldcg(p.seq_lens + sp.b) : 0, p.window, p.sinks);
-            for (int base = 0; base < cnt; base += 32) {
-                const int jj = win_logical_tile(wt, sp.j + base + lane);
-                int pid = 0;
-                if (base + lane < cnt) pid = __ldg(bt + (jj >> p.page_tile_shift));
-                float ks = 0.f, vs = 0.f;  // FP8: the page's scales for this kv head, one tile per lane
+            // The per-tile metadata (block-table entry, then -- FP8 -- the page's two scales, which depend on it)
+            // is fetched 32 tiles at a time, one tile per lane, and kept TWO batches ahead of the tiles being
+            // issued: a batch's loads are in flight while the previous batches' TMAs are issued, so the dependent
+            // round trips to L2 / DRAM never stop the issue loop (they did: half of the producers' samples).
+            auto load_pid = [&](int base) -> int {
+                if (base + lane >= cnt) return 0;
+                return __ldg(bt + (win_logical_tile(wt, sp.j + base + lane) >> p.page_tile_shift));
+            };
+            auto load_scales = [&](int base, int pid, float &ks, float &vs) {
+                ks = vs = 0.f;
                 if constexpr (kFp8) {
                     if (base + lane < cnt) {
                         ks = __ldg(p.k_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
                         vs = __ldg(p.v_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
                     }
                 }
+            };
+            // (bf16: one L2-latency load per 32 tiles of 8 KiB is covered by the ring, and a short CTA -- config 2
+            // has ~110 tiles -- is better off with the shortest path to its first TMA: measured, so not pipelined.)
+            constexpr bool kMetaAhead = kFp8;
+            int pid = kMetaAhead ? load_pid(0) : 0, pid_next = kMetaAhead ? load_pid(32) : 0;
+            float ks = 0.f, vs = 0.f;  // FP8: the page's scales for this kv head
+            if constexpr (kMetaAhead) load_scales(0, pid, ks, vs);
+            for (int base = 0; base < cnt; base += 32) {
+                float ks_next = 0.f, vs_next = 0.f;
+                int pid_next2 = 0;
+                if constexpr (kMetaAhead) {
+                    load_scales(base + 32, pid_next, ks_next, vs_next);
+                    pid_next2 = load_pid(base + 64);
+                } else {
+                    pid = load_pid(base);
+                }
+                const int jj = win_logical_tile(wt, sp.j + base + lane);
                 const int m = cnt - base < 32 ? cnt - base : 32;
                 for (int i = (pw - (tl0 + base)) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
                     const int tl = tl0 + base + i;
@@ -372,16 +402,22 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                         vs_i = __shfl_sync(kFull, vs, i);
                     }
                     if (lane == 0) {
-                        const int row = pid_i * p.page_size + ((jj_i & tiles_per_page_mask) << kTileShift);
+                        const int slot0 = (jj_i & tiles_per_page_mask) << kTileShift;
+                        const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid_i * p.page_size + slot0;
+                        const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid_i : sp.kvh;
                         const uint32_t dst = ring + stage * C::kStageBytes;
                         const uint32_t bar = full0 + 8 * stage;
                         if constexpr (kFp8)  // ordered before the consumers' wait by the arrive below (release) and their wait (acquire)
                             asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(scales0 + 8 * stage), "f"(ks_i), "f"(vs_i) : "memory");
                         mbar_arrive_expect_tx(bar, C::kStageBytes);
-                        tma_load_4d_hint(dst, &tm_k, bar, 0, row, 0, sp.kvh, stream_policy);
-                        tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, row, 0, sp.kvh, stream_policy);
+                        tma_load_4d_hint(dst, &tm_k, bar, 0, c1, c2, c3, stream_policy);
+                        tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, c1, c2, c3, stream_policy);
                     }
                 }
+                pid = pid_next;
+                pid_next = pid_next2;
+                ks = ks_next;
+                vs = vs_next;
             }
             x += cnt;
             tl0 += cnt;
@@ -502,91 +538,146 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 #pragma unroll
         for (int mt = 0; mt < C::kKSteps; ++mt) acc[mt][0] = acc[mt][1] = acc[mt][2] = acc[mt][3] = 0.f;
 
-        for (; t < n + cnt; t += kConsumerWarps) {
-            mbar_wait(full0 + 8 * stage, phase);
+        // One pass of S3..S5 over NT of this warp's tiles (t, t + 8, ...) with ONE online-softmax update for all of
+        // them.  NT = 2 (FP8 cache) gives the warp two independent load -> convert -> MMA chains to interleave:
+        // with half the bytes per tile, a single chain per warp is latency-bound below the HBM rate.
+        auto tiles_pass = [&](auto nt_tag) {
+            constexpr int NT = decltype(nt_tag)::value;
+            uint32_t k_base[NT], v_base[NT];
+            unsigned alive[NT];
+            int stg[NT];
+            {
+                int sg = stage;
+                uint32_t ph = phase;
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    mbar_wait(full0 + 8 * sg, ph);
+                    stg[k] = sg;
+                    k_base[k] = ring + sg * C::kStageBytes;
+                    v_base[k] = k_base[k] + C::kTileBytes;
+                    // which of the tile's 16 tokens count: all but the ones past seq_len (last tile) and, under a
+                    // sliding window, the ones in the gap between the sinks and the window
+                    alive[k] = win_alive_mask(wt, seq_len, win_logical_tile(wt, sp.j + (t + k * kConsumerWarps - n)));
+                    sg += kConsumerWarps;
+                    if (sg >= C::kStages) {
+                        sg -= C::kStages;
+                        ph ^= 1u;
+                    }
+                }
+            }
 #ifdef COMEM_TRACE
             if (t == 0) COMEM_STAMP(3);
 #endif
-            const uint32_t k_base = ring + stage * C::kStageBytes;
-            const uint32_t v_base = k_base + C::kTileBytes;
-            // which of the tile's 16 tokens count: all but the ones past seq_len (last tile) and, under a
-            // sliding window, the ones in the gap between the sinks and the window
-            const unsigned alive = win_alive_mask(wt, seq_len, win_logical_tile(wt, sp.j + (t - n)));
 
-            // S3: scores for 2 n-tiles of 8 tokens
-            float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-            float sl2 = p.scale_log2, v_scale = 1.f;
+            // S3: scores for 2 n-tiles of 8 tokens per tile
+            float s[NT][2][4];
+            float sl2[NT], v_scale[NT];
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) s[k][0][j] = s[k][1][j] = 0.f;
+                sl2[k] = p.scale_log2;
+                v_scale[k] = 1.f;
+            }
             if constexpr (kFp8) {
                 // The tile is [16 tokens][128 B], 128-byte swizzled.  Lane (quad, qlane) reads, of token rows
                 // quad and quad + 8, the 16-byte chunks 2 qlane and 2 qlane + 1: a quarter-warp (two rows that
                 // differ in bit 0, even chunks ^ row) touches every bank once.  Each 32-bit word is one k-step's
                 // B fragment: bytes 0,1 -> b0, bytes 2,3 -> b1 (the permutation q was loaded with).
-                float2 sc;
-                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(sc.x), "=f"(sc.y) : "r"(scales0 + 8 * stage));
-                sl2 *= sc.x;
-                v_scale = sc.y;
-                const uint32_t row_lo = k_base + quad * 128, row_hi = row_lo + 8 * 128;  // (quad + 8) & 7 == quad
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    float2 sc;
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(sc.x), "=f"(sc.y) : "r"(scales0 + 8 * stg[k]));
+                    sl2[k] *= sc.x;
+                    v_scale[k] = sc.y;
+                }
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     const uint32_t off = ((uint32_t)(2 * qlane + c) ^ (uint32_t)quad) << 4;
-                    const uint4 ka = lds128(row_lo + off), kb = lds128(row_hi + off);
-                    const uint32_t wa[4] = {ka.x, ka.y, ka.z, ka.w}, wb[4] = {kb.x, kb.y, kb.z, kb.w};
 #pragma unroll
-                    for (int w = 0; w < 4; ++w) {
-                        const int kk = 4 * c + w;
-                        mma_f16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wa[w]), e4m3x2_hi_to_f16x2(wa[w]));
-                        mma_f16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wb[w]), e4m3x2_hi_to_f16x2(wb[w]));
+                    for (int k = 0; k < NT; ++k) {
+                        const uint32_t row_lo = k_base[k] + quad * 128 + off;  // (quad + 8) & 7 == quad: same swizzle
+                        const uint4 ka = lds128(row_lo), kb = lds128(row_lo + 8 * 128);
+                        const uint32_t wa[4] = {ka.x, ka.y, ka.z, ka.w}, wb[4] = {kb.x, kb.y, kb.z, kb.w};
+#pragma unroll
+                        for (int w = 0; w < 4; ++w) {
+                            const int kk = 4 * c + w;
+                            mma_f16_16816(s[k][0], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wa[w]), e4m3x2_hi_to_f16x2(wa[w]));
+                            mma_f16_16816(s[k][1], qf[kk][0], 0u, qf[kk][1], 0u, e4m3x2_lo_to_f16x2(wb[w]), e4m3x2_hi_to_f16x2(wb[w]));
+                        }
                     }
                 }
             } else {
 #pragma unroll
                 for (int kk = 0; kk < C::kKSteps; ++kk) {
-                    uint32_t kf[4];
-                    const uint32_t chunk = ((2 * kk) & 7) | ld_half;
-                    ldmatrix_x4(kf, k_base + (kk >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
-                    mma_bf16_16816(s[0], qf[kk][0], 0u, qf[kk][1], 0u, kf[0], kf[1]);
-                    mma_bf16_16816(s[1], qf[kk][0], 0u, qf[kk][1], 0u, kf[2], kf[3]);
+#pragma unroll
+                    for (int k = 0; k < NT; ++k) {
+                        uint32_t kf[4];
+                        const uint32_t chunk = ((2 * kk) & 7) | ld_half;
+                        ldmatrix_x4(kf, k_base[k] + (kk >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                        mma_bf16_16816(s[k][0], qf[kk][0], 0u, qf[kk][1], 0u, kf[0], kf[1]);
+                        mma_bf16_16816(s[k][1], qf[kk][0], 0u, qf[kk][1], 0u, kf[2], kf[3]);
+                    }
                 }
             }
-            float s0 = s[0][0] * sl2, s1 = s[0][1] * sl2;
-            float s2 = s[1][0] * sl2, s3 = s[1][1] * sl2;
-            if (alive != 0xffffu) {
-                // edge tile: mask by index (never by arithmetic) and zero the dead V rows so that
-                // NaN/Inf garbage in tokens that do not count cannot reach the accumulators (0 * NaN).
-                const int tok = 2 * qlane;
-                if (!((alive >> tok) & 1u)) s0 = -INFINITY;
-                if (!((alive >> (tok + 1)) & 1u)) s1 = -INFINITY;
-                if (!((alive >> (tok + 8)) & 1u)) s2 = -INFINITY;
-                if (!((alive >> (tok + 9)) & 1u)) s3 = -INFINITY;
-                constexpr int kChunksPerRow = D * C::kElemBytes / 16;  // 16-byte chunks per V row
-                for (int idx = lane; idx < kTileTokens * kChunksPerRow; idx += 32) {
-                    const int row = idx / kChunksPerRow;
-                    if ((alive >> row) & 1u) continue;
-                    const int ch = idx % kChunksPerRow;
-                    const uint32_t a = v_base + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+            float sv[NT][4];  // tokens 2q, 2q+1, 2q+8, 2q+9 of head `quad`
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+                sv[k][0] = s[k][0][0] * sl2[k];
+                sv[k][1] = s[k][0][1] * sl2[k];
+                sv[k][2] = s[k][1][0] * sl2[k];
+                sv[k][3] = s[k][1][1] * sl2[k];
+                if (alive[k] != 0xffffu) {
+                    // edge tile: mask by index (never by arithmetic) and zero the dead V rows so that
+                    // NaN/Inf garbage in tokens that do not count cannot reach the accumulators (0 * NaN).
+                    const int tok = 2 * qlane;
+                    if (!((alive[k] >> tok) & 1u)) sv[k][0] = -INFINITY;
+                    if (!((alive[k] >> (tok + 1)) & 1u)) sv[k][1] = -INFINITY;
+                    if (!((alive[k] >> (tok + 8)) & 1u)) sv[k][2] = -INFINITY;
+                    if (!((alive[k] >> (tok + 9)) & 1u)) sv[k][3] = -INFINITY;
+                    constexpr int kChunksPerRow = D * C::kElemBytes / 16;  // 16-byte chunks per V row
+                    for (int idx = lane; idx < kTileTokens * kChunksPerRow; idx += 32) {
+                        const int row = idx / kChunksPerRow;
+                        if ((alive[k] >> row) & 1u) continue;
+                        const int ch = idx % kChunksPerRow;
+                        const uint32_t a = v_base[k] + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
                 }
-                fence_proxy_async_smem();
-                __syncwarp();
             }
 
-            // S4: online softmax for head `quad` over this tile's 16 tokens
-            float tmax = fmaxf(fmaxf(s0, s1), fmaxf(s2, s3));
+            // S4: online softmax for head `quad` over these tiles' tokens
+            float tmax = fmaxf(fmaxf(sv[0][0], sv[0][1]), fmaxf(sv[0][2], sv[0][3]));
+#pragma unroll
+            for (int k = 1; k < NT; ++k) tmax = fmaxf(tmax, fmaxf(fmaxf(sv[k][0], sv[k][1]), fmaxf(sv[k][2], sv[k][3])));
             tmax = fmaxf(tmax, __shfl_xor_sync(kFull, tmax, 1));
             tmax = fmaxf(tmax, __shfl_xor_sync(kFull, tmax, 2));
             const float m_new = fmaxf(m_run, tmax);
             const float alpha = ex2(m_run - m_new);
             m_run = m_new;
-            const float e0 = ex2(s0 - m_new), e1 = ex2(s1 - m_new), e2 = ex2(s2 - m_new), e3 = ex2(s3 - m_new);
-            // FP8: the page's v_scale rides on p (fp16, 11 significant bits); the normaliser is the unrounded sum
-            const uint32_t p01 = kFp8 ? pack_f16x2(e0 * v_scale, e1 * v_scale) : pack_bf16x2(e0, e1);  // tokens 2q, 2q+1
-            const uint32_t p23 = kFp8 ? pack_f16x2(e2 * v_scale, e3 * v_scale) : pack_bf16x2(e2, e3);  // tokens 2q+8, 2q+9
-            lx_run = lx_run * alpha + ((e0 + e1) + (e2 + e3));
-            if constexpr (kFp8)
-                l_run = lx_run;
-            else
-                l_run = l_run * alpha + ((bf16lo_to_f32(p01) + bf16hi_to_f32(p01)) +
-                                         (bf16lo_to_f32(p23) + bf16hi_to_f32(p23)));
+            uint32_t p01[NT], p23[NT];
+            float esum = 0.f;
+            [[maybe_unused]] float rsum = 0.f;
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+                const float e0 = ex2(sv[k][0] - m_new), e1 = ex2(sv[k][1] - m_new);
+                const float e2 = ex2(sv[k][2] - m_new), e3 = ex2(sv[k][3] - m_new);
+                esum += (e0 + e1) + (e2 + e3);
+                if constexpr (kFp8) {
+                    // the page's v_scale rides on p (fp16, 11 significant bits); the normaliser is the unrounded sum
+                    p01[k] = pack_f16x2(e0 * v_scale[k], e1 * v_scale[k]);  // tokens 2q, 2q+1
+                    p23[k] = pack_f16x2(e2 * v_scale[k], e3 * v_scale[k]);  // tokens 2q+8, 2q+9
+                } else {
+                    p01[k] = pack_bf16x2(e0, e1);
+                    p23[k] = pack_bf16x2(e2, e3);
+                    rsum += (bf16lo_to_f32(p01[k]) + bf16hi_to_f32(p01[k])) + (bf16lo_to_f32(p23[k]) + bf16hi_to_f32(p23[k]));
+                }
+            }
+            lx_run = lx_run * alpha + esum;
+            if constexpr (kFp8) l_run = lx_run;
+            else l_run = l_run * alpha + rsum;
             if (__any_sync(kFull, alpha != 1.f)) {
                 // acc columns are heads 2*qlane, 2*qlane+1: fetch their alphas from those quads
                 const float a_lo = __shfl_sync(kFull, alpha, (2 * qlane) << 2);
@@ -609,39 +700,53 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 // {row quad: d = 16 quad + 2u, row quad + 8: d = 16 quad + 2u + 1}; S6 scatters accordingly.
                 const int t0 = 2 * qlane;
                 const uint32_t ch = (uint32_t)quad;
-                const uint4 r0 = lds128(v_base + t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4));
-                const uint4 r1 = lds128(v_base + (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4));
-                const uint4 r2 = lds128(v_base + (t0 + 8) * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4));
-                const uint4 r3 = lds128(v_base + (t0 + 9) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4));
-                const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
-                const uint32_t w2[4] = {r2.x, r2.y, r2.z, r2.w}, w3[4] = {r3.x, r3.y, r3.z, r3.w};
+                const uint32_t o_even = t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4);
+                const uint32_t o_odd = (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4);
 #pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    const uint32_t x01e = prmt(w0[w], w1[w], 0x5140u), x23e = prmt(w2[w], w3[w], 0x5140u);
-                    const uint32_t x01o = prmt(w0[w], w1[w], 0x7362u), x23o = prmt(w2[w], w3[w], 0x7362u);
-                    mma_f16_16816(acc[2 * w], e4m3x2_lo_to_f16x2(x01e), e4m3x2_hi_to_f16x2(x01e),
-                                  e4m3x2_lo_to_f16x2(x23e), e4m3x2_hi_to_f16x2(x23e), p01, p23);
-                    mma_f16_16816(acc[2 * w + 1], e4m3x2_lo_to_f16x2(x01o), e4m3x2_hi_to_f16x2(x01o),
-                                  e4m3x2_lo_to_f16x2(x23o), e4m3x2_hi_to_f16x2(x23o), p01, p23);
+                for (int k = 0; k < NT; ++k) {
+                    const uint4 r0 = lds128(v_base[k] + o_even), r1 = lds128(v_base[k] + o_odd);
+                    const uint4 r2 = lds128(v_base[k] + o_even + 8 * 128), r3 = lds128(v_base[k] + o_odd + 8 * 128);
+                    const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
+                    const uint32_t w2[4] = {r2.x, r2.y, r2.z, r2.w}, w3[4] = {r3.x, r3.y, r3.z, r3.w};
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) {
+                        const uint32_t x01e = prmt(w0[w], w1[w], 0x5140u), x23e = prmt(w2[w], w3[w], 0x5140u);
+                        const uint32_t x01o = prmt(w0[w], w1[w], 0x7362u), x23o = prmt(w2[w], w3[w], 0x7362u);
+                        mma_f16_16816(acc[2 * w], e4m3x2_lo_to_f16x2(x01e), e4m3x2_hi_to_f16x2(x01e),
+                                      e4m3x2_lo_to_f16x2(x23e), e4m3x2_hi_to_f16x2(x23e), p01[k], p23[k]);
+                        mma_f16_16816(acc[2 * w + 1], e4m3x2_lo_to_f16x2(x01o), e4m3x2_hi_to_f16x2(x01o),
+                                      e4m3x2_lo_to_f16x2(x23o), e4m3x2_hi_to_f16x2(x23o), p01[k], p23[k]);
+                    }
                 }
             } else {
 #pragma unroll
-                for (int mt = 0; mt < C::kKSteps; ++mt) {
-                    uint32_t vf[4];
-                    const uint32_t chunk = ((2 * mt) & 7) | ld_half;
-                    ldmatrix_x4_trans(vf, v_base + (mt >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
-                    mma_bf16_16816(acc[mt], vf[0], vf[1], vf[2], vf[3], p01, p23);
+                for (int k = 0; k < NT; ++k) {
+#pragma unroll
+                    for (int mt = 0; mt < C::kKSteps; ++mt) {
+                        uint32_t vf[4];
+                        const uint32_t chunk = ((2 * mt) & 7) | ld_half;
+                        ldmatrix_x4_trans(vf, v_base[k] + (mt >> 2) * 2048 + ld_row_off + ((chunk ^ ld_xor) << 4));
+                        mma_bf16_16816(acc[mt], vf[0], vf[1], vf[2], vf[3], p01[k], p23[k]);
+                    }
                 }
             }
 
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-            stage += kConsumerWarps;
-            if (stage >= C::kStages) {
-                stage -= C::kStages;
-                phase ^= 1u;
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+                if (lane == 0) mbar_arrive(empty0 + 8 * stg[k]);
+                stage += kConsumerWarps;
+                if (stage >= C::kStages) {
+                    stage -= C::kStages;
+                    phase ^= 1u;
+                }
             }
+            t += NT * kConsumerWarps;
+        };
+        if constexpr (C::kTilesPerPass == 2) {
+            while (t + kConsumerWarps < n + cnt) tiles_pass(std::integral_constant<int, 2>{});
         }
+        while (t < n + cnt) tiles_pass(std::integral_constant<int, 1>{});
 
         // S6: merge the consumer warps' states (warp-index order) and write the row or a partial.
         // Scratch layout per warp: acc as [head][D + 4] (the +4 pad makes both the fragment

@@ -106,12 +106,13 @@ class Fp8DecodeBatch:
     softmax_scale: float
     name: str = ""
     seed: int = 0
+    kv_layout: str = "NHD"     # "HND": k_pages / v_pages are [P, Hkv, page_size, D]
 
     batch = property(lambda self: self.q.shape[0])
     num_q_heads = property(lambda self: self.q.shape[1])
-    num_kv_heads = property(lambda self: self.k_pages.shape[2])
+    num_kv_heads = property(lambda self: self.k_pages.shape[1 if self.kv_layout == "HND" else 2])
     head_dim = property(lambda self: self.q.shape[2])
-    page_size = property(lambda self: self.k_pages.shape[1])
+    page_size = property(lambda self: self.k_pages.shape[2 if self.kv_layout == "HND" else 1])
     num_pages = property(lambda self: self.k_pages.shape[0])
     max_pages_per_seq = property(lambda self: self.block_table.shape[1])
 
@@ -163,6 +164,13 @@ def quantize_batch_fp8(batch: "DecodeBatch") -> Fp8DecodeBatch:
                           block_table=batch.block_table, seq_lens=batch.seq_lens,
                           softmax_scale=batch.softmax_scale, name=(batch.name + "+fp8kv") if batch.name else "fp8kv",
                           seed=batch.seed)
+
+
+def to_hnd(batch: Fp8DecodeBatch) -> Fp8DecodeBatch:
+    """Same cache, pools re-laid out [P, Hkv, page_size, D] (pure data movement)."""
+    assert batch.kv_layout == "NHD"
+    return dataclasses.replace(batch, k_pages=batch.k_pages.permute(0, 2, 1, 3).contiguous(),
+                               v_pages=batch.v_pages.permute(0, 2, 1, 3).contiguous(), kv_layout="HND")
 
 
 def permute_pages_fp8(batch: Fp8DecodeBatch, seed: int) -> Fp8DecodeBatch:

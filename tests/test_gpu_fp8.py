@@ -22,9 +22,9 @@ def bits(t):
 def run8(f, window=0, sinks=0, ws=None):
     out = torch.full_like(f.q, float("nan"))
     lse = torch.full((f.batch, f.num_q_heads), float("nan"), dtype=torch.float32, device=DEV)
-    ws = ws if ws is not None else comem.alloc_workspace(f.q, f.k_pages, f.block_table)
+    ws = ws if ws is not None else comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
     comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
-                                      f.softmax_scale, out, ws, window, sinks, lse_out=lse)
+                                      f.softmax_scale, out, ws, window, sinks, lse_out=lse, kv_layout=f.kv_layout)
     torch.cuda.synchronize()
     return out, lse
 
@@ -47,7 +47,7 @@ def check(oracle, f, what, window=0, sinks=0):
     out, lse = run8(f, window, sinks)
     c = f.to("cpu")
     ref, ref_lse = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table,
-                                          c.seq_lens, c.softmax_scale, window, sinks)
+                                          c.seq_lens, c.softmax_scale, window, sinks, kv_layout=c.kv_layout)
     gate(out.double().cpu().numpy(), ref, lse.double().cpu().numpy(), ref_lse, what)
     return out, lse
 
@@ -131,6 +131,22 @@ def test_fp8_scale_moves_between_page_and_bytes(oracle):
     f2 = dataclasses.replace(f, v_scale=torch.nan_to_num(f.v_scale, nan=1.0) * torch.exp2(e),
                              k_scale=torch.nan_to_num(f.k_scale, nan=1.0) * torch.exp2(-e.abs() / 2))
     check(oracle, f2, "wild page scales")
+
+
+@pytest.mark.parametrize("G,ps", [(4, 32), (8, 16), (3, 16)])
+def test_fp8_hnd_layout(oracle, G, ps):
+    """[P, Hkv, page_size, D] pools: parity vs the oracle's HND reading, and bit-identical to the NHD call (the
+    arithmetic and its order do not depend on where a tile sits in DRAM)."""
+    lens = [1, 17, 33, 128, 1000, 0, 2049, 20000]
+    f = fp8_batch(lens, 2 * G, 2, ps, seed=540 + G + ps)
+    h = W.to_hnd(f)
+    a, la = run8(f)
+    b, lb = check(oracle, h, f"hnd G{G} ps{ps}")
+    assert torch.equal(bits(a), bits(b)) and torch.equal(la, lb)
+    for window, sinks in ((100, 4), (4096, 0)):
+        a, la = run8(f, window, sinks)
+        b, lb = check(oracle, h, f"hnd G{G} ps{ps} w{window}", window, sinks)
+        assert torch.equal(bits(a), bits(b)) and torch.equal(la, lb)
 
 
 def test_fp8_rejects_head_dim_64_and_null_scales():

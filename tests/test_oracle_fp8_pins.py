@@ -14,6 +14,8 @@ What fixes it other than itself:
   F5  tail slots, unowned pages and their scales are irrelevant (NaN poison) -> bit-identical
   F6  brute-force dense softmax in numpy fp64 on the dequantised arrays (dequantised with torch's
       cast, not the oracle's table), per-page scales that differ page to page
+  F7  kv_layout "HND" ([P, Hkv, page_size, D]) on the transposed pools is bit-identical to "NHD" on the
+      original ones (only the row address differs)
 """
 import numpy as np
 import pytest
@@ -166,3 +168,18 @@ def test_f6_brute_force_dense(oracle, ps, window, sinks):
             want = (w[:, None] * v[:, h // g, :]).sum(0) / w.sum()
             assert np.max(np.abs(out[b, h] - want)) <= 1e-13
             assert abs(lse[b, h] - (s.max() + np.log(w.sum()))) <= 1e-12
+
+
+def test_f7_hnd_layout_is_a_relayout(oracle):
+    f = W.quantize_batch_fp8(W.make_batch([130, 47, 0, 16], 8, 2, 64, 32, seed=417))
+    h = W.to_hnd(f)
+    assert h.k_pages.shape == (f.num_pages, 2, 32, 64) and h.num_kv_heads == 2 and h.page_size == 32
+    for window, sinks in ((0, 0), (40, 3)):
+        a, la = _run8(oracle, f, window, sinks)
+        b, lb = oracle.decode_attn_fp8(h.q, h.k_pages, h.v_pages, h.k_scale, h.v_scale, h.block_table, h.seq_lens,
+                                       h.softmax_scale, window, sinks, kv_layout="HND")
+        assert np.array_equal(a, b) and np.array_equal(la, lb)
+    # and it is not a no-op: reading the transposed pools as NHD gives something else
+    c, _ = oracle.decode_attn_fp8(h.q, h.k_pages.view(f.k_pages.shape), h.v_pages.view(f.v_pages.shape), h.k_scale,
+                                  h.v_scale, h.block_table, h.seq_lens, h.softmax_scale)
+    assert not np.array_equal(a, c)
