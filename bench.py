@@ -65,6 +65,9 @@ def parse_args():
                     help="extra: time comem_decode_attn_fp8_async (E4M3 cache + page scales) on --workload c2|c3|c4")
     ap.add_argument("--kv-layout", default="nhd", choices=["nhd", "hnd"],
                     help="for --kv-fp8: pools [P, page, Hkv, D] (nhd) or [P, Hkv, page, D] (hnd)")
+    ap.add_argument("--pipeline", type=int, default=0, metavar="K",
+                    help="extra: drive 64 agent steps of the k-step-off pipeline (Algorithm 1) from comem_kstep_plan "
+                         "and check eq. 5 against the measured decode-attention times")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
@@ -663,6 +666,144 @@ def run_fp8(args) -> int:
     return 0
 
 
+def run_pipeline(args) -> int:
+    """Extra: the k-step-off pipeline (Algorithm 1) over 64 agent steps
+    (L261), shaped like the paper's crossover benchmark (section 4.5: fixed-length turns, concurrency 32,
+    k = 3; CoMem prompt bounded at a few K tokens, full-context prompt growing to ~40K).  The library's
+    comem_kstep_plan says, per step, which summary is in use; the agent batch's decode attention (one layer,
+    64q/8kv, D 128, page 16) is timed at the CoMem context and at the full context, L2 flushed before every
+    launch; eq. 5's predicted saving (L_full - L_sum) * S / W, with S = the batch's KV bytes per token position
+    and W = the slope of the measured times themselves, is compared with the measured saving.  Where a memory
+    job is launched, the memory model's decode attention (32q/8kv over the full history, same concurrency) runs
+    on a second stream under the agent's next steps and the agent's slowdown is reported."""
+    import statistics
+
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    K, T, TURN, SUMM, CONC = args.pipeline, 64, 640, 3072, 32
+    arr, events = comem.comem_kstep_plan(T, K, 0)
+    ctx_comem, ctx_full, mem_in = comem.comem_kstep_context_lengths(arr, T, TURN, SUMM)
+    agent = W.make_batch([T * TURN] * CONC, 64, 8, 128, 16, 1201, device, name="pipeline-agent")
+    memory = W.make_batch([T * TURN] * CONC, 32, 8, 128, 16, 1202, device, name="pipeline-memory")
+    sa, sb = torch.cuda.Stream(device), torch.cuda.Stream(device)
+    out_a, out_m = torch.empty_like(agent.q), torch.empty_like(memory.q)
+    ws_a = comem.alloc_workspace(agent.q, agent.k_pages, agent.block_table, stream=sa)
+    ws_m = comem.alloc_workspace(memory.q, memory.k_pages, memory.block_table, stream=sb)
+    lens_a = torch.empty(CONC, dtype=torch.int32, device=device)
+    lens_m = torch.empty(CONC, dtype=torch.int32, device=device)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+    torch.cuda.synchronize()
+
+    def launch(b, lens, out, ws, stream):
+        comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, lens, b.softmax_scale, out, ws,
+                                      stream=stream)
+
+    def time_agent(ctx, reps=5):
+        ts = []
+        with torch.cuda.stream(sa):
+            lens_a.fill_(ctx)
+            for i in range(reps + 1):
+                flush.fill_(i)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(sa)
+                launch(agent, lens_a, out_a, ws_a, sa)
+                e1.record(sa)
+                sa.synchronize()
+                if i:
+                    ts.append(e0.elapsed_time(e1) * 1e3)
+        return statistics.median(ts)
+
+    t_comem = [time_agent(c) for c in ctx_comem]
+    t_full = [time_agent(c) for c in ctx_full]
+    # W from the measured times themselves: least-squares slope of t over context (both series), eq. 5's premise
+    xs, ys = ctx_comem + ctx_full, t_comem + t_full
+    n = len(xs)
+    mx, my = sum(xs) / n, sum(ys) / n
+    slope = sum((x - mx) * (y - my) for x, y in zip(xs, ys)) / sum((x - mx) ** 2 for x in xs)   # us per token
+    fixed = my - slope * mx
+    s_bytes = CONC * agent.num_kv_heads * agent.head_dim * 2 * 2                                  # per token position
+    w_gbs = s_bytes / slope / 1e3
+    rel = []
+    for t in range(T):
+        if ctx_full[t] - ctx_comem[t] >= 4 * TURN:
+            pred = comem.comem_decode_saving_seconds(ctx_full[t], ctx_comem[t], s_bytes / 1e9, w_gbs) * 1e6
+            rel.append(abs((t_full[t] - t_comem[t]) - pred) / pred)
+    # overlap: memory-model decode attention on stream B under the agent's next steps on stream A
+    overlap = []
+    for t in range(T - 1):
+        if not mem_in[t] or len(overlap) >= 4 and t < T - K - 1:
+            continue
+        reps = 6
+        with torch.cuda.stream(sb):
+            lens_m.fill_(mem_in[t])
+        with torch.cuda.stream(sa):
+            lens_a.fill_(ctx_comem[t + 1])
+        torch.cuda.synchronize()
+        for _ in range(4 * reps):
+            launch(memory, lens_m, out_m, ws_m, sb)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(sa)
+        for _ in range(reps):
+            launch(agent, lens_a, out_a, ws_a, sa)
+        e1.record(sa)
+        torch.cuda.synchronize()
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e2.record(sa)
+        for _ in range(reps):
+            launch(agent, lens_a, out_a, ws_a, sa)
+        e3.record(sa)
+        torch.cuda.synchronize()
+        rec = {"after_step": t + 1, "memory_ctx": mem_in[t], "agent_ctx": ctx_comem[t + 1],
+               "agent_us_overlapped": e0.elapsed_time(e1) * 1e3 / reps,
+               "agent_us_alone": e2.elapsed_time(e3) * 1e3 / reps, "sm_partition": []}
+        # SM partitioning: both kernels are persistent one-CTA-per-SM grids, so two full grids time-share the GPU
+        # and a short agent step queues behind a long memory step.  Giving each stream a share of the SMs
+        # (comem_set_grid_ctas is read at enqueue time) lets both grids be resident at once.
+        sms = comem.comem_grid_ctas(128)
+        try:
+            comem.comem_set_programmatic_launch(False)   # else stream B's next kernel parks on the SMs left free
+            for agent_sms in (sms // 4, sms // 2):
+                comem.comem_set_grid_ctas(sms - agent_sms)
+                for _ in range(4 * reps):
+                    launch(memory, lens_m, out_m, ws_m, sb)
+                comem.comem_set_grid_ctas(agent_sms)
+                p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                p0.record(sa)
+                for _ in range(reps):
+                    launch(agent, lens_a, out_a, ws_a, sa)
+                p1.record(sa)
+                m0 = torch.cuda.Event(enable_timing=True)
+                m0.record(sb)
+                torch.cuda.synchronize()
+                rec["sm_partition"].append({"agent_sms": agent_sms, "memory_sms": sms - agent_sms,
+                                            "agent_us": p0.elapsed_time(p1) * 1e3 / reps})
+        finally:
+            comem.comem_set_grid_ctas(0)
+            comem.comem_set_programmatic_launch(True)
+        overlap.append(rec)
+    print(json.dumps({
+        "extra": "k-step-off pipeline (Algorithm 1) driven from comem_kstep_plan; eq. 5 vs measured",
+        "k": K, "steps": T, "turn_tokens": TURN, "summary_tokens": SUMM, "concurrency": CONC,
+        "uncached_prefills": sum(int(e.prefill_uncached) for e in events),
+        "memory_launches": sum(int(e.launch_memory) for e in events),
+        "ctx_comem_min_max": [min(ctx_comem), max(ctx_comem)], "ctx_full_final": ctx_full[-1],
+        "decode_attn_us_comem_sum": sum(t_comem), "decode_attn_us_full_sum": sum(t_full),
+        "trajectory_speedup": sum(t_full) / sum(t_comem),
+        "peak_step_speedup": max(f / c for f, c in zip(t_full, t_comem)),
+        "fit": {"us_per_token": slope, "fixed_us": fixed, "W_gbs": w_gbs, "S_bytes_per_token": s_bytes},
+        "eq5_rel_err": {"mean": sum(rel) / max(len(rel), 1), "max": max(rel) if rel else None, "steps": len(rel)},
+        "per_step_us": {"comem": [round(x, 2) for x in t_comem], "full": [round(x, 2) for x in t_full]},
+        "overlap": overlap, "l2": "flushed (512 MiB written) before every timed launch"}), flush=True)
+    return 0
+
+
 def main() -> int:
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -670,6 +811,8 @@ def main() -> int:
         return run_reference(args, rank)
     if args.window > 0:
         return run_window(args) if rank == 0 else 0
+    if args.pipeline > 0:
+        return run_pipeline(args) if rank == 0 else 0
     if args.kv_fp8:
         return run_fp8(args) if rank == 0 else 0
     if args.affine:

@@ -169,6 +169,44 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 size_t workspace_bytes, void *cuda_stream, int window, int sink_tokens,
                                 int kv_layout);
 
+/*
+ * k-step-off pipeline schedule and latency model — HOST functions, no device work.
+ *
+ * comem_kstep_plan — Algorithm 1 for agent steps t = 1 .. num_steps with retain-turns k:
+ * events[t-1] says whether a finished memory job is adopted at the start of step t (lines 4-7: s <- result,
+ * KV cache invalidated), which summary is then in use (summary_upto = u: s = f(tau_{<= u}), 0 = none yet;
+ * the raw buffer is tau_{u+1 : t}, eq. 4), whether the prefill is full-context (lines 9-13; also true
+ * at step 1, when nothing is cached) and whether a memory job is launched after the step (lines 19-21,
+ * t mod k = 0, input tau_{<= t}).  mem_delay = agent steps until a launched job counts as complete; <= 0
+ * means k ("available at the start of the next cycle"); > k is COMEM_ERR_INVALID_ARG (line 20 would
+ * overwrite a job in flight, which the paper leaves undefined; reading R19).
+ * `events` is caller-owned, num_steps entries.
+ *
+ * comem_kstep_context_lengths — token counts per step for turns of turn_tokens tokens and summaries of
+ * summary_tokens tokens: the agent's context under CoMem (summary + raw buffer), under the full-context
+ * baseline (tau_{<= t}) and the memory model's input where a job is launched (else 0).
+ *
+ * comem_decode_saving_seconds (eq. 5), comem_net_speedup (eq. 6, returns 0 / 1),
+ * comem_max_compression_ratio (eq. 7): S in GB per token, W in GB/s, P in tokens/s, Y in tokens.
+ */
+typedef struct {
+    int32_t step;              /* t, 1-based */
+    int32_t summary_upto;      /* u */
+    uint8_t adopt_summary;
+    uint8_t prefill_uncached;
+    uint8_t launch_memory;
+    uint8_t reserved;
+} comem_kstep_event;
+int comem_kstep_plan(int num_steps, int k, int mem_delay, comem_kstep_event *events);
+int comem_kstep_context_lengths(const comem_kstep_event *events, int num_steps, int turn_tokens,
+                                int summary_tokens, int32_t *comem_ctx, int32_t *full_ctx,
+                                int32_t *memory_input);
+double comem_decode_saving_seconds(double l_full, double l_sum, double s_gb_per_token, double w_gb_per_s);
+int comem_net_speedup(double y_tokens, double l_full, double l_sum, double s_gb_per_token,
+                      double w_gb_per_s, double p_tokens_per_s);
+double comem_max_compression_ratio(double w_gb_per_s, double y_tokens, double s_gb_per_token,
+                                   double p_tokens_per_s);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,
@@ -253,6 +291,16 @@ int comem_validate_inputs(const int32_t *block_table, const int32_t *seq_lens, i
  * concurrently running batches a share of the SMs. */
 int comem_grid_ctas(int head_dim);
 int comem_set_grid_ctas(int n);
+
+/*
+ * comem_set_programmatic_launch — process-wide launch policy, read at enqueue time (default 1).  With 1 the
+ * attention kernel is launched with programmatic stream serialization: the next launch on the same stream
+ * starts its prologue on SMs the previous one has released, which shortens back-to-back steps (config 2) but
+ * also means a stream's NEXT kernel occupies every free SM while it waits.  Set 0 while two streams share the
+ * GPU by SM partition (comem_set_grid_ctas per enqueue: agent and memory-model grids that sum to the SM
+ * count), so that the other stream's kernel can be resident at the same time.
+ */
+int comem_set_programmatic_launch(int enabled);
 
 const char *comem_status_string(int status);
 int comem_version(void);

@@ -21,11 +21,17 @@ from .binding import (  # noqa: F401
     COMEM_PHASE_COMBINE,
     comem_decode_attn_fp8_async,
     comem_decode_attn_workspace_bytes,
+    comem_decode_saving_seconds,
+    comem_kstep_context_lengths,
+    comem_kstep_plan,
+    comem_max_compression_ratio,
+    comem_net_speedup,
     comem_decode_step_host,
     comem_grid_ctas,
     comem_kv_append_async,
     comem_schedule_host,
     comem_set_grid_ctas,
+    comem_set_programmatic_launch,
     comem_validate_inputs,
     comem_status_string,
     comem_version,

@@ -72,12 +72,25 @@ def load_library():
     lib.comem_decode_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                            i32, i64, vp, vp, sz, vp]
     lib.comem_decode_step_host.restype = i32
+    f64 = c.c_double
+    lib.comem_kstep_plan.argtypes = [i32, i32, i32, vp]
+    lib.comem_kstep_plan.restype = i32
+    lib.comem_kstep_context_lengths.argtypes = [vp, i32, i32, i32, vp, vp, vp]
+    lib.comem_kstep_context_lengths.restype = i32
+    lib.comem_decode_saving_seconds.argtypes = [f64] * 4
+    lib.comem_decode_saving_seconds.restype = f64
+    lib.comem_net_speedup.argtypes = [f64] * 6
+    lib.comem_net_speedup.restype = i32
+    lib.comem_max_compression_ratio.argtypes = [f64] * 4
+    lib.comem_max_compression_ratio.restype = f64
     lib.comem_schedule_host.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.comem_schedule_host.restype = i32
     lib.comem_grid_ctas.argtypes = [i32]
     lib.comem_grid_ctas.restype = i32
     lib.comem_set_grid_ctas.argtypes = [i32]
     lib.comem_set_grid_ctas.restype = i32
+    lib.comem_set_programmatic_launch.argtypes = [i32]
+    lib.comem_set_programmatic_launch.restype = i32
     lib.comem_status_string.argtypes = [i32]
     lib.comem_status_string.restype = c.c_char_p
     lib.comem_version.restype = i32
@@ -104,6 +117,10 @@ def comem_set_grid_ctas(n: int) -> None:
     load_library().comem_set_grid_ctas(int(n))
 
 
+def comem_set_programmatic_launch(enabled: bool) -> None:
+    load_library().comem_set_programmatic_launch(1 if enabled else 0)
+
+
 def comem_schedule_host(seq_lens, num_kv_heads: int, grid_ctas: int):
     """Host mirror of the device split-KV schedule: list of CTA tile-range boundaries."""
     import numpy as np
@@ -116,6 +133,44 @@ def comem_schedule_host(seq_lens, num_kv_heads: int, grid_ctas: int):
     if st != COMEM_OK:
         raise ComemError(st, "comem_schedule_host")
     return begins[:nc.value + 1].tolist()
+
+
+class KstepEvent(ctypes.Structure):
+    _fields_ = [("step", ctypes.c_int32), ("summary_upto", ctypes.c_int32), ("adopt_summary", ctypes.c_uint8),
+                ("prefill_uncached", ctypes.c_uint8), ("launch_memory", ctypes.c_uint8), ("reserved", ctypes.c_uint8)]
+
+
+def comem_kstep_plan(num_steps: int, k: int, mem_delay: int = 0):
+    """Algorithm 1 as a list of KstepEvent (host function of the library)."""
+    ev = (KstepEvent * max(num_steps, 1))()
+    st = load_library().comem_kstep_plan(int(num_steps), int(k), int(mem_delay), ctypes.cast(ev, ctypes.c_void_p))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_kstep_plan")
+    return ev, [ev[i] for i in range(num_steps)]
+
+
+def comem_kstep_context_lengths(events_array, num_steps: int, turn_tokens: int, summary_tokens: int):
+    """(comem_ctx, full_ctx, memory_input) token counts per step, as python lists."""
+    a, b, c_ = ((ctypes.c_int32 * max(num_steps, 1))() for _ in range(3))
+    st = load_library().comem_kstep_context_lengths(ctypes.cast(events_array, ctypes.c_void_p), int(num_steps),
+                                                    int(turn_tokens), int(summary_tokens),
+                                                    ctypes.cast(a, ctypes.c_void_p), ctypes.cast(b, ctypes.c_void_p),
+                                                    ctypes.cast(c_, ctypes.c_void_p))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_kstep_context_lengths")
+    return list(a)[:num_steps], list(b)[:num_steps], list(c_)[:num_steps]
+
+
+def comem_decode_saving_seconds(l_full, l_sum, s_gb_per_token, w_gb_per_s) -> float:
+    return float(load_library().comem_decode_saving_seconds(l_full, l_sum, s_gb_per_token, w_gb_per_s))
+
+
+def comem_net_speedup(y_tokens, l_full, l_sum, s_gb_per_token, w_gb_per_s, p_tokens_per_s) -> bool:
+    return bool(load_library().comem_net_speedup(y_tokens, l_full, l_sum, s_gb_per_token, w_gb_per_s, p_tokens_per_s))
+
+
+def comem_max_compression_ratio(w_gb_per_s, y_tokens, s_gb_per_token, p_tokens_per_s) -> float:
+    return float(load_library().comem_max_compression_ratio(w_gb_per_s, y_tokens, s_gb_per_token, p_tokens_per_s))
 
 
 def comem_decode_attn_workspace_bytes(batch: int, num_q_heads: int, num_kv_heads: int, head_dim: int,

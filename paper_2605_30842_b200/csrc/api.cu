@@ -23,6 +23,7 @@ constexpr float kLog2e = 1.4426950408889634f;
 static_assert(kMaxBatch == COMEM_MAX_BATCH, "header and scheduler disagree on the batch limit");
 
 std::atomic<int> g_grid_override{0};
+std::atomic<int> g_pdl{1};
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -306,6 +307,12 @@ int comem_set_grid_ctas(int n)
     return COMEM_OK;
 }
 
+int comem_set_programmatic_launch(int enabled)
+{
+    g_pdl.store(enabled ? 1 : 0);
+    return COMEM_OK;
+}
+
 int comem_grid_ctas(int head_dim)
 {
     if (head_dim != 64 && head_dim != 128) return -COMEM_ERR_UNSUPPORTED;
@@ -378,6 +385,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.k_scale = kv_fp8 ? k_scale : nullptr;
     p.v_scale = kv_fp8 ? v_scale : nullptr;
     p.kv_hnd = hnd;
+    p.no_pdl = g_pdl.load() ? 0 : 1;
     p.q = static_cast<const __nv_bfloat16 *>(q);
     p.block_table = block_table;
     p.seq_lens = seq_lens;

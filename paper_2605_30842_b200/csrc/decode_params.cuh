@@ -34,6 +34,7 @@ struct DecodeParams {
     int sinks;                   // attention-sink tokens kept at the start of every sequence
     const float *k_scale;        // FP8 cache only (reading R18): fp32 [P][Hkv] page scales, else nullptr
     const float *v_scale;
+    int no_pdl;                  // host-side only: launch without programmatic stream serialization (comem_set_programmatic_launch)
     int kv_hnd;                  // FP8 cache only: pools laid out [P][Hkv][ps][D] (a tile is 2 KiB contiguous) instead of [P][ps][Hkv][D]
 };
 

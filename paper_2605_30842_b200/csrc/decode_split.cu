@@ -905,7 +905,7 @@ cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = p.no_pdl ? 0 : 1;
     if (kv_fp8) return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, p, cfg) : cudaErrorInvalidValue;
     if (head_dim == 128) return launch_variant<128, false>(tm_k, tm_v, p, cfg);
     return launch_variant<64, false>(tm_k, tm_v, p, cfg);
