@@ -646,12 +646,50 @@ def run_fp8(args) -> int:
         replays = max(4, min(int(2e6 / (est_us * per_graph)), max(1, args.steps // per_graph)))
         for _ in range(3):
             g.replay()
+        # burst: a short run from an idle, cool GPU (SM clock at its maximum) ...
+        stream.synchronize()
+        time.sleep(1.0)
+        bs = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), 0)
+        bs.start()
+        burst_replays = max(1, min(replays, int(40e3 / (est_us * per_graph))))   # ~40 ms
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g.replay()
+        stream.synchronize()
+        bs.active = True
+        b0.record(stream)
+        for _ in range(burst_replays):
+            g.replay()
+        b1.record(stream)
+        stream.synchronize()
+        bs.active = False
+        bs.stop()
+        burst_us = b0.elapsed_time(b1) * 1e3 / (burst_replays * per_graph)
+        # ... then the sustained run (seconds): this kernel plus HBM at full rate reaches the board's power cap
+        sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), 0)
+        sampler.start()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        sampler.active = True
         e0.record(stream)
         for _ in range(replays):
             g.replay()
         e1.record(stream)
         stream.synchronize()
+        sampler.active = False
+        sampler.stop()
+        # the same step launched on its own after an L2 flush (no back-to-back overlap, idle-stream launch latency inside)
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+        iso = []
+        for i in range(12):
+            flush.fill_(i)
+            i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            i0.record(stream)
+            step(i)
+            i1.record(stream)
+            stream.synchronize()
+            if i >= 2:
+                iso.append(i0.elapsed_time(i1) * 1e3)
+        iso.sort()
     us = e0.elapsed_time(e1) * 1e3 / (replays * per_graph)
     gbs = nbytes / us / 1e3
     print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload),
@@ -660,7 +698,10 @@ def run_fp8(args) -> int:
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
                       "frac_of_measured_peak": gbs / peaks["hbm_gbs"], "peak": peaks["hbm_gbs"],
                       "bf16_cache_bytes_same_tokens": bf16_bytes,
-                      "equivalent_bf16_gbs": bf16_bytes / us / 1e3,
+                      "equivalent_bf16_gbs": bf16_bytes / us / 1e3, "clocks": sampler.summary(),
+                      "burst": {"steps": burst_replays * per_graph, "us_per_step": burst_us, "value": nbytes / burst_us / 1e3,
+                                "equivalent_bf16_gbs": bf16_bytes / burst_us / 1e3, "clocks": bs.summary()},
+                      "isolated_step_us": {"n": len(iso), "min": iso[0], "median": iso[len(iso) // 2]},
                       "l2": "cold: steps rotate over %d pools (%.2f GiB)" % (len(pools), len(pools) * nbytes / 2 ** 30)}),
           flush=True)
     return 0
