@@ -128,3 +128,22 @@ def test_schedule_segment_aligned_variant(lib):
     begins = comem.comem_schedule_host([20000] * 32, 8, 148)
     sizes = np.diff(begins)
     assert sizes.max() - sizes.min() <= 1
+
+
+def test_fp8_entry_point_validates_before_any_launch(lib):
+    """comem_decode_attn_fp8_async: null scales, head_dim 64 and an unknown layout are rejected on the host."""
+    import ctypes
+    vp = ctypes.c_void_p
+    d = vp(0x1000)
+
+    def call(ks=d, vs=d, head_dim=128, layout=0, sinks=0):
+        return lib.comem_decode_attn_fp8_async(d, d, d, ks, vs, d, d, 64, 8, head_dim, 16, ctypes.c_float(0.088), d, 1,
+                                               2048, 4096, None, d, 1 << 30, None, 0, sinks, layout)
+
+    assert call(ks=None) == comem.COMEM_ERR_INVALID_ARG
+    assert call(vs=None) == comem.COMEM_ERR_INVALID_ARG
+    assert call(head_dim=64) == comem.COMEM_ERR_UNSUPPORTED
+    assert call(layout=7) == comem.COMEM_ERR_INVALID_ARG
+    assert call(sinks=-1) == comem.COMEM_ERR_INVALID_ARG
+    # valid arguments get as far as the device check (no GPU here) or the launch (never reached with these pointers)
+    assert call() in (comem.COMEM_ERR_CUDA, comem.COMEM_ERR_UNSUPPORTED, comem.COMEM_ERR_WORKSPACE)
