@@ -183,3 +183,35 @@ def test_fp8_config4_full_size_sampled(oracle):
     g = W.permute_pages_fp8(f, seed=77)
     po, pl = run8(g)
     assert torch.equal(bits(out), bits(po)) and torch.equal(lse, pl)
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_fp8_randomised_shapes(oracle, case):
+    """Seeded random draws over what the FP8 entry point accepts: batch, kv heads, group 1..8, page size, pool
+    layout, ragged lengths with zeros and tile / page-boundary values, window + sinks, and the persistent grid
+    size (linear and segment-aligned schedules, whole and cut segments, one- and multi-round merges); each case
+    also under a page permutation (bit-identical)."""
+    rng = np.random.default_rng(9500 + case)
+    G = int(rng.integers(1, 9))
+    hkv = int(rng.integers(1, 9))
+    ps = int(rng.choice([16, 32]))
+    batch = int(rng.integers(1, 11))
+    special = [0, 1, 15, 16, 17, ps - 1, ps, ps + 1, 255, 256, 257]
+    lens = [int(rng.choice(special)) if rng.random() < 0.3 else int(rng.integers(1, 6000)) for _ in range(batch)]
+    if case % 5 == 0:
+        lens[0] = int(rng.integers(20000, 60000))
+    grid = int(rng.choice([0, 0, 3, 17, 61, 148, 211, 600]))
+    window, sinks = (0, 0) if rng.random() < 0.6 else (int(rng.integers(1, 3000)), int(rng.integers(0, 70)))
+    pool = max(1, sum(W.pages_needed(l, ps) for l in lens)) + int(rng.integers(0, 9))
+    f = fp8_batch(lens, G * hkv, hkv, ps, seed=9600 + case, num_pages=pool)
+    if rng.random() < 0.5:
+        f = W.to_hnd(f)
+    what = f"case {case}: G{G} hkv{hkv} ps{ps} {f.kv_layout} lens{lens} grid{grid} w{window} s{sinks}"
+    try:
+        comem.comem_set_grid_ctas(grid)
+        out, lse = check(oracle, f, what, window, sinks)
+        out2, lse2 = run8(W.permute_pages_fp8(f, seed=case), window, sinks)
+        assert torch.equal(bits(out), bits(out2)), what
+        assert torch.equal(lse.nan_to_num(neginf=-1e30), lse2.nan_to_num(neginf=-1e30)), what
+    finally:
+        comem.comem_set_grid_ctas(0)
