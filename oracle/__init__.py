@@ -57,6 +57,10 @@ def _load():
         lib.oracle_lse_merge.restype = i32
         lib.oracle_kv_append.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32]
         lib.oracle_kv_append.restype = i32
+        lib.oracle_e4m3_encode.argtypes = [f32]
+        lib.oracle_e4m3_encode.restype = i32
+        lib.oracle_kv_append_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]
+        lib.oracle_kv_append_fp8.restype = i32
         lib.oracle_max_threads.restype = i32
         _lib = lib
     return _lib
@@ -232,3 +236,28 @@ def kv_append(k_bits, v_bits, block_table, seq_lens, new_k, new_v):
                               d, ps, bt.shape[0], bt.shape[1])
     if rc != 0:
         raise ValueError("oracle_kv_append: sequence would outgrow its block-table row")
+
+
+def e4m3_encode(x: float) -> int:
+    """fp32 -> E4M3 byte, round-to-nearest-even, saturating at +-448 (NaN -> 0x7f)."""
+    return int(_load().oracle_e4m3_encode(ctypes.c_float(x)))
+
+
+def kv_append_fp8(k_bytes, v_bytes, k_scale, v_scale, block_table, seq_lens, new_k, new_v, kv_layout: str = "NHD"):
+    """In place: quantise one new bf16 (k, v) row per sequence with its page's scales into the E4M3 pools
+    (numpy uint8, writable, C-contiguous), seq_lens (numpy int32) += 1."""
+    lib = _load()
+    assert k_bytes.dtype == np.uint8 and k_bytes.flags.c_contiguous and k_bytes.flags.writeable
+    assert v_bytes.dtype == np.uint8 and v_bytes.flags.c_contiguous and v_bytes.flags.writeable
+    assert seq_lens.dtype == np.int32 and seq_lens.flags.c_contiguous
+    ks = np.ascontiguousarray(np.asarray(k_scale, np.float32))
+    vs = np.ascontiguousarray(np.asarray(v_scale, np.float32))
+    bt = _as_i32(block_table)
+    nk, nv = as_bits(new_k), as_bits(new_v)
+    hnd = kv_layout == "HND"
+    _, a, b_, d = k_bytes.shape
+    hkv, ps = (a, b_) if hnd else (b_, a)
+    rc = lib.oracle_kv_append_fp8(_p(k_bytes), _p(v_bytes), _p(ks), _p(vs), _p(bt), _p(seq_lens), _p(nk), _p(nv),
+                                  hkv, d, ps, bt.shape[0], bt.shape[1], 1 if hnd else 0)
+    if rc != 0:
+        raise ValueError("oracle_kv_append_fp8: sequence would outgrow its block-table row")

@@ -420,3 +420,62 @@ int oracle_kv_append(uint16_t *k_pages, uint16_t *v_pages, const int32_t *block_
     }
     return 0;
 }
+
+/*
+ * E4M3 encoder (round-to-nearest-even, saturating to +-448, "satfinite"): the grid is the decode table above.
+ * NaN -> 0x7f.  Written from the format's definition (bias 7, 3 mantissa bits, subnormal step 2^-9).
+ */
+static uint8_t e4m3_from_float(float xf)
+{
+    if (xf != xf) return 0x7f;
+    const uint8_t sign = signbit(xf) ? 0x80 : 0x00;
+    const double a = fabs((double)xf);
+    if (a > 448.0) return sign | 0x7e;          /* includes +-inf; (448, 464) would round to 448 anyway */
+    if (a < ldexp(1.0, -6)) {                   /* subnormal range: multiples of 2^-9; 8 steps = 2^-6 = code 0x08 */
+        const double q = nearbyint(a * 512.0);  /* default rounding mode: to nearest, ties to even */
+        return sign | (uint8_t)q;
+    }
+    int e;
+    const double f = frexp(a, &e);              /* a = f * 2^e, f in [0.5, 1) */
+    e -= 1;                                     /* a = m * 2^e, m = 2f in [1, 2) */
+    int q = (int)nearbyint((2.0 * f - 1.0) * 8.0);
+    if (q == 8) { q = 0; e += 1; }
+    if (e > 8 || (e == 8 && q == 7)) return sign | 0x7e;
+    return sign | (uint8_t)(((e + 7) << 3) | q);
+}
+
+int oracle_e4m3_encode(float x) { return (int)e4m3_from_float(x); }
+
+/*
+ * KV append into the FP8 cache (the step right before the path, for reading R18's cache): the new
+ * token's bf16 K row of kv head h is stored as   byte = e4m3_rne_sat( (float)k[h][d] / k_scale[pid][h] )
+ * -- the IEEE fp32 quotient, then the encoder above -- with pid the page that holds position seq_lens[b]; the
+ * page's scale is whatever the caller has put there (how it was chosen is the serving engine's policy);
+ * V likewise; then seq_lens[b] += 1.  kv_hnd as in oracle_decode_attn_fp8.
+ */
+int oracle_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
+                         const int32_t *block_table, int32_t *seq_lens, const uint16_t *new_k,
+                         const uint16_t *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
+                         int max_pages_per_seq, int kv_hnd)
+{
+    for (int b = 0; b < batch; ++b) {
+        const int64_t t = seq_lens[b];
+        if (t / page_size >= max_pages_per_seq) return 1;
+        const int64_t pid = block_table[(int64_t)b * max_pages_per_seq + t / page_size];
+        const int64_t slot = t % page_size;
+        for (int h = 0; h < num_kv_heads; ++h) {
+            const int64_t dst = (kv_hnd ? (pid * num_kv_heads + h) * page_size + slot
+                                        : (pid * page_size + slot) * num_kv_heads + h) * (int64_t)head_dim;
+            const float ks = k_scale[pid * num_kv_heads + h], vs = v_scale[pid * num_kv_heads + h];
+            for (int d = 0; d < head_dim; ++d) {
+                const int64_t src = ((int64_t)b * num_kv_heads + h) * head_dim + d;
+                const float kq = (float)bf16_to_double(new_k[src]) / ks;
+                const float vq = (float)bf16_to_double(new_v[src]) / vs;
+                k_pages[dst + d] = e4m3_from_float(kq);
+                v_pages[dst + d] = e4m3_from_float(vq);
+            }
+        }
+        seq_lens[b] = (int32_t)(t + 1);
+    }
+    return 0;
+}

@@ -183,3 +183,78 @@ def test_f7_hnd_layout_is_a_relayout(oracle):
     c, _ = oracle.decode_attn_fp8(h.q, h.k_pages.view(f.k_pages.shape), h.v_pages.view(f.v_pages.shape), h.k_scale,
                                   h.v_scale, h.block_table, h.seq_lens, h.softmax_scale)
     assert not np.array_equal(a, c)
+
+
+# ---- the E4M3 encoder and the quantising append (oracle.e4m3_encode, oracle.kv_append_fp8) -------------------
+#   E1  decode(encode(v)) == v for every finite code, signs of zero kept
+#   E2  torch's float8_e4m3fn cast (round-to-nearest-even) on random floats, on every midpoint between adjacent
+#       codes (the ties) and on their fp32 neighbours
+#   E3  saturation: everything above 448 (and inf) -> 0x7e / 0xfe; NaN -> a NaN code
+#   E4  hand-computed ties: 1.0625 -> 1.0 (0x38), 1.1875 -> 1.25 (0x3a), 2^-10 -> 0, 3 * 2^-10 -> 2 * 2^-9 (0x02)
+#   A1  append: the row lands at (page of position L, slot L % ps), nothing else in the pools changes, L += 1;
+#       a full page moves on to the next table entry; HND == NHD transposed
+def test_e1_encode_inverts_decode(oracle):
+    for b in range(256):
+        if b & 0x7f == 0x7f:
+            continue
+        assert oracle.e4m3_encode(oracle.e4m3_decode(b)) == b, hex(b)
+
+
+def test_e2_encode_matches_torch_cast(oracle):
+    dec = np.array([oracle.e4m3_decode(b) for b in range(0x7f)])            # positive codes, ascending
+    mids = (dec[:-1] + dec[1:]) / 2                                         # exact in fp32: few significant bits
+    pts = np.concatenate([mids, np.nextafter(mids.astype(np.float32), np.float32(1e9)),
+                          np.nextafter(mids.astype(np.float32), np.float32(-1e9)), dec])
+    rng = np.random.default_rng(7)
+    pts = np.concatenate([pts, rng.uniform(0, 448, 20000), rng.uniform(0, 0.05, 20000), 2.0 ** rng.uniform(-12, 8.8, 20000)])
+    pts = np.concatenate([pts, -pts]).astype(np.float32)
+    pts = pts[np.abs(pts) <= 448]
+    want = torch.from_numpy(pts).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    got = np.array([oracle.e4m3_encode(float(x)) for x in pts], dtype=np.uint8)
+    assert np.array_equal(got, want)
+
+
+def test_e3_saturation_and_nan(oracle):
+    for x in (448.0001, 449.0, 464.0, 480.0, 1e9, float("inf")):
+        assert oracle.e4m3_encode(x) == 0x7e and oracle.e4m3_encode(-x) == 0xfe
+    assert oracle.e4m3_encode(float("nan")) & 0x7f == 0x7f
+
+
+def test_e4_ties_to_even_by_hand(oracle):
+    assert oracle.e4m3_encode(1.0625) == 0x38 and oracle.e4m3_encode(1.1875) == 0x3a
+    assert oracle.e4m3_encode(2.0 ** -10) == 0x00 and oracle.e4m3_encode(3 * 2.0 ** -10) == 0x02
+    assert oracle.e4m3_encode(-2.0 ** -10) == 0x80
+    assert oracle.e4m3_encode(15 * 2.0 ** -10) == 0x08                       # 7.5 steps -> 8 steps = min normal
+
+
+@pytest.mark.parametrize("layout", ["NHD", "HND"])
+def test_a1_append_fp8_places_and_quantises(oracle, layout):
+    ps, hkv, d = 16, 2, 64
+    b = W.make_batch([15, 16, 0, 40], 4, hkv, d, ps, seed=431, spare_tokens=3)
+    f = W.quantize_batch_fp8(b)
+    f.k_scale.nan_to_num_(nan=0.01)
+    f.v_scale.nan_to_num_(nan=0.02)
+    f = f if layout == "NHD" else W.to_hnd(f)
+    k8, v8 = f.k_pages.numpy().copy(), f.v_pages.numpy().copy()
+    lens = f.seq_lens.numpy().astype(np.int32).copy()
+    g = torch.Generator().manual_seed(3)
+    nk = (torch.randn((4, hkv, d), generator=g) * 2).to(torch.bfloat16)
+    nv = (torch.randn((4, hkv, d), generator=g) * 2).to(torch.bfloat16)
+    nk[0, 0, 0], nk[0, 0, 1], nv[1, 1, 5] = 1e6, -1e6, 0.0                    # saturation both ways, a zero
+    k0, v0, l0 = k8.copy(), v8.copy(), lens.copy()
+    oracle.kv_append_fp8(k8, v8, f.k_scale, f.v_scale, f.block_table, lens, nk, nv, kv_layout=layout)
+    assert np.array_equal(lens, l0 + 1)
+    touched = np.zeros(k8.shape, bool)
+    for s in range(4):
+        L = int(l0[s])
+        pid, slot = int(f.block_table[s, L // ps]), L % ps
+        for h in range(hkv):
+            idx = (pid, h, slot) if layout == "HND" else (pid, slot, h)
+            touched[idx] = True
+            for arr, new, sc in ((k8, nk, f.k_scale), (v8, nv, f.v_scale)):
+                q = (new[s, h].float() / sc[pid, h]).clamp(-448, 448)          # fp32 quotient, saturated
+                want = q.to(torch.float8_e4m3fn).view(torch.uint8).numpy()     # torch's RNE cast
+                assert np.array_equal(arr[idx], want), (s, h)
+    assert np.array_equal(k8[~touched], k0[~touched]) and np.array_equal(v8[~touched], v0[~touched])
+    assert k8[(int(f.block_table[0, 0]), 0, 15) if layout == "HND" else (int(f.block_table[0, 0]), 15, 0)][0] == 0x7e
+    assert int(f.block_table[1, 1]) != int(f.block_table[1, 0])               # sequence 1 (L = 16) opened its second page
