@@ -170,6 +170,20 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 int kv_layout);
 
 /*
+ * comem_kv_append_fp8_async — comem_kv_append_async for the FP8 cache of comem_decode_attn_fp8_async (P:L61 for
+ * reading R18's cache): the new token's bf16 K row of kv head h is stored as
+ *     byte = e4m3( (float)new_k[b][h][d] / k_scale[pid][h] )      pid = block_table[b][seq_lens[b] / page_size]
+ * — the IEEE fp32 quotient rounded to nearest even, saturating at +-448 — V likewise with v_scale, then
+ * seq_lens[b] += 1.  The page's scales are read, never written: choosing them (calibration, first-row amax, …)
+ * is the caller's policy, and a page must have its scales set before its first row is appended.
+ * new_k / new_v: bf16 [batch, num_kv_heads, head_dim], device.  kv_layout as above.  Enqueue-only.
+ */
+int comem_kv_append_fp8_async(void *k_pages, void *v_pages, const float *k_scale, const float *v_scale,
+                              const int32_t *block_table, int32_t *seq_lens, const void *new_k,
+                              const void *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
+                              int max_pages_per_seq, int kv_layout, void *cuda_stream);
+
+/*
  * k-step-off pipeline schedule and latency model — HOST functions, no device work.
  *
  * comem_kstep_plan — Algorithm 1 for agent steps t = 1 .. num_steps with retain-turns k:

@@ -29,6 +29,7 @@ from .binding import (  # noqa: F401
     comem_decode_step_host,
     comem_grid_ctas,
     comem_kv_append_async,
+    comem_kv_append_fp8_async,
     comem_schedule_host,
     comem_set_grid_ctas,
     comem_set_programmatic_launch,

@@ -69,6 +69,8 @@ def load_library():
     lib.comem_validate_inputs.restype = i32
     lib.comem_kv_append_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
     lib.comem_kv_append_async.restype = i32
+    lib.comem_kv_append_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
+    lib.comem_kv_append_fp8_async.restype = i32
     lib.comem_decode_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                            i32, i64, vp, vp, sz, vp]
     lib.comem_decode_step_host.restype = i32
@@ -295,6 +297,24 @@ def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_tab
         workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens), 1 if hnd else 0)
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_fp8_async")
+
+
+def comem_kv_append_fp8_async(k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, new_k, new_v,
+                              stream=None, kv_layout: str = "NHD") -> None:
+    """Quantise one new bf16 (k, v) row per sequence into the E4M3 pools with the page's scales; seq_lens += 1."""
+    assert kv_layout in ("NHD", "HND")
+    hnd = kv_layout == "HND"
+    assert k_pages.dtype == torch.uint8 and v_pages.dtype == torch.uint8 and k_pages.is_contiguous() and v_pages.is_contiguous()
+    assert new_k.dtype == torch.bfloat16 and new_v.dtype == torch.bfloat16 and new_k.is_contiguous() and new_v.is_contiguous()
+    page_size, hkv = (k_pages.shape[2], k_pages.shape[1]) if hnd else (k_pages.shape[1], k_pages.shape[2])
+    assert tuple(new_k.shape) == (block_table.shape[0], hkv, k_pages.shape[3]) and new_v.shape == new_k.shape
+    assert k_scale.dtype == torch.float32 and tuple(k_scale.shape) == (k_pages.shape[0], hkv) and v_scale.shape == k_scale.shape
+    st = load_library().comem_kv_append_fp8_async(
+        _ptr(k_pages), _ptr(v_pages), _ptr(k_scale), _ptr(v_scale), _ptr(block_table), _ptr(seq_lens), _ptr(new_k),
+        _ptr(new_v), hkv, k_pages.shape[3], page_size, block_table.shape[0], block_table.shape[1], 1 if hnd else 0,
+        _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_kv_append_fp8_async")
 
 
 def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out=None,

@@ -515,6 +515,33 @@ int comem_kv_append_async(void *k_pages, void *v_pages, const int32_t *block_tab
     return COMEM_OK;
 }
 
+int comem_kv_append_fp8_async(void *k_pages, void *v_pages, const float *k_scale, const float *v_scale,
+                              const int32_t *block_table, int32_t *seq_lens, const void *new_k, const void *new_v,
+                              int num_kv_heads, int head_dim, int page_size, int batch, int max_pages_per_seq,
+                              int kv_layout, void *cuda_stream)
+{
+    if (!k_pages || !v_pages || !k_scale || !v_scale || !block_table || !seq_lens || !new_k || !new_v)
+        return COMEM_ERR_INVALID_ARG;
+    if (batch <= 0 || num_kv_heads <= 0 || max_pages_per_seq <= 0) return COMEM_ERR_INVALID_ARG;
+    if (kv_layout != COMEM_KV_LAYOUT_NHD && kv_layout != COMEM_KV_LAYOUT_HND) return COMEM_ERR_INVALID_ARG;
+    if (head_dim != 64 && head_dim != 128) return COMEM_ERR_UNSUPPORTED;
+    if (page_size != 16 && page_size != 32) return COMEM_ERR_UNSUPPORTED;
+    if (!aligned(k_pages, 16) || !aligned(v_pages, 16) || !aligned(new_k, 4) || !aligned(new_v, 4) ||
+        !aligned(k_scale, 4) || !aligned(v_scale, 4))
+        return COMEM_ERR_INVALID_ARG;
+    const int st = check_device();
+    if (st != COMEM_OK) return st;
+    if (launch_kv_append_fp8(static_cast<uint8_t *>(k_pages), static_cast<uint8_t *>(v_pages), k_scale, v_scale,
+                             block_table, seq_lens, static_cast<const __nv_bfloat16 *>(new_k),
+                             static_cast<const __nv_bfloat16 *>(new_v), num_kv_heads, head_dim, page_size, batch,
+                             max_pages_per_seq, kv_layout == COMEM_KV_LAYOUT_HND ? 1 : 0,
+                             static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return COMEM_OK;
+}
+
 int comem_decode_step_host(const void *q_host, const void *new_k_host, const void *new_v_host, void *k_pages,
                            void *v_pages, const int32_t *block_table, int32_t *seq_lens, int num_q_heads,
                            int num_kv_heads, int head_dim, int page_size, float softmax_scale,

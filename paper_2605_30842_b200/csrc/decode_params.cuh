@@ -49,6 +49,10 @@ cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
                              int page_size, int batch, int max_pages, cudaStream_t stream,
                              const __nv_bfloat16 *q_src = nullptr, __nv_bfloat16 *q_dst = nullptr,
                              int q_row_elems = 0);
+cudaError_t launch_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
+                                 const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
+                                 const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
+                                 int max_pages, int hnd, cudaStream_t stream);
 cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,
                             int page_size, int64_t num_pages, int *flag, cudaStream_t stream, int extra_tokens = 0);
 // occupancy-derived persistent grid for the split kernel on the current device

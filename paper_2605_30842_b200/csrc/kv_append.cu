@@ -45,6 +45,41 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
     if (threadIdx.x == 0) seq_lens[b] = t + 1;
 }
 
+// FP8 cache (reading R18): the new token's bf16 rows are quantised with the scales of the page they land in,
+//   byte = e4m3_rne_satfinite((float)x / scale[pid][kv head])      (IEEE fp32 quotient, then cvt.rn.satfinite)
+// one CTA per sequence, one thread per pair of elements; then seq_lens[b] += 1.  hnd: pools [P][Hkv][ps][D].
+__global__ void __launch_bounds__(128)
+kv_append_fp8_kernel(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
+                     const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
+                     const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int max_pages, int hnd)
+{
+    pdl_wait_prior_grid();
+    const int b = blockIdx.x;
+    const int t = seq_lens[b];
+    const int page = t / page_size;
+    const int slot = t - page * page_size;
+    const int64_t pid = block_table[(int64_t)b * max_pages + page];
+    const int row_elems = num_kv_heads * head_dim;
+    const uint32_t *sk = reinterpret_cast<const uint32_t *>(new_k + (int64_t)b * row_elems);
+    const uint32_t *sv = reinterpret_cast<const uint32_t *>(new_v + (int64_t)b * row_elems);
+    for (int i = threadIdx.x; i < row_elems / 2; i += blockDim.x) {
+        const int h = (2 * i) / head_dim, d = 2 * i - h * head_dim;
+        const int64_t dst = (hnd ? (pid * num_kv_heads + h) * page_size + slot
+                                 : (pid * page_size + slot) * num_kv_heads + h) * (int64_t)head_dim + d;
+        const float ks = k_scale[pid * num_kv_heads + h], vs = v_scale[pid * num_kv_heads + h];
+        const uint32_t kw = sk[i], vw = sv[i];
+        uint16_t kq, vq;
+        asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(kq)
+            : "f"(__fdiv_rn(bf16hi_to_f32(kw), ks)), "f"(__fdiv_rn(bf16lo_to_f32(kw), ks)));
+        asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(vq)
+            : "f"(__fdiv_rn(bf16hi_to_f32(vw), vs)), "f"(__fdiv_rn(bf16lo_to_f32(vw), vs)));
+        *reinterpret_cast<uint16_t *>(k_pages + dst) = kq;
+        *reinterpret_cast<uint16_t *>(v_pages + dst) = vq;
+    }
+    __syncthreads();  // every thread has read seq_lens[b] before it changes
+    if (threadIdx.x == 0) seq_lens[b] = t + 1;
+}
+
 // Debug aid (comem_validate_inputs): one CTA per sequence checks what the hot path trusts --
 // seq_len within the table row's reach and every USED table entry a page id inside the pool.
 // flag: 0 = fine; otherwise 1 + index of the first offending sequence seen.
@@ -73,6 +108,16 @@ cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens,
     cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), stream);
     if (e != cudaSuccess) return e;
     validate_kernel<<<batch, 128, 0, stream>>>(block_table, seq_lens, max_pages, page_size, (long long)num_pages, flag, extra_tokens);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
+                                 const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
+                                 const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
+                                 int max_pages, int hnd, cudaStream_t stream)
+{
+    kv_append_fp8_kernel<<<batch, 128, 0, stream>>>(k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, new_k,
+                                                   new_v, num_kv_heads, head_dim, page_size, max_pages, hnd);
     return cudaGetLastError();
 }
 

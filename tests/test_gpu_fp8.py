@@ -215,3 +215,43 @@ def test_fp8_randomised_shapes(oracle, case):
         assert torch.equal(lse.nan_to_num(neginf=-1e30), lse2.nan_to_num(neginf=-1e30)), what
     finally:
         comem.comem_set_grid_ctas(0)
+
+
+@pytest.mark.parametrize("layout,ps", [("NHD", 16), ("HND", 32)])
+def test_fp8_append_then_attend_loop(oracle, layout, ps):
+    """40 decode steps on the FP8 cache: comem_kv_append_fp8_async then attention.  The appended BYTES and
+    seq_lens must equal the oracle's (byte work: bit-exact; both sides take the fp32 quotient and round it to
+    E4M3 nearest-even, saturating), including rows that saturate, tiny quotients (subnormal codes), zeros and
+    page crossings; the attention output after each of several steps matches the FP8 attention oracle on the
+    oracle-appended cache."""
+    hq, hkv = 16, 4
+    lens = [ps - 3, 5000, 0, 2 * ps - 1, 777]
+    b = W.make_batch(lens, hq, hkv, 128, ps, seed=561, device=DEV, spare_tokens=48)
+    f = W.quantize_batch_fp8(b)
+    # pages that will be opened by the appends hold nothing yet: give them the scales a serving engine would
+    f.k_scale.copy_(torch.where(torch.isnan(f.k_scale) | (f.k_scale == 1.0), torch.full_like(f.k_scale, 0.011), f.k_scale))
+    f.v_scale.copy_(torch.where(torch.isnan(f.v_scale) | (f.v_scale == 1.0), torch.full_like(f.v_scale, 0.009), f.v_scale))
+    if layout == "HND":
+        f = W.to_hnd(f)
+    f = dataclasses.replace(f, seq_lens=f.seq_lens.clone())
+    ok8, ov8 = f.k_pages.cpu().numpy().copy(), f.v_pages.cpu().numpy().copy()
+    olens = f.seq_lens.cpu().numpy().astype(np.int32).copy()
+    ks_c, vs_c, bt_c = f.k_scale.cpu(), f.v_scale.cpu(), f.block_table.cpu()
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=layout)
+    for step in range(40):
+        q, nk, nv = W.decode_step_rows(b, step, seed_base=7000)
+        if step % 7 == 0:
+            nk[0, 0, :4] = torch.tensor([1e4, -1e4, 0.0, 1e-5], dtype=torch.bfloat16, device=DEV)   # saturate, zero, subnormal code
+            nv[1, 1, :2] = torch.tensor([-0.0, 3e-6], dtype=torch.bfloat16, device=DEV)
+        comem.comem_kv_append_fp8_async(f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens, nk, nv,
+                                        kv_layout=layout)
+        oracle.kv_append_fp8(ok8, ov8, ks_c, vs_c, bt_c, olens, nk.cpu(), nv.cpu(), kv_layout=layout)
+        fq = dataclasses.replace(f, q=q)
+        if step in (0, 1, 2, 3, ps - 1, ps, 39):
+            torch.cuda.synchronize()
+            assert np.array_equal(f.seq_lens.cpu().numpy(), olens), step
+            assert np.array_equal(f.k_pages.cpu().numpy(), ok8) and np.array_equal(f.v_pages.cpu().numpy(), ov8), step
+            out, lse = run8(fq, ws=ws)
+            ref, ref_lse = oracle.decode_attn_fp8(q.cpu(), ok8, ov8, ks_c, vs_c, bt_c, olens, f.softmax_scale, kv_layout=layout)
+            gate(out.double().cpu().numpy(), ref, lse.double().cpu().numpy(), ref_lse, f"{layout} step {step}")
+    assert (ok8 == 0x7e).any() and (ok8 == 0xfe).any()          # the saturating rows did saturate
