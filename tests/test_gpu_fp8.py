@@ -255,3 +255,48 @@ def test_fp8_append_then_attend_loop(oracle, layout, ps):
             ref, ref_lse = oracle.decode_attn_fp8(q.cpu(), ok8, ov8, ks_c, vs_c, bt_c, olens, f.softmax_scale, kv_layout=layout)
             gate(out.double().cpu().numpy(), ref, lse.double().cpu().numpy(), ref_lse, f"{layout} step {step}")
     assert (ok8 == 0x7e).any() and (ok8 == 0xfe).any()          # the saturating rows did saturate
+
+
+def test_fp8_two_streams_overlap_equals_serial():
+    """Config-5 style on the FP8 cache: an agent batch (64q/8kv, NHD) and a memory-model batch (32q/8kv, HND) each
+    run 16 append + attend steps, once serially and once overlapped on two streams with their own workspaces:
+    every step's output is bit-identical (no CTA ever waits for another; nothing depends on arrival order)."""
+    def mk(hq, lens, seed, layout):
+        b = W.make_batch(lens, hq, 8, 128, 16, seed=seed, device=DEV, spare_tokens=16)
+        f = W.quantize_batch_fp8(b)
+        for sc in (f.k_scale, f.v_scale):
+            sc.copy_(torch.where(torch.isnan(sc) | (sc == 1.0), torch.full_like(sc, 0.01), sc))
+        f = W.to_hnd(f) if layout == "HND" else f
+        rows = [W.decode_step_rows(b, s, seed_base=seed * 10) for s in range(16)]
+        return f, rows
+
+    specs = [(64, [9000, 30000, 17, 12000, 4097, 20000], 571, "NHD"), (32, [40000, 65000, 33000], 572, "HND")]
+
+    def run(overlap):
+        outs = []
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        state = []
+        for (hq, lens, seed, layout), st in zip(specs, streams):
+            f, rows = mk(hq, lens, seed, layout)
+            f = dataclasses.replace(f, seq_lens=f.seq_lens.clone(), k_pages=f.k_pages.clone(), v_pages=f.v_pages.clone())
+            ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, stream=st, kv_layout=layout)
+            state.append((f, rows, ws, st, [torch.empty_like(f.q) for _ in range(16)]))
+        torch.cuda.synchronize()
+        for step in range(16):
+            for f, rows, ws, st, o in state:
+                q, nk, nv = rows[step]
+                comem.comem_kv_append_fp8_async(f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                                nk, nv, stream=st, kv_layout=f.kv_layout)
+                comem.comem_decode_attn_fp8_async(q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table,
+                                                  f.seq_lens, f.softmax_scale, o[step], ws, stream=st,
+                                                  kv_layout=f.kv_layout)
+                if not overlap:
+                    torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        return [[bits(x).clone() for x in s[4]] for s in state]
+
+    serial, both = run(False), run(True)
+    for a, b in zip(serial, both):
+        for step, (x, y) in enumerate(zip(a, b)):
+            assert torch.equal(x, y), step
+            assert torch.isfinite(x.view(torch.bfloat16).float()).all()
