@@ -56,12 +56,28 @@ def test_p3_shorter_memory_job_is_adopted_earlier():
         KP.kstep_plan(12, 3, mem_delay=4)
 
 
+def _golden_case_study():
+    """tests/golden/eq7_case_study.txt: the values the paper prints, key=value lines."""
+    import os
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "eq7_case_study.txt")) as fh:
+        for line in fh:
+            if "=" in line and not line.startswith("#"):
+                k, v = line.strip().split("=")
+                vals[k] = float(v)
+    return vals
+
+
 def test_p4_case_study_numbers():
-    r = KP.max_compression_ratio(w_gbs=2000.0, y=1000.0, s_gb=2e-4, p_tok_s=3000.0)
+    g = _golden_case_study()
+    r = KP.max_compression_ratio(w_gbs=g["W_GBps"], y=g["Y_tokens"], s_gb=g["S_GB_per_tok"], p_tok_s=g["P_tok_s"])
     assert abs(r - 1.0 / (1.0 + 2000.0 / 600.0)) < 1e-15
-    assert round(r, 2) == 0.23                                      # "L_sum / L_full < 0.23"
-    assert abs(0.23 * 32000 - 7360) < 1e-9                          # "within 7.36K tokens"
-    assert 7360 < r * 32768 < 7600
+    assert round(r, 2) == g["ratio_printed"]                        # "L_sum / L_full < 0.23"
+    assert abs(g["ratio_printed"] * 32000 - g["summary_tokens_printed"]) < 1e-9   # "within 7.36K tokens"
+    assert g["summary_tokens_printed"] < r * 32768 < 7600
+    # eq. 6 at the printed operating point: a 7.36K summary of a 32K prefix is just inside the bound
+    assert KP.net_speedup(g["Y_tokens"], 32000.0, g["summary_tokens_printed"], g["S_GB_per_tok"], g["W_GBps"], g["P_tok_s"])
+    assert not KP.net_speedup(g["Y_tokens"], 32000.0, 7500.0, g["S_GB_per_tok"], g["W_GBps"], g["P_tok_s"])
 
 
 def test_p5_eq6_iff_below_eq7_bound():
