@@ -47,6 +47,8 @@ L2_BYTES_NOMINAL = 126e6
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE split-KV launch from the committed
 # `ncu --set full` capture (profiles/r1_b_fused.md names the command).
 NCU_TRAFFIC_BYTES = {"c2": 137_632_512, "c3": 4_838_226_768, "c4": 8_595_141_560}  # profiles/r1_b_fused.md
+# same for the FP8 kernel (profiles/r1_c_fp8_pipeline.md section 3): (workload, layout) -> bytes
+NCU_TRAFFIC_BYTES_FP8 = {("c4", "NHD"): 4_324_995_000 + 3_796_224, ("c4", "HND"): 4_301_188_000 + 3_680_768}
 
 
 def parse_args():
@@ -697,6 +699,11 @@ def run_fp8(args) -> int:
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
                       "frac_of_measured_peak": gbs / peaks["hbm_gbs"], "peak": peaks["hbm_gbs"],
+                      "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128, 1>", "achieved": gbs,
+                                   "peak": peaks["hbm_gbs"], "unit": UNIT, "frac": gbs / peaks["hbm_gbs"],
+                                   "us_per_launch": us,
+                                   "traffic": NCU_TRAFFIC_BYTES_FP8.get((args.workload, pools[0].kv_layout))},
+                      "gpu_launches": replays * per_graph,
                       "bf16_cache_bytes_same_tokens": bf16_bytes,
                       "equivalent_bf16_gbs": bf16_bytes / us / 1e3, "clocks": sampler.summary(),
                       "burst": {"steps": burst_replays * per_graph, "us_per_step": burst_us, "value": nbytes / burst_us / 1e3,
@@ -937,7 +944,7 @@ def main() -> int:
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
                 "data": "synthetic", "config": cfg,
                 "frac_of_8TBps": value / world / 8000.0,
-                "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128>", "achieved": achieved,
+                "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128, 0>", "achieved": achieved,
                              "peak": peak, "peak_source": peak_src, "unit": UNIT, "frac": achieved / peak,
                              "us_per_launch": ms_max / args.steps * 1e3,
                              "split_only_us": ms_split_max / args.steps * 1e3,
