@@ -157,7 +157,7 @@ int comem_decode_attn_window_async(const void *q, const void *k_pages, const voi
  * q, out, lse_out, block_table, seq_lens, workspace, stream, determinism and the error contract are
  * those of comem_decode_attn_async.  Arithmetic: E4M3 widens exactly to fp16 and the tensor op runs in
  * fp16 with fp32 accumulation; q is converted bf16 -> fp16 (exact for 2^-14 <= |q| < 65504) and
- * p * v_scale is rounded to fp16.  COMEM_ERR_UNSUPPORTED unless head_dim == 128.
+ * p * v_scale is rounded to fp16.  head_dim 64 or 128.
  */
 enum { COMEM_KV_LAYOUT_NHD = 0, COMEM_KV_LAYOUT_HND = 1 };
 int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *v_pages,

@@ -199,6 +199,12 @@ def alloc_workspace(q: torch.Tensor, k_pages: torch.Tensor, block_table: torch.T
     n = comem_decode_attn_workspace_bytes(q.shape[0], q.shape[1], hkv, q.shape[2], ps, block_table.shape[1])
     ws = torch.empty(n, dtype=torch.uint8, device=q.device)
     with torch.cuda.device(q.device):
+        if isinstance(stream, torch.cuda.Stream):
+            # torch's caching allocator hands out blocks that are free in CURRENT-stream order: work queued there
+            # may still be writing this block's previous contents.  The init below runs on `stream`, so order it
+            # after the current stream and tell the allocator where the block is used.
+            stream.wait_stream(torch.cuda.current_stream())
+            ws.record_stream(stream)
         comem_workspace_init_async(ws, q.shape[0], q.shape[1], hkv, q.shape[2], stream)
     return ws
 

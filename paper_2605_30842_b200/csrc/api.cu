@@ -166,8 +166,10 @@ int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, 
             gstride8[0] = (cuuint64_t)d; gstride8[1] = (cuuint64_t)ps * d; gstride8[2] = (cuuint64_t)hkv * ps * d;
         }
         const cuuint32_t box8[4] = {(cuuint32_t)d, (cuuint32_t)kTileTokens, 1, 1};
+        // D = 128: 128-byte rows, 128-byte swizzle; D = 64: plain 64-byte rows (decode_split.cu, Cfg)
         r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void *>(pool), gdim8, gstride8, box8, estr,
-                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, d == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                d == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     } else {
         r = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(pool), gdim, gstride,
@@ -361,7 +363,6 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
     if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
-    if (kv_fp8 && head_dim == 64) return COMEM_ERR_UNSUPPORTED;
     if (kv_layout != COMEM_KV_LAYOUT_NHD && !(kv_fp8 && kv_layout == COMEM_KV_LAYOUT_HND)) return COMEM_ERR_INVALID_ARG;
     if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !out) return COMEM_ERR_INVALID_ARG;

@@ -58,7 +58,8 @@ constexpr unsigned kFull = 0xffffffffu;
 // must be issued every ~85 ns per SM to keep up with HBM).
 template <int D, bool kFp8>
 struct Cfg {
-    static_assert(!kFp8 || D == 128, "the FP8 fragment mapping is written for head_dim 128");
+    // FP8 tiles: [16 tokens][D bytes]; D = 128: 128-byte swizzled rows; D = 64: plain 64-byte rows (the tiny case:
+    // its shared-memory reads are not conflict-free and need not be)
     static constexpr int kElemBytes = kFp8 ? 1 : 2;
     // one elected lane per producer warp; tiles are dealt round-robin to them (one lane is issue-rate bound)
     static constexpr int kProducerWarps = kFp8 ? 4 : 2;
@@ -121,6 +122,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     using C = Cfg<D, kFp8>;
     constexpr int kThreads = C::kThreads;
     constexpr int kProducerWarps = C::kProducerWarps;
+    [[maybe_unused]] constexpr int kFp8Chunks = D / 64;  // FP8: 16-byte chunks of a K row each lane reads (S3)
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t ring = (raw + 1023u) & ~1023u;  // 1024-aligned: the 128B-swizzle atom
@@ -339,7 +341,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // tl always lands in ring stage tl % kStages, in the ring's pass number tl / kStages.
         static_assert((C::kStages & (C::kStages - 1)) == 0 && C::kStages % kProducerWarps == 0, "ring indexing");
         static_assert((kProducerWarps & (kProducerWarps - 1)) == 0, "round-robin by mask");
-        constexpr int kStageShift = (C::kStages == 16) ? 4 : 5;
+        constexpr int kStageShift = (C::kStages == 16) ? 4 : (C::kStages == 32 ? 5 : 6);
         static_assert((1 << kStageShift) == C::kStages, "kStageShift");
         const int pw = warp - kConsumerWarps;
         // K/V bytes are used once per step: evict-first keeps them from displacing the L2-resident
@@ -513,12 +515,13 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             if constexpr (kFp8) {
                 // E4M3 widens exactly to fp16, so the tensor op runs in fp16 and q is converted once per
                 // segment.  The contraction index is permuted to suit 16-byte shared-memory reads of K
-                // (see S3): k-step 4c + w of lane qlane covers d = 16 (2 qlane + c) + 4 w + {0,1 | 2,3}.
+                // (see S3): k-step 4c + w of lane qlane covers d = 16 (2 qlane + c) + 4 w + {0,1 | 2,3}
+                // (D = 64: one chunk per lane, d = 16 qlane + 4 w + ...).
 #pragma unroll
-                for (int c = 0; c < 2; ++c)
+                for (int c = 0; c < kFp8Chunks; ++c)
 #pragma unroll
                     for (int w = 0; w < 4; ++w) {
-                        const int i32 = 8 * (2 * qlane + c) + 2 * w;
+                        const int i32 = 8 * (kFp8Chunks * qlane + c) + 2 * w;
                         qf[4 * c + w][0] = live ? bf16x2_to_f16x2(__ldg(qrow + i32)) : 0u;
                         qf[4 * c + w][1] = live ? bf16x2_to_f16x2(__ldg(qrow + i32 + 1)) : 0u;
                     }
@@ -592,12 +595,13 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     v_scale[k] = sc.y;
                 }
 #pragma unroll
-                for (int c = 0; c < 2; ++c) {
-                    const uint32_t off = ((uint32_t)(2 * qlane + c) ^ (uint32_t)quad) << 4;
+                for (int c = 0; c < kFp8Chunks; ++c) {
+                    const uint32_t chunk = (uint32_t)(kFp8Chunks * qlane + c);
+                    const uint32_t off = (D == 128 ? (chunk ^ (uint32_t)quad) : chunk) << 4;
 #pragma unroll
                     for (int k = 0; k < NT; ++k) {
-                        const uint32_t row_lo = k_base[k] + quad * 128 + off;  // (quad + 8) & 7 == quad: same swizzle
-                        const uint4 ka = lds128(row_lo), kb = lds128(row_lo + 8 * 128);
+                        const uint32_t row_lo = k_base[k] + quad * D + off;  // (quad + 8) & 7 == quad: same swizzle
+                        const uint4 ka = lds128(row_lo), kb = lds128(row_lo + 8 * D);
                         const uint32_t wa[4] = {ka.x, ka.y, ka.z, ka.w}, wb[4] = {kb.x, kb.y, kb.z, kb.w};
 #pragma unroll
                         for (int w = 0; w < 4; ++w) {
@@ -640,7 +644,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                         const int row = idx / kChunksPerRow;
                         if ((alive[k] >> row) & 1u) continue;
                         const int ch = idx % kChunksPerRow;
-                        const uint32_t a = v_base[k] + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
+                        const uint32_t a = (kFp8 && D == 64) ? v_base[k] + row * 64 + (ch << 4)
+                                                             : v_base[k] + (ch >> 3) * 2048 + row * 128 + ((ch & 7) << 4);
                         asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(a), "r"(0u) : "memory");
                     }
                     fence_proxy_async_smem();
@@ -698,18 +703,36 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 // 2j+1 -> every bank once).  A-fragment registers pair two TOKENS of one d: PRMT interleaves the
                 // bytes of two rows, the conversion widens each byte pair.  m-tile u of this lane is
                 // {row quad: d = 16 quad + 2u, row quad + 8: d = 16 quad + 2u + 1}; S6 scatters accordingly.
+                // (D = 64: 8 bytes per row and lane, d = 8 quad .. 8 quad + 7, two words, four m-tiles.)
                 const int t0 = 2 * qlane;
-                const uint32_t ch = (uint32_t)quad;
-                const uint32_t o_even = t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4);
-                const uint32_t o_odd = (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4);
+                constexpr int kWords = D / 32;  // 32-bit words of a V row each lane reads
+                uint32_t o_even, o_odd;
+                if constexpr (D == 128) {
+                    const uint32_t ch = (uint32_t)quad;
+                    o_even = t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4);
+                    o_odd = (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4);
+                } else {
+                    o_even = t0 * 64 + 8 * quad;
+                    o_odd = (t0 + 1) * 64 + 8 * quad;
+                }
 #pragma unroll
                 for (int k = 0; k < NT; ++k) {
-                    const uint4 r0 = lds128(v_base[k] + o_even), r1 = lds128(v_base[k] + o_odd);
-                    const uint4 r2 = lds128(v_base[k] + o_even + 8 * 128), r3 = lds128(v_base[k] + o_odd + 8 * 128);
-                    const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
-                    const uint32_t w2[4] = {r2.x, r2.y, r2.z, r2.w}, w3[4] = {r3.x, r3.y, r3.z, r3.w};
+                    uint32_t w0[4], w1[4], w2[4], w3[4];
+                    if constexpr (D == 128) {
+                        const uint4 r0 = lds128(v_base[k] + o_even), r1 = lds128(v_base[k] + o_odd);
+                        const uint4 r2 = lds128(v_base[k] + o_even + 8 * 128), r3 = lds128(v_base[k] + o_odd + 8 * 128);
+                        w0[0] = r0.x; w0[1] = r0.y; w0[2] = r0.z; w0[3] = r0.w;
+                        w1[0] = r1.x; w1[1] = r1.y; w1[2] = r1.z; w1[3] = r1.w;
+                        w2[0] = r2.x; w2[1] = r2.y; w2[2] = r2.z; w2[3] = r2.w;
+                        w3[0] = r3.x; w3[1] = r3.y; w3[2] = r3.z; w3[3] = r3.w;
+                    } else {
+                        const uint2 r0 = lds64(v_base[k] + o_even), r1 = lds64(v_base[k] + o_odd);
+                        const uint2 r2 = lds64(v_base[k] + o_even + 8 * 64), r3 = lds64(v_base[k] + o_odd + 8 * 64);
+                        w0[0] = r0.x; w0[1] = r0.y; w1[0] = r1.x; w1[1] = r1.y;
+                        w2[0] = r2.x; w2[1] = r2.y; w3[0] = r3.x; w3[1] = r3.y;
+                    }
 #pragma unroll
-                    for (int w = 0; w < 4; ++w) {
+                    for (int w = 0; w < kWords; ++w) {
                         const uint32_t x01e = prmt(w0[w], w1[w], 0x5140u), x23e = prmt(w2[w], w3[w], 0x5140u);
                         const uint32_t x01o = prmt(w0[w], w1[w], 0x7362u), x23o = prmt(w2[w], w3[w], 0x7362u);
                         mma_f16_16816(acc[2 * w], e4m3x2_lo_to_f16x2(x01e), e4m3x2_hi_to_f16x2(x01e),
@@ -756,8 +779,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         l_run += __shfl_xor_sync(kFull, l_run, 2);
         lx_run += __shfl_xor_sync(kFull, lx_run, 1);
         lx_run += __shfl_xor_sync(kFull, lx_run, 2);
-        if constexpr (kFp8) {  // acc[u] = {d = 16 quad + 2u: heads 2q, 2q+1; d + 1: heads 2q, 2q+1}
-            float *lo = my_scratch + (2 * qlane) * C::kRowPitch + 16 * quad;
+        if constexpr (kFp8) {  // acc[u] = {d = (D/8) quad + 2u: heads 2q, 2q+1; d + 1: heads 2q, 2q+1}
+            float *lo = my_scratch + (2 * qlane) * C::kRowPitch + (D / 8) * quad;
             float *hi = lo + C::kRowPitch;
 #pragma unroll
             for (int u = 0; u < C::kKSteps; ++u) {
@@ -906,7 +929,7 @@ cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = p.no_pdl ? 0 : 1;
-    if (kv_fp8) return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, p, cfg) : cudaErrorInvalidValue;
+    if (kv_fp8) return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, p, cfg) : launch_variant<64, true>(tm_k, tm_v, p, cfg);
     if (head_dim == 128) return launch_variant<128, false>(tm_k, tm_v, p, cfg);
     return launch_variant<64, false>(tm_k, tm_v, p, cfg);
 }

@@ -168,6 +168,12 @@ __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t v)
 {
     return pack_f16x2(__uint_as_float(v << 16), __uint_as_float(v & 0xffff0000u));
 }
+__device__ __forceinline__ uint2 lds64(uint32_t addr)
+{
+    uint2 r;
+    asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(addr));
+    return r;
+}
 __device__ __forceinline__ uint4 lds128(uint32_t addr)
 {
     uint4 r;

@@ -131,7 +131,7 @@ def test_schedule_segment_aligned_variant(lib):
 
 
 def test_fp8_entry_point_validates_before_any_launch(lib):
-    """comem_decode_attn_fp8_async: null scales, head_dim 64 and an unknown layout are rejected on the host."""
+    """comem_decode_attn_fp8_async: null scales, an unsupported head_dim and an unknown layout are rejected on the host."""
     import ctypes
     vp = ctypes.c_void_p
     d = vp(0x1000)
@@ -142,7 +142,7 @@ def test_fp8_entry_point_validates_before_any_launch(lib):
 
     assert call(ks=None) == comem.COMEM_ERR_INVALID_ARG
     assert call(vs=None) == comem.COMEM_ERR_INVALID_ARG
-    assert call(head_dim=64) == comem.COMEM_ERR_UNSUPPORTED
+    assert call(head_dim=96) == comem.COMEM_ERR_UNSUPPORTED
     assert call(layout=7) == comem.COMEM_ERR_INVALID_ARG
     assert call(sinks=-1) == comem.COMEM_ERR_INVALID_ARG
     # valid arguments get as far as the device check (no GPU here) or the launch (never reached with these pointers)
