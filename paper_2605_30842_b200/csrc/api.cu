@@ -135,7 +135,7 @@ struct MapEntry {
     CUtensorMap map;
 };
 
-// FP8 pools (elem_bytes 1, head_dim 128 only): a token row of one kv head is 128 B, the swizzle span, so
+// FP8 pools (elem_bytes 1): a token row of one kv head is D bytes (128 B = the swizzle span at D 128; D 64: unswizzled), so
 //   dim0 = 128 bytes of d, dim1 = P * ps token rows (stride Hkv*D B), dim2 = 1, dim3 = Hkv (stride D B),
 // box {128, 16, 1, 1}: a [16 tokens][128 B] tile, 128-byte swizzled, read with 16-byte shared loads.
 // HND layout [P][Hkv][ps][D]: dim1 = ps slots (stride D B), dim2 = Hkv (stride ps*D B), dim3 = P (stride Hkv*ps*D B).

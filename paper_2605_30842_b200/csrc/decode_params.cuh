@@ -39,7 +39,7 @@ struct DecodeParams {
 };
 
 // launchers (defined in decode_split.cu / combine.cu / kv_append.cu)
-// kv_fp8: the pools hold E4M3 bytes and p.k_scale / p.v_scale are set (head_dim 128 only)
+// kv_fp8: the pools hold E4M3 bytes and p.k_scale / p.v_scale are set
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                                 const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false);
 cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
