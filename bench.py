@@ -596,6 +596,32 @@ def run_window(args) -> int:
     return 0
 
 
+def fp8_parity(fb, gpu_out, seq: int = 0):
+    """Oracle (oracle.decode_attn_fp8, all host cores) on ONE whole sequence of the FP8 batch, all its query heads,
+    from the same bytes and scales; returns (parity block, oracle seconds)."""
+    import numpy as np
+    import torch
+    import oracle
+
+    oracle.build()
+    ps = fb.page_size
+    n = (int(fb.seq_lens[seq]) + ps - 1) // ps
+    ids = fb.block_table[seq, :n].long()
+    t0 = time.perf_counter()
+    ref, _ = oracle.decode_attn_fp8(fb.q[seq:seq + 1].cpu(), fb.k_pages[ids].cpu(), fb.v_pages[ids].cpu(),
+                                    fb.k_scale[ids].cpu(), fb.v_scale[ids].cpu(),
+                                    torch.arange(n, dtype=torch.int32).view(1, n), fb.seq_lens[seq:seq + 1].cpu(),
+                                    fb.softmax_scale, kv_layout=fb.kv_layout)
+    secs = time.perf_counter() - t0
+    got = gpu_out[seq:seq + 1].double().cpu().numpy()
+    d = np.abs(got - ref)
+    par = {"rows": fb.num_q_heads, "max_abs": float(d.max()), "mean_abs": float(d.mean()),
+           "rel_l2": float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)),
+           "tol": {"max_abs": 2e-2, "mean_abs": 2e-3, "rel_l2": 5e-3}}
+    par["ok"] = bool(par["max_abs"] <= 2e-2 and par["mean_abs"] <= 2e-3 and par["rel_l2"] <= 5e-3)
+    return par, secs
+
+
 def run_fp8(args) -> int:
     """Extra: the FP8 (E4M3 + per-page, per-kv-head scale) KV-cache variant on the
     C2 / C3 / C4 batch, quantised by the input recipe (workloads.quantize_batch_fp8).  Algorithmic bytes =
@@ -694,6 +720,10 @@ def run_fp8(args) -> int:
         iso.sort()
     us = e0.elapsed_time(e1) * 1e3 / (replays * per_graph)
     gbs = nbytes / us / 1e3
+    with torch.cuda.stream(stream):
+        step(0)
+        stream.synchronize()
+    parity, oracle_s = (None, None) if args.no_cpu_baseline else fp8_parity(pools[0], outs[0])
     print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload),
                       "kv_layout": pools[0].kv_layout,
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
@@ -703,7 +733,7 @@ def run_fp8(args) -> int:
                                    "peak": peaks["hbm_gbs"], "unit": UNIT, "frac": gbs / peaks["hbm_gbs"],
                                    "us_per_launch": us,
                                    "traffic": NCU_TRAFFIC_BYTES_FP8.get((args.workload, pools[0].kv_layout))},
-                      "gpu_launches": replays * per_graph,
+                      "gpu_launches": replays * per_graph, "parity": parity, "oracle_seconds_one_sequence": oracle_s,
                       "bf16_cache_bytes_same_tokens": bf16_bytes,
                       "equivalent_bf16_gbs": bf16_bytes / us / 1e3, "clocks": sampler.summary(),
                       "burst": {"steps": burst_replays * per_graph, "us_per_step": burst_us, "value": nbytes / burst_us / 1e3,
