@@ -584,7 +584,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             }
             if constexpr (kFp8) {
                 // The tile is [16 tokens][128 B], 128-byte swizzled.  Lane (quad, qlane) reads, of token rows
-                // quad and quad + 8, the 16-byte chunks 2 qlane and 2 qlane + 1: a quarter-warp (two rows that
+                // row0 and row0 + 2 (below), the 16-byte chunks 2 qlane and 2 qlane + 1: a quarter-warp (two rows that
                 // differ in bit 0, even chunks ^ row) touches every bank once.  Each 32-bit word is one k-step's
                 // B fragment: bytes 0,1 -> b0, bytes 2,3 -> b1 (the permutation q was loaded with).
 #pragma unroll
@@ -596,12 +596,16 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 }
 #pragma unroll
                 for (int c = 0; c < kFp8Chunks; ++c) {
+                    // Score column `quad` of n-tile 0 is token row0 = 4 (quad / 2) + quad % 2 and of n-tile 1 token
+                    // row0 + 2, so that a lane's four scores are the CONSECUTIVE tokens 4 qlane .. 4 qlane + 3: the
+                    // token order in which ldmatrix.trans.b8 hands out V (S5).
                     const uint32_t chunk = (uint32_t)(kFp8Chunks * qlane + c);
-                    const uint32_t off = (D == 128 ? (chunk ^ (uint32_t)quad) : chunk) << 4;
+                    const int row0 = 4 * (quad >> 1) + (quad & 1);
+                    const uint32_t off0 = (D == 128 ? (chunk ^ (uint32_t)(row0 & 7)) : chunk) << 4;
+                    const uint32_t off1 = (D == 128 ? (chunk ^ (uint32_t)((row0 + 2) & 7)) : chunk) << 4;
 #pragma unroll
                     for (int k = 0; k < NT; ++k) {
-                        const uint32_t row_lo = k_base[k] + quad * D + off;  // (quad + 8) & 7 == quad: same swizzle
-                        const uint4 ka = lds128(row_lo), kb = lds128(row_lo + 8 * D);
+                        const uint4 ka = lds128(k_base[k] + row0 * D + off0), kb = lds128(k_base[k] + (row0 + 2) * D + off1);
                         const uint32_t wa[4] = {ka.x, ka.y, ka.z, ka.w}, wb[4] = {kb.x, kb.y, kb.z, kb.w};
 #pragma unroll
                         for (int w = 0; w < 4; ++w) {
@@ -624,7 +628,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                     }
                 }
             }
-            float sv[NT][4];  // tokens 2q, 2q+1, 2q+8, 2q+9 of head `quad`
+            float sv[NT][4];  // tokens 2q, 2q+1, 2q+8, 2q+9 (FP8: 4q .. 4q+3) of head `quad`
 #pragma unroll
             for (int k = 0; k < NT; ++k) {
                 sv[k][0] = s[k][0][0] * sl2[k];
@@ -634,11 +638,13 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 if (alive[k] != 0xffffu) {
                     // edge tile: mask by index (never by arithmetic) and zero the dead V rows so that
                     // NaN/Inf garbage in tokens that do not count cannot reach the accumulators (0 * NaN).
-                    const int tok = 2 * qlane;
+                    // this lane's four scores: tokens 2q, 2q+1, 2q+8, 2q+9 (bf16) or 4q .. 4q+3 (FP8, see S3)
+                    const int tok = kFp8 ? 4 * qlane : 2 * qlane;
+                    constexpr int kSecond = kFp8 ? 2 : 8;
                     if (!((alive[k] >> tok) & 1u)) sv[k][0] = -INFINITY;
                     if (!((alive[k] >> (tok + 1)) & 1u)) sv[k][1] = -INFINITY;
-                    if (!((alive[k] >> (tok + 8)) & 1u)) sv[k][2] = -INFINITY;
-                    if (!((alive[k] >> (tok + 9)) & 1u)) sv[k][3] = -INFINITY;
+                    if (!((alive[k] >> (tok + kSecond)) & 1u)) sv[k][2] = -INFINITY;
+                    if (!((alive[k] >> (tok + kSecond + 1)) & 1u)) sv[k][3] = -INFINITY;
                     constexpr int kChunksPerRow = D * C::kElemBytes / 16;  // 16-byte chunks per V row
                     for (int idx = lane; idx < kTileTokens * kChunksPerRow; idx += 32) {
                         const int row = idx / kChunksPerRow;
@@ -672,8 +678,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 esum += (e0 + e1) + (e2 + e3);
                 if constexpr (kFp8) {
                     // the page's v_scale rides on p (fp16, 11 significant bits); the normaliser is the unrounded sum
-                    p01[k] = pack_f16x2(e0 * v_scale[k], e1 * v_scale[k]);  // tokens 2q, 2q+1
-                    p23[k] = pack_f16x2(e2 * v_scale[k], e3 * v_scale[k]);  // tokens 2q+8, 2q+9
+                    p01[k] = pack_f16x2(e0 * v_scale[k], e1 * v_scale[k]);  // tokens 4q, 4q+1   (k slots 2q, 2q+1)
+                    p23[k] = pack_f16x2(e2 * v_scale[k], e3 * v_scale[k]);  // tokens 4q+2, 4q+3 (k slots 2q+8, 2q+9)
                 } else {
                     p01[k] = pack_bf16x2(e0, e1);
                     p23[k] = pack_bf16x2(e2, e3);
@@ -698,47 +704,24 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 
             // S5: O^T[16 d x 8 heads] += V^T[16 d x 16 tok] * P^T[16 tok x 8 heads]
             if constexpr (kFp8) {
-                // Lane (quad, qlane) reads the 16-byte chunk `quad` (d = 16 quad .. 16 quad + 15) of its four
-                // token rows 2q, 2q+1, 2q+8, 2q+9 (a quarter-warp: rows & 7 all even or all odd, chunks 2j and
-                // 2j+1 -> every bank once).  A-fragment registers pair two TOKENS of one d: PRMT interleaves the
-                // bytes of two rows, the conversion widens each byte pair.  m-tile u of this lane is
-                // {row quad: d = 16 quad + 2u, row quad + 8: d = 16 quad + 2u + 1}; S6 scatters accordingly.
-                // (D = 64: 8 bytes per row and lane, d = 8 quad .. 8 quad + 7, two words, four m-tiles.)
-                const int t0 = 2 * qlane;
-                constexpr int kWords = D / 32;  // 32-bit words of a V row each lane reads
-                uint32_t o_even, o_odd;
-                if constexpr (D == 128) {
-                    const uint32_t ch = (uint32_t)quad;
-                    o_even = t0 * 128 + ((ch ^ (uint32_t)(t0 & 7)) << 4);
-                    o_odd = (t0 + 1) * 128 + ((ch ^ (uint32_t)((t0 + 1) & 7)) << 4);
-                } else {
-                    o_even = t0 * 64 + 8 * quad;
-                    o_odd = (t0 + 1) * 64 + 8 * quad;
-                }
+                // ldmatrix.m16n16.trans.b8 hands each lane, per 16-token x 16-d byte block, the tokens 4q .. 4q+3 of
+                // columns d = quad and quad + 8: the two byte pairs of a register widen (exactly) to the fp16 pairs
+                // {a0 | a2} (row quad) and {a1 | a3} (row quad + 8) of the A fragment of m-tile mt -- the same
+                // accumulator layout as the bf16 path, no byte shuffling.  One x2 load covers two m-tiles.
+                const int lrow = lane & 15, lmat = lane >> 4;
 #pragma unroll
                 for (int k = 0; k < NT; ++k) {
-                    uint32_t w0[4], w1[4], w2[4], w3[4];
-                    if constexpr (D == 128) {
-                        const uint4 r0 = lds128(v_base[k] + o_even), r1 = lds128(v_base[k] + o_odd);
-                        const uint4 r2 = lds128(v_base[k] + o_even + 8 * 128), r3 = lds128(v_base[k] + o_odd + 8 * 128);
-                        w0[0] = r0.x; w0[1] = r0.y; w0[2] = r0.z; w0[3] = r0.w;
-                        w1[0] = r1.x; w1[1] = r1.y; w1[2] = r1.z; w1[3] = r1.w;
-                        w2[0] = r2.x; w2[1] = r2.y; w2[2] = r2.z; w2[3] = r2.w;
-                        w3[0] = r3.x; w3[1] = r3.y; w3[2] = r3.z; w3[3] = r3.w;
-                    } else {
-                        const uint2 r0 = lds64(v_base[k] + o_even), r1 = lds64(v_base[k] + o_odd);
-                        const uint2 r2 = lds64(v_base[k] + o_even + 8 * 64), r3 = lds64(v_base[k] + o_odd + 8 * 64);
-                        w0[0] = r0.x; w0[1] = r0.y; w1[0] = r1.x; w1[1] = r1.y;
-                        w2[0] = r2.x; w2[1] = r2.y; w3[0] = r3.x; w3[1] = r3.y;
-                    }
 #pragma unroll
-                    for (int w = 0; w < kWords; ++w) {
-                        const uint32_t x01e = prmt(w0[w], w1[w], 0x5140u), x23e = prmt(w2[w], w3[w], 0x5140u);
-                        const uint32_t x01o = prmt(w0[w], w1[w], 0x7362u), x23o = prmt(w2[w], w3[w], 0x7362u);
-                        mma_f16_16816(acc[2 * w], e4m3x2_lo_to_f16x2(x01e), e4m3x2_hi_to_f16x2(x01e),
-                                      e4m3x2_lo_to_f16x2(x23e), e4m3x2_hi_to_f16x2(x23e), p01[k], p23[k]);
-                        mma_f16_16816(acc[2 * w + 1], e4m3x2_lo_to_f16x2(x01o), e4m3x2_hi_to_f16x2(x01o),
-                                      e4m3x2_lo_to_f16x2(x23o), e4m3x2_hi_to_f16x2(x23o), p01[k], p23[k]);
+                    for (int mp = 0; mp < C::kKSteps / 2; ++mp) {
+                        const uint32_t chunk = (uint32_t)(2 * mp + lmat);
+                        const uint32_t a = D == 128 ? v_base[k] + lrow * 128 + ((chunk ^ (uint32_t)(lrow & 7)) << 4)
+                                                    : v_base[k] + lrow * 64 + (chunk << 4);
+                        uint32_t r[4];
+                        ldmatrix_b8_x2_trans(r, a);
+                        mma_f16_16816(acc[2 * mp], e4m3x2_lo_to_f16x2(r[0]), e4m3x2_lo_to_f16x2(r[1]),
+                                      e4m3x2_hi_to_f16x2(r[0]), e4m3x2_hi_to_f16x2(r[1]), p01[k], p23[k]);
+                        mma_f16_16816(acc[2 * mp + 1], e4m3x2_lo_to_f16x2(r[2]), e4m3x2_lo_to_f16x2(r[3]),
+                                      e4m3x2_hi_to_f16x2(r[2]), e4m3x2_hi_to_f16x2(r[3]), p01[k], p23[k]);
                     }
                 }
             } else {
@@ -779,15 +762,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         l_run += __shfl_xor_sync(kFull, l_run, 2);
         lx_run += __shfl_xor_sync(kFull, lx_run, 1);
         lx_run += __shfl_xor_sync(kFull, lx_run, 2);
-        if constexpr (kFp8) {  // acc[u] = {d = (D/8) quad + 2u: heads 2q, 2q+1; d + 1: heads 2q, 2q+1}
-            float *lo = my_scratch + (2 * qlane) * C::kRowPitch + (D / 8) * quad;
-            float *hi = lo + C::kRowPitch;
-#pragma unroll
-            for (int u = 0; u < C::kKSteps; ++u) {
-                *reinterpret_cast<float2 *>(lo + 2 * u) = make_float2(acc[u][0], acc[u][2]);
-                *reinterpret_cast<float2 *>(hi + 2 * u) = make_float2(acc[u][1], acc[u][3]);
-            }
-        } else {
+        {
             float *lo = my_scratch + (2 * qlane) * C::kRowPitch + quad;
             float *hi = lo + C::kRowPitch;
 #pragma unroll

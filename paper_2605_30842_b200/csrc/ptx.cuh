@@ -168,6 +168,16 @@ __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t v)
 {
     return pack_f16x2(__uint_as_float(v << 16), __uint_as_float(v & 0xffff0000u));
 }
+// Two 16x16 BYTE matrices, transposed on the way (sm_100a): lanes 0..15 give the 16-byte row addresses of
+// matrix 0, lanes 16..31 those of matrix 1.  With rows = tokens and columns = d, lane (quad = lane / 4, q = lane % 4)
+// gets r[0] = {tokens 4q..4q+3 of column quad}, r[1] = {same tokens, column quad + 8} of matrix 0, r[2], r[3]
+// likewise of matrix 1 (layout measured with a probe kernel; it is the 8-bit A-fragment layout).
+__device__ __forceinline__ void ldmatrix_b8_x2_trans(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(addr));
+}
 __device__ __forceinline__ uint2 lds64(uint32_t addr)
 {
     uint2 r;
