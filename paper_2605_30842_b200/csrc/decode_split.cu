@@ -3,14 +3,14 @@
 // for one decode step of paged GQA attention.
 //
 // Shape of the kernel (sm_100a):
-//   * persistent grid, ONE CTA per SM (10 warps, ~214 KiB of shared memory), one contiguous range
+//   * persistent grid, ONE CTA per SM (12 warps, ~214 KiB of shared memory), one contiguous range
 //     of 16-token tiles per CTA (schedule.cuh);
 //   * before griddepcontrol.wait (i.e. under the previous kernel's tail): mbarrier init, tensor-map
 //     prefetch, an L2 prefetch of the small control inputs (seq_lens, block table, q), the whole
 //     schedule computed SPECULATIVELY from seq_lens as it reads now (validated after the wait),
 //     and a TMA L2 prefetch of the CTA's first 16 tiles;
-//   * warps 8, 9 = producers: each reads the block table 32 entries at a time and issues, for
-//     every other tile of the CTA, one TMA tiled load for K and one for V ([16 tokens][D] of one kv
+//   * warps 8..11 = producers: each reads the block table 32 entries at a time and issues, for
+//     every fourth tile of the CTA, one TMA tiled load for K and one for V ([16 tokens][D] of one kv
 //     head, 128-byte swizzle) into a 16-stage shared-memory ring guarded by full/empty
 //     mbarriers -- 128 KiB of K+V in flight per SM (one producer lane is issue-rate bound);
 //   * warps 0..7 = consumers: tile n of the CTA goes to warp n % 8, so eight independent
@@ -31,6 +31,9 @@
 //     stand-alone K2 (combine.cu) does the merge.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
+#ifndef COMEM_BF16_PRODUCER_WARPS
+#define COMEM_BF16_PRODUCER_WARPS 4  // measured on config 2: 2 -> 25.8 us, 4 -> 25.4 us per step (faster ring fill after the PDL wait)
+#endif
 #ifndef COMEM_FP8_TILES_PER_PASS
 #define COMEM_FP8_TILES_PER_PASS 1
 #endif
@@ -62,7 +65,7 @@ struct Cfg {
     // its shared-memory reads are not conflict-free and need not be)
     static constexpr int kElemBytes = kFp8 ? 1 : 2;
     // one elected lane per producer warp; tiles are dealt round-robin to them (one lane is issue-rate bound)
-    static constexpr int kProducerWarps = kFp8 ? 4 : 2;
+    static constexpr int kProducerWarps = kFp8 ? 4 : COMEM_BF16_PRODUCER_WARPS;
     static constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
     static constexpr int kPrefetch = kFp8 ? 2 * kPrefetchTiles : kPrefetchTiles;
     static_assert(kPrefetch <= 32, "one prefetched tile per lane");
