@@ -45,8 +45,8 @@ FALLBACK_PEAK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES_NOMINAL = 126e6
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE split-KV launch from the committed
-# `ncu --set full` capture (profiles/r1_b_fused.md names the command).
-NCU_TRAFFIC_BYTES = {"c2": 137_632_512, "c3": 4_838_226_768, "c4": 8_595_141_560}  # profiles/r1_b_fused.md
+# `ncu --set full` capture (profiles/r1_b_fused.md names the command; c2 re-captured in profiles/r1_c_fp8_pipeline.md).
+NCU_TRAFFIC_BYTES = {"c2": 137_713_664, "c3": 4_838_226_768, "c4": 8_595_141_560}  # profiles/r1_b_fused.md
 # same for the FP8 kernel (profiles/r1_c_fp8_pipeline.md section 3): (workload, layout) -> bytes
 NCU_TRAFFIC_BYTES_FP8 = {("c4", "NHD"): 4_324_995_000 + 3_796_224, ("c4", "HND"): 4_301_188_000 + 3_680_768}
 
