@@ -67,7 +67,7 @@ struct Cfg {
     // one elected lane per producer warp; tiles are dealt round-robin to them (one lane is issue-rate bound)
     static constexpr int kProducerWarps = kFp8 ? 4 : COMEM_BF16_PRODUCER_WARPS;
     static constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
-    static constexpr int kPrefetch = kFp8 ? 2 * kPrefetchTiles : kPrefetchTiles;
+    static constexpr int kPrefetch = kFp8 ? (2 * kPrefetchTiles < 32 ? 2 * kPrefetchTiles : 32) : kPrefetchTiles;
     static_assert(kPrefetch <= 32, "one prefetched tile per lane");
     static constexpr int kTileBytes = kTileTokens * D * kElemBytes;  // one K (or V) tile
     static constexpr int kStageBytes = 2 * kTileBytes;      // K + V
