@@ -19,6 +19,9 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
                  int row_elems, int page_size, int max_pages, const __nv_bfloat16 *q_src,
                  __nv_bfloat16 *q_dst, int q_row_elems)
 {
+    // let the attention kernel queued behind this one start its prologue now (it computes its schedule
+    // speculatively and re-validates after ITS griddepcontrol.wait, which still waits for this grid to finish)
+    pdl_launch_dependents();
     pdl_wait_prior_grid();
     const int b = blockIdx.x;
     if (q_src != nullptr) {
@@ -53,6 +56,7 @@ kv_append_fp8_kernel(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, c
                      const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
                      const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int max_pages, int hnd)
 {
+    pdl_launch_dependents();  // as in kv_append_kernel
     pdl_wait_prior_grid();
     const int b = blockIdx.x;
     const int t = seq_lens[b];
