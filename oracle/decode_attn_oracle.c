@@ -39,6 +39,9 @@
  * decode table vs the format's published values and vs torch's float8_e4m3fn cast; equals the pinned
  * bf16 oracle on a cache whose values both formats hold exactly; L = 1 closed form; scale
  * linearity; tail / unused-page poison independence; brute-force dense numpy fp64).
+ * oracle_e4m3_encode / oracle_kv_append_fp8: E1..E4, A1 (same file: inverse of the decode table; torch's cast on
+ * random values and on every tie; saturation; hand-computed ties; placement, untouched bytes, page crossing, HND).
+ * F7: the HND layout is a relayout of NHD (bit-identical).
  */
 #include <math.h>
 #include <stdint.h>
