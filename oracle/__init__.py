@@ -61,6 +61,8 @@ def _load():
         lib.oracle_e4m3_encode.restype = i32
         lib.oracle_kv_append_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32]
         lib.oracle_kv_append_fp8.restype = i32
+        lib.oracle_prefill_attn.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, vp, i32, i32, i32]
+        lib.oracle_prefill_attn.restype = i32
         lib.oracle_max_threads.restype = i32
         _lib = lib
     return _lib
@@ -261,3 +263,23 @@ def kv_append_fp8(k_bytes, v_bytes, k_scale, v_scale, block_table, seq_lens, new
                                   hkv, d, ps, bt.shape[0], bt.shape[1], 1 if hnd else 0)
     if rc != 0:
         raise ValueError("oracle_kv_append_fp8: sequence would outgrow its block-table row")
+
+
+def prefill_attn(q, k_pages, v_pages, block_table, seq_lens, q_start, softmax_scale, num_threads: int = 0):
+    """Causal prefill attention of the last q_len_b = q_start[b+1] - q_start[b] tokens of every sequence over the
+    paged cache (reading R20).  q: bf16 [total_q, Hq, D] ragged.  Returns (out [total_q, Hq, D], lse [total_q, Hq])."""
+    lib = _load()
+    qb, kb, vb = as_bits(q), as_bits(k_pages), as_bits(v_pages)
+    bt, sl, qs = _as_i32(block_table), _as_i32(seq_lens), _as_i32(q_start)
+    total_q, hq, d = qb.shape
+    _, ps, hkv, _ = kb.shape
+    batch = sl.shape[0]
+    assert qs.shape == (batch + 1,) and int(qs[-1]) == total_q
+    out = np.empty((total_q, hq, d), np.float64)
+    lse = np.empty((total_q, hq), np.float64)
+    rc = lib.oracle_prefill_attn(_p(qb), _p(kb), _p(vb), _p(bt), _p(sl), _p(qs), hq, hkv, d, ps,
+                                 ctypes.c_float(float(np.float32(softmax_scale))), _p(out), _p(lse), batch,
+                                 bt.shape[1], int(num_threads))
+    if rc != 0:
+        raise ValueError("oracle_prefill_attn: invalid argument")
+    return out, lse

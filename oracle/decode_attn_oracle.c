@@ -42,6 +42,8 @@
  * oracle_e4m3_encode / oracle_kv_append_fp8: E1..E4, A1 (same file: inverse of the decode table; torch's cast on
  * random values and on every tie; saturation; hand-computed ties; placement, untouched bytes, page crossing, HND).
  * F7: the HND layout is a relayout of NHD (bit-identical).
+ * oracle_prefill_attn: PF1..PF5 (tests/test_oracle_prefill_pins.py: q_len 1 is the decode oracle; every row equals
+ * the decode oracle on the cache truncated at its position; torch causal SDPA fp64; chunked == full; brute force).
  */
 #include <math.h>
 #include <stdint.h>
@@ -479,6 +481,77 @@ int oracle_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scal
             }
         }
         seq_lens[b] = (int32_t)(t + 1);
+    }
+    return 0;
+}
+
+/*
+ * Prefill attention over the paged cache (Alg. 1 lines 9-13: "Prefill new tokens
+ * only" (cached) / "Prefill full context" (uncached); reading R20).  Sequence b has seq_lens[b] = L cached tokens,
+ * the LAST n_b = q_start[b+1] - q_start[b] of which are the new ones; their queries are rows
+ * q[q_start[b] .. q_start[b+1]) of the ragged q [total_q][Hq][D].  Query i of the chunk sits at position
+ * pos = L - n_b + i and attends causally: keys t <= pos.
+ *     out[row][h] = softmax_{t <= pos}(softmax_scale * q[row][h] . k_t) . V
+ * n_b = 1 is the decode step (oracle_decode_attn); n_b = L is the uncached full prefill.  Same two-pass fp64
+ * statement per (row, h).  Rows with n_b > L are invalid (return 1).
+ */
+int oracle_prefill_attn(const uint16_t *q,           /* bf16 [total_q][Hq][D] */
+                        const uint16_t *k_pages, const uint16_t *v_pages, const int32_t *block_table,
+                        const int32_t *seq_lens, const int32_t *q_start /* [batch + 1] */, int num_q_heads,
+                        int num_kv_heads, int head_dim, int page_size, float softmax_scale, double *out,
+                        double *lse, int batch, int max_pages_per_seq, int num_threads)
+{
+    if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !q_start || !out) return 1;
+    if (num_q_heads <= 0 || num_kv_heads <= 0 || num_q_heads % num_kv_heads != 0) return 1;
+    if (head_dim <= 0 || page_size <= 0 || batch <= 0 || q_start[0] != 0) return 1;
+    for (int b = 0; b < batch; ++b) {
+        const int n = q_start[b + 1] - q_start[b];
+        if (n < 0 || n > seq_lens[b]) return 1;
+    }
+    const int G = num_q_heads / num_kv_heads;
+    const int D = head_dim;
+    const int64_t rows = (int64_t)q_start[batch] * num_q_heads;
+    const double scale = (double)softmax_scale;
+#ifdef _OPENMP
+    if (num_threads <= 0) num_threads = omp_get_max_threads();
+#else
+    (void)num_threads;
+#endif
+#pragma omp parallel for schedule(dynamic, 1) num_threads(num_threads)
+    for (int64_t r = 0; r < rows; ++r) {
+        const int row = (int)(r / num_q_heads), h = (int)(r % num_q_heads);
+        int b = 0;
+        while (q_start[b + 1] <= row) ++b;            /* the sequence this query row belongs to */
+        const int kvh = h / G;
+        const int64_t L = seq_lens[b];
+        const int64_t n = q_start[b + 1] - q_start[b];
+        const int64_t pos = L - n + (row - q_start[b]);  /* position of this query; attends t <= pos */
+        const int32_t *bt = block_table + (int64_t)b * max_pages_per_seq;
+        double *o = out + r * D;
+        for (int d = 0; d < D; ++d) o[d] = 0.0;
+        double *qd = (double *)malloc(sizeof(double) * D);
+        double *s = (double *)malloc(sizeof(double) * (size_t)(pos + 1));
+        const uint16_t *qrow = q + r * D;
+        for (int d = 0; d < D; ++d) qd[d] = bf16_to_double(qrow[d]);
+        double m = -INFINITY;
+        for (int64_t t = 0; t <= pos; ++t) {
+            const uint16_t *krow = paged_row(k_pages, bt, t, kvh, num_kv_heads, D, page_size);
+            double dot = 0.0;
+            for (int d = 0; d < D; ++d) dot += qd[d] * bf16_to_double(krow[d]);
+            s[t] = scale * dot;
+            if (s[t] > m) m = s[t];
+        }
+        double Z = 0.0;
+        for (int64_t t = 0; t <= pos; ++t) {
+            const double w = exp(s[t] - m);
+            const uint16_t *vrow = paged_row(v_pages, bt, t, kvh, num_kv_heads, D, page_size);
+            Z += w;
+            for (int d = 0; d < D; ++d) o[d] += w * bf16_to_double(vrow[d]);
+        }
+        for (int d = 0; d < D; ++d) o[d] /= Z;
+        if (lse) lse[r] = m + log(Z);
+        free(s);
+        free(qd);
     }
     return 0;
 }
