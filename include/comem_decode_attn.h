@@ -221,6 +221,36 @@ int comem_net_speedup(double y_tokens, double l_full, double l_sum, double s_gb_
 double comem_max_compression_ratio(double w_gb_per_s, double y_tokens, double s_gb_per_token,
                                    double p_tokens_per_s);
 
+/*
+ * comem_prefill_attn_async — causal prefill attention over the paged cache: the compute-bound
+ * step of the path.  P:L149-156 (Algorithm 1 lines 9-13): "Prefill new tokens only" when the KV cache is valid
+ * (cached, incremental prefill), "Prefill full context" after a summary adoption invalidated it (uncached);
+ * P:L57-59 (§2.2: prefill is compute-bound, it sets TTFT); P:L122 (§3.2: "a full uncached prefill is required"
+ * after every adoption); P:L245 (chunked prefill + prefix caching in the paper's serving engine).  The formula is
+ * DESIGN.md reading R20: sequence b holds seq_lens[b] = L_b cached tokens, the LAST n_b = q_start[b+1] - q_start[b]
+ * of which are the new ones (their K/V rows are already in the cache); query i of the chunk sits at position
+ * pos = L_b - n_b + i and attends the keys t <= pos:
+ *     out[q_start[b] + i, h, :] = sum_{t <= pos} softmax_t(softmax_scale * q[q_start[b] + i, h, :] . k_t[kvh, :]) v_t[kvh, :]
+ * n_b = 1 is the decode step; n_b = L_b is the uncached full prefill; n_b = 0 contributes no rows.
+ *
+ *   q            device, bf16 [total_q][num_q_heads][head_dim], contiguous: the chunks of all sequences back to back
+ *   q_start      device, int32 [batch + 1], q_start[0] = 0, non-decreasing, q_start[batch] = total_q;
+ *                n_b <= seq_lens[b] (a longer chunk is undefined behaviour, like every other device-side datum)
+ *   out          device, bf16 [total_q][num_q_heads][head_dim]; lse_out device fp32 [total_q][num_q_heads] or NULL
+ *   total_q      host copy of q_start[batch] (sizes the grid and the q tensor map)
+ *   k_pages, v_pages, block_table, seq_lens, softmax_scale, num_pages, max_pages_per_seq: as comem_decode_attn_async
+ * Shapes: head_dim 64 or 128, page_size 16 or 32, G = num_q_heads / num_kv_heads <= 16.
+ * Enqueue-only, 1 kernel (tcgen05 tensor cores, accumulators in tensor memory), no workspace.  Deterministic: a row
+ * is reduced by one thread in logical token order; physical page placement never enters the arithmetic.
+ * Arithmetic: bf16 x bf16 -> fp32 on the tensor cores, softmax in fp32 (log2 domain), P rounded to bf16 for the
+ * second product with the normaliser summed from the ROUNDED p (reading R16), bf16 output, round-to-nearest-even.
+ */
+int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_pages,
+                             const int32_t *block_table, const int32_t *seq_lens, const int32_t *q_start,
+                             int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                             float softmax_scale, void *out, int batch, int total_q, int max_pages_per_seq,
+                             int64_t num_pages, float *lse_out, void *cuda_stream);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,

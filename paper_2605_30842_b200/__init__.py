@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     COMEM_PHASE_SPLIT,
     COMEM_PHASE_COMBINE,
     comem_decode_attn_fp8_async,
+    comem_prefill_attn_async,
     comem_decode_attn_workspace_bytes,
     comem_decode_saving_seconds,
     comem_kstep_context_lengths,

@@ -58,6 +58,9 @@ def load_library():
     lib.comem_decode_attn_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                                 i32, i64, vp, vp, sz, vp, i32, i32, i32]
     lib.comem_decode_attn_fp8_async.restype = i32
+    lib.comem_prefill_attn_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i32,
+                                             i64, vp, vp]
+    lib.comem_prefill_attn_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
     lib.comem_decode_attn.restype = i32
@@ -252,7 +255,7 @@ def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, s
 
 def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
                             workspace, lse_out=None, stream=None) -> None:
-    """Enqueue one decode-attention step (2 kernel launches) on ``stream``; returns at once."""
+    """Enqueue one decode-attention step (1 fused kernel launch) on ``stream``; returns at once."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
     st = load_library().comem_decode_attn_async(
@@ -323,6 +326,28 @@ def comem_kv_append_fp8_async(k_pages, v_pages, k_scale, v_scale, block_table, s
         raise ComemError(st, "comem_kv_append_fp8_async")
 
 
+def comem_prefill_attn_async(q, k_pages, v_pages, block_table, seq_lens, q_start, softmax_scale: float, out,
+                             lse_out=None, stream=None) -> None:
+    """Causal prefill attention of each sequence's last q_start[b+1] - q_start[b] tokens over the paged cache
+    (one tcgen05 kernel on ``stream``).  q, out: bf16 [total_q, Hq, D]; q_start: int32 [batch + 1] on the device."""
+    assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.dim() == 3
+    assert k_pages.dtype == torch.bfloat16 and v_pages.dtype == torch.bfloat16
+    assert k_pages.is_contiguous() and v_pages.is_contiguous() and k_pages.dim() == 4 and k_pages.shape == v_pages.shape
+    assert k_pages.shape[3] == q.shape[2]
+    assert block_table.dtype == torch.int32 and block_table.is_contiguous() and block_table.dim() == 2
+    assert seq_lens.dtype == torch.int32 and seq_lens.is_contiguous() and seq_lens.shape == (block_table.shape[0],)
+    assert q_start.dtype == torch.int32 and q_start.is_contiguous() and q_start.shape == (block_table.shape[0] + 1,)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    if lse_out is not None:
+        assert lse_out.dtype == torch.float32 and lse_out.is_contiguous() and tuple(lse_out.shape) == tuple(q.shape[:2])
+    st = load_library().comem_prefill_attn_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), _ptr(q_start), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        block_table.shape[0], q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_prefill_attn_async")
+
+
 def comem_decode_attn(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out=None,
                       workspace=None, lse_out=None):
     """Synchronous form (legacy default stream + cudaStreamSynchronize).  Returns ``out``."""
@@ -377,6 +402,3 @@ def comem_decode_step_host(q_host, new_k_host, new_v_host, k_pages, v_pages, blo
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_step_host")
 
-
-# kept for symmetry with the header's name list
-comem_decode_attn_host = comem_decode_step_host

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "decode_params.cuh"
+#include "prefill_params.cuh"
 #include "schedule.cuh"
 
 namespace comem {
@@ -20,6 +21,7 @@ namespace {
 constexpr int kMaxGridCtas = 1024;  // workspace is sized for this many persistent CTAs
 static_assert(kMaxGridCtas == kMaxGridCtasBound, "schedule.cuh's 32-bit fast paths assume this bound");
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr int kPrefillMaxGroup = 16;  // a 128-row query tile holds 128 / G positions x G heads
 static_assert(kMaxBatch == COMEM_MAX_BATCH, "header and scheduler disagree on the batch limit");
 
 std::atomic<int> g_grid_override{0};
@@ -182,6 +184,26 @@ int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, 
     else { cache[next_evict] = e; next_evict = (next_evict + 1) % cache.size(); }
     *out = e.map;
     return COMEM_OK;
+}
+
+// Ragged query tensor q [total_q][Hq][D] of the prefill kernel, as a 4-D tensor
+//   dim0 = 64 elements of d (128 B)   dim1 = Hq heads (stride D*2 B)   dim2 = total_q rows (stride Hq*D*2 B)
+//   dim3 = D / 64 halves (stride 128 B)
+// with box {64, G, R, D/64}: one load brings the G heads of one kv head's group for R consecutive query rows and lays
+// them in shared memory as [D/64][R][G][128 B], 128-byte swizzled -- row (position * G + head) of a K-major
+// tcgen05 A operand.  Rows past total_q are zero-filled.  Not cached: one encode per call (host arithmetic only).
+int make_q_tensor_map(const void *q, int64_t total_q, int hq, int d, int group, int rows, CUtensorMap *out)
+{
+    EncodeFn enc = encode_fn();
+    if (!enc) return COMEM_ERR_CUDA;
+    const cuuint64_t gdim[4] = {64, (cuuint64_t)hq, (cuuint64_t)total_q, (cuuint64_t)(d / 64)};
+    const cuuint64_t gstride[3] = {(cuuint64_t)d * 2, (cuuint64_t)hq * d * 2, 128};
+    const cuuint32_t box[4] = {64, (cuuint32_t)group, (cuuint32_t)rows, (cuuint32_t)(d / 64)};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(q), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? COMEM_OK : COMEM_ERR_CUDA;
 }
 
 int grid_for(int head_dim, int *grid)
@@ -473,6 +495,59 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                                           head_dim, page_size, softmax_scale, out, batch, max_pages_per_seq,
                                           num_pages, lse_out, workspace, workspace_bytes, cuda_stream,
                                           COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
+}
+
+int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,
+                             const int32_t *seq_lens, const int32_t *q_start, int num_q_heads, int num_kv_heads,
+                             int head_dim, int page_size, float softmax_scale, void *out, int batch, int total_q,
+                             int max_pages_per_seq, int64_t num_pages, float *lse_out, void *cuda_stream)
+{
+    if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !q_start || !out) return COMEM_ERR_INVALID_ARG;
+    if (batch <= 0 || total_q <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || max_pages_per_seq <= 0 || num_pages <= 0)
+        return COMEM_ERR_INVALID_ARG;
+    if (num_q_heads % num_kv_heads != 0) return COMEM_ERR_INVALID_ARG;
+    const int g = num_q_heads / num_kv_heads;
+    if (head_dim != 64 && head_dim != 128) return COMEM_ERR_UNSUPPORTED;
+    if (page_size != 16 && page_size != 32) return COMEM_ERR_UNSUPPORTED;
+    if (g > kPrefillMaxGroup || batch > COMEM_MAX_BATCH) return COMEM_ERR_UNSUPPORTED;
+    if (num_pages * page_size >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
+    if (!std::isfinite(softmax_scale) || softmax_scale < 0.f) return COMEM_ERR_INVALID_ARG;
+    if (!aligned(q, 16) || !aligned(out, 16) || !aligned(k_pages, 128) || !aligned(v_pages, 128) ||
+        !aligned(block_table, 4) || !aligned(seq_lens, 4) || !aligned(q_start, 4) || (lse_out && !aligned(lse_out, 4)))
+        return COMEM_ERR_INVALID_ARG;
+    int st = check_device();
+    if (st != COMEM_OK) return st;
+
+    PrefillParams p;
+    p.block_table = block_table;
+    p.seq_lens = seq_lens;
+    p.q_start = q_start;
+    p.out = static_cast<__nv_bfloat16 *>(out);
+    p.lse_out = lse_out;
+    p.batch = batch;
+    p.num_q_heads = num_q_heads;
+    p.num_kv_heads = num_kv_heads;
+    p.group = g;
+    p.rows_per_tile = 128 / g;
+    p.max_pages = max_pages_per_seq;
+    p.page_size = page_size;
+    p.page_tile_shift = page_size == 32 ? 1 : 0;
+    p.scale_log2 = softmax_scale * kLog2e;
+
+    CUtensorMap tm_q, tm_k, tm_v;
+    if ((st = make_q_tensor_map(q, total_q, num_q_heads, head_dim, g, p.rows_per_tile, &tm_q)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v)) != COMEM_OK) return st;
+    // upper bound on sum_b ceil(n_b / 2R): the chunk lengths live on the device
+    const int64_t pair_pos = 2 * (int64_t)p.rows_per_tile;
+    const int64_t items = ((int64_t)total_q / pair_pos + (batch < total_q ? batch : total_q)) * num_kv_heads;
+    if (items >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
+    if (launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, (int)items, static_cast<cudaStream_t>(cuda_stream),
+                            g_pdl.load() != 0) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return COMEM_OK;
 }
 
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,

@@ -55,6 +55,7 @@ constexpr int kConsumerThreads = kConsumerWarps * 32;
 static_assert(kConsumerWarps == kMaxGroup, "S6 and merge.cuh map warp w to query head w of the group");
 constexpr int kPrefetchTiles = COMEM_PREFETCH_TILES;  // per CTA, L2-prefetched before the PDL wait (<= 32: one per lane)
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kFp8PShift = 14;  // FP8 cache: p * f * 2^(ev - eref) * 2^14 < 2 * 2^14 stays below fp16's 65504 (S4)
 
 // kFp8: the FP8 (E4M3 + per-page, per-kv-head scale) cache of reading R18.  Tiles are half the bytes,
 // so the ring has twice the stages (same 128 KiB in flight) and twice the producer warps (a tile
@@ -540,6 +541,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         float m_run = -INFINITY;  // running max (log2 domain) of head `quad`
         float l_run = 0.f;        // this thread's share of the running sum of the bf16-ROUNDED p (normaliser)
         float lx_run = 0.f;       // same for the unrounded p (only feeds lse_out)
+        // FP8 cache: acc is kept in units of 2^(eref - 127 - kFp8PShift), eref = the largest biased exponent of a
+        // page's v_scale seen so far (warp-uniform); see S4
+        [[maybe_unused]] int eref = 0;
         float acc[C::kKSteps][4]; // O^T: rows d = 16*mt + quad (+8), cols heads 2*qlane (+1)
 #pragma unroll
         for (int mt = 0; mt < C::kKSteps; ++mt) acc[mt][0] = acc[mt][1] = acc[mt][2] = acc[mt][3] = 0.f;
@@ -674,15 +678,43 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             uint32_t p01[NT], p23[NT];
             float esum = 0.f;
             [[maybe_unused]] float rsum = 0.f;
+            // FP8 cache: the page's v_scale = f * 2^ev rides on p, which the tensor op wants in fp16.  p <= 1 times a
+            // scale of ~1e-3 would sit in the fp16 SUBNORMALS (below 2^-14) for every token more than a few nats under
+            // the row maximum and lose its bits while l still counts it.  So only f * 2^(ev - eref) goes on p, lifted
+            // by 2^kFp8PShift to the top of the fp16 range (p' < 2^15, normal down to e = 2^-(14 + kFp8PShift)), with
+            // eref the running maximum of ev: when a page with a larger exponent arrives, acc is multiplied by the
+            // exact power of two beta = 2^(eref_old - eref_new), like alpha for the running softmax maximum.  S6
+            // multiplies the finished accumulator by 2^(eref - 127 - kFp8PShift).  A zero / subnormal scale counts as 0.
+            [[maybe_unused]] float pscale[NT];
+            float beta = 1.f;
+            if constexpr (kFp8) {
+                int ev[NT], emax = eref;
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    ev[k] = (int)((__float_as_uint(v_scale[k]) >> 23) & 0xffu);
+                    emax = max(emax, ev[k]);
+                }
+                if (emax != eref) {
+                    const int sh = 127 + eref - emax;
+                    beta = sh > 0 ? __uint_as_float((uint32_t)sh << 23) : 0.f;
+                    eref = emax;
+                }
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    const int ee = ev[k] - eref + 127 + kFp8PShift;
+                    pscale[k] = (ev[k] == 0 || ee <= 0) ? 0.f
+                              : __uint_as_float((__float_as_uint(v_scale[k]) & 0x807fffffu) | ((uint32_t)ee << 23));
+                }
+            }
 #pragma unroll
             for (int k = 0; k < NT; ++k) {
                 const float e0 = ex2(sv[k][0] - m_new), e1 = ex2(sv[k][1] - m_new);
                 const float e2 = ex2(sv[k][2] - m_new), e3 = ex2(sv[k][3] - m_new);
                 esum += (e0 + e1) + (e2 + e3);
                 if constexpr (kFp8) {
-                    // the page's v_scale rides on p (fp16, 11 significant bits); the normaliser is the unrounded sum
-                    p01[k] = pack_f16x2(e0 * v_scale[k], e1 * v_scale[k]);  // tokens 4q, 4q+1   (k slots 2q, 2q+1)
-                    p23[k] = pack_f16x2(e2 * v_scale[k], e3 * v_scale[k]);  // tokens 4q+2, 4q+3 (k slots 2q+8, 2q+9)
+                    // fp16, 11 significant bits; the normaliser is the unrounded sum
+                    p01[k] = pack_f16x2(e0 * pscale[k], e1 * pscale[k]);  // tokens 4q, 4q+1   (k slots 2q, 2q+1)
+                    p23[k] = pack_f16x2(e2 * pscale[k], e3 * pscale[k]);  // tokens 4q+2, 4q+3 (k slots 2q+8, 2q+9)
                 } else {
                     p01[k] = pack_bf16x2(e0, e1);
                     p23[k] = pack_bf16x2(e2, e3);
@@ -692,10 +724,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             lx_run = lx_run * alpha + esum;
             if constexpr (kFp8) l_run = lx_run;
             else l_run = l_run * alpha + rsum;
-            if (__any_sync(kFull, alpha != 1.f)) {
+            if (__any_sync(kFull, alpha != 1.f) || beta != 1.f) {  // beta is warp-uniform
                 // acc columns are heads 2*qlane, 2*qlane+1: fetch their alphas from those quads
-                const float a_lo = __shfl_sync(kFull, alpha, (2 * qlane) << 2);
-                const float a_hi = __shfl_sync(kFull, alpha, (2 * qlane + 1) << 2);
+                const float a_lo = __shfl_sync(kFull, alpha, (2 * qlane) << 2) * beta;
+                const float a_hi = __shfl_sync(kFull, alpha, (2 * qlane + 1) << 2) * beta;
 #pragma unroll
                 for (int mt = 0; mt < C::kKSteps; ++mt) {
                     acc[mt][0] *= a_lo;
@@ -765,6 +797,14 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         l_run += __shfl_xor_sync(kFull, l_run, 2);
         lx_run += __shfl_xor_sync(kFull, lx_run, 1);
         lx_run += __shfl_xor_sync(kFull, lx_run, 2);
+        if constexpr (kFp8) {  // back to plain units: acc *= 2^(eref - 127 - kFp8PShift) (exact, unless it leaves the fp32 range)
+            const int sh = eref - kFp8PShift;
+            const float unit = sh <= 0 ? 0.f : __uint_as_float((uint32_t)(sh < 254 ? sh : 254) << 23);
+#pragma unroll
+            for (int mt = 0; mt < C::kKSteps; ++mt) {
+                acc[mt][0] *= unit; acc[mt][1] *= unit; acc[mt][2] *= unit; acc[mt][3] *= unit;
+            }
+        }
         {
             float *lo = my_scratch + (2 * qlane) * C::kRowPitch + quad;
             float *hi = lo + C::kRowPitch;

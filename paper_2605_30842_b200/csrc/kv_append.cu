@@ -33,6 +33,8 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
     const int t = seq_lens[b];
     const int page = t / page_size;
     const int slot = t - page * page_size;
+    // a full (or corrupt) row: the next table entry would be another sequence's -- append nothing, bump nothing
+    if (t < 0 || page >= max_pages) return;
     const int64_t pid = block_table[(int64_t)b * max_pages + page];
     const int64_t dst = (pid * page_size + slot) * (int64_t)row_elems;
     const int vecs = row_elems / 8;  // uint4 = 8 bf16
@@ -62,6 +64,7 @@ kv_append_fp8_kernel(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, c
     const int t = seq_lens[b];
     const int page = t / page_size;
     const int slot = t - page * page_size;
+    if (t < 0 || page >= max_pages) return;  // as in kv_append_kernel
     const int64_t pid = block_table[(int64_t)b * max_pages + page];
     const int row_elems = num_kv_heads * head_dim;
     const uint32_t *sk = reinterpret_cast<const uint32_t *>(new_k + (int64_t)b * row_elems);

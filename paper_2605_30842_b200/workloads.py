@@ -304,6 +304,67 @@ def make_batch(seq_lens: Sequence[int], num_q_heads: int, num_kv_heads: int, hea
                        softmax_scale=f32(softmax_scale), name=name, seed=seed)
 
 
+@dataclasses.dataclass
+class PrefillBatch:
+    """Inputs of the paged causal prefill (reading R20): a DecodeBatch's cache plus the ragged chunk queries."""
+
+    q: torch.Tensor            # bf16 [total_q, Hq, D]: the chunks of all sequences back to back
+    q_start: torch.Tensor      # int32 [batch + 1]
+    k_pages: torch.Tensor
+    v_pages: torch.Tensor
+    block_table: torch.Tensor
+    seq_lens: torch.Tensor     # tokens in the cache, the chunk's own included
+    softmax_scale: float
+    name: str = ""
+
+    batch = property(lambda self: self.seq_lens.shape[0])
+    total_q = property(lambda self: self.q.shape[0])
+    num_q_heads = property(lambda self: self.q.shape[1])
+    num_kv_heads = property(lambda self: self.k_pages.shape[2])
+    head_dim = property(lambda self: self.q.shape[2])
+    page_size = property(lambda self: self.k_pages.shape[1])
+
+    def to(self, device) -> "PrefillBatch":
+        mv = lambda t: t.to(device)
+        return dataclasses.replace(self, q=mv(self.q), q_start=mv(self.q_start), k_pages=mv(self.k_pages),
+                                   v_pages=mv(self.v_pages), block_table=mv(self.block_table), seq_lens=mv(self.seq_lens))
+
+    def causal_pairs(self) -> int:
+        """Number of (query, key <= pos) pairs per query head: sum_b sum_i (L_b - n_b + i + 1)."""
+        lens = [int(x) for x in self.seq_lens.cpu()]
+        qs = [int(x) for x in self.q_start.cpu()]
+        tot = 0
+        for b, L in enumerate(lens):
+            n = qs[b + 1] - qs[b]
+            tot += n * (L - n) + n * (n + 1) // 2
+        return tot
+
+    def algorithmic_flops(self) -> int:
+        """4 * D flop per (query, key <= pos) pair and query head: the causal flops, not the dense square."""
+        return 4 * self.head_dim * self.num_q_heads * self.causal_pairs()
+
+
+def make_prefill_batch(seq_lens: Sequence[int], q_lens: Sequence[int], num_q_heads: int, num_kv_heads: int,
+                       head_dim: int, page_size: int, seed: int, device="cpu", *, k_scale: float = 1.0,
+                       poison_unused: bool = False, num_pages: Optional[int] = None,
+                       max_pages_per_seq: Optional[int] = None, softmax_scale: Optional[float] = None,
+                       name: str = "") -> PrefillBatch:
+    """A paged cache of make_batch(seq_lens, ...) plus, per sequence, the queries of its last q_lens[b] tokens
+    (N(0,1) -> bf16 from the same seeded generator family).  q_lens[b] <= seq_lens[b]."""
+    assert len(seq_lens) == len(q_lens) and all(0 <= int(n) <= int(l) for n, l in zip(q_lens, seq_lens))
+    base = make_batch(seq_lens, num_q_heads, num_kv_heads, head_dim, page_size, seed, device, k_scale=k_scale,
+                      poison_unused=poison_unused, num_pages=num_pages, max_pages_per_seq=max_pages_per_seq,
+                      softmax_scale=softmax_scale)
+    device = torch.device(device)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(seed + 7919)
+    total_q = int(sum(int(n) for n in q_lens))
+    q = _randn_bf16((total_q, num_q_heads, head_dim), gen, device)
+    q_start = torch.tensor([0] + list(np.cumsum([int(n) for n in q_lens])), dtype=torch.int32, device=device)
+    return PrefillBatch(q=q, q_start=q_start, k_pages=base.k_pages, v_pages=base.v_pages, block_table=base.block_table,
+                        seq_lens=base.seq_lens, softmax_scale=base.softmax_scale, name=name)
+
+
 # ---------------------------------------------------------------------------
 # BASELINE.json configs (C1..C5), concrete per SURVEY.md §8(d)
 # ---------------------------------------------------------------------------
