@@ -843,28 +843,28 @@ def run_pipeline(args) -> int:
                "agent_us_alone": e2.elapsed_time(e3) * 1e3 / reps, "sm_partition": []}
         # SM partitioning: both kernels are persistent one-CTA-per-SM grids, so two full grids time-share the GPU
         # and a short agent step queues behind a long memory step.  Giving each stream a share of the SMs
-        # (comem_set_grid_ctas is read at enqueue time) lets both grids be resident at once.
+        # (per-call comem_launch_opts.grid_ctas, programmatic launch off so that a stream's next kernel does not park
+        # on the other's SMs) lets both grids be resident at once.  The split is the library's policy
+        # (comem_sm_partition: proportional to the bytes each batch streams); sms/4 and sms/2 are shown beside it.
         sms = comem.comem_grid_ctas(128)
-        try:
-            comem.comem_set_programmatic_launch(False)   # else stream B's next kernel parks on the SMs left free
-            for agent_sms in (sms // 4, sms // 2):
-                comem.comem_set_grid_ctas(sms - agent_sms)
-                for _ in range(4 * reps):
-                    launch(memory, lens_m, out_m, ws_m, sb)
-                comem.comem_set_grid_ctas(agent_sms)
-                p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                p0.record(sa)
-                for _ in range(reps):
-                    launch(agent, lens_a, out_a, ws_a, sa)
-                p1.record(sa)
-                m0 = torch.cuda.Event(enable_timing=True)
-                m0.record(sb)
-                torch.cuda.synchronize()
-                rec["sm_partition"].append({"agent_sms": agent_sms, "memory_sms": sms - agent_sms,
-                                            "agent_us": p0.elapsed_time(p1) * 1e3 / reps})
-        finally:
-            comem.comem_set_grid_ctas(0)
-            comem.comem_set_programmatic_launch(True)
+        by_a = ctx_comem[t + 1] * CONC * agent.num_kv_heads * agent.head_dim * 4
+        by_m = mem_in[t] * CONC * memory.num_kv_heads * memory.head_dim * 4
+        pol_a, _ = comem.comem_sm_partition(by_a, by_m, sms)
+        for agent_sms, how in ((pol_a, "comem_sm_partition"), (sms // 4, "fixed"), (sms // 2, "fixed")):
+            for _ in range(4 * reps):
+                comem.comem_decode_attn_async(memory.q, memory.k_pages, memory.v_pages, memory.block_table, lens_m,
+                                              memory.softmax_scale, out_m, ws_m, stream=sb,
+                                              grid_ctas=sms - agent_sms, programmatic_launch=False)
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(sa)
+            for _ in range(reps):
+                comem.comem_decode_attn_async(agent.q, agent.k_pages, agent.v_pages, agent.block_table, lens_a,
+                                              agent.softmax_scale, out_a, ws_a, stream=sa,
+                                              grid_ctas=agent_sms, programmatic_launch=False)
+            p1.record(sa)
+            torch.cuda.synchronize()
+            rec["sm_partition"].append({"agent_sms": agent_sms, "memory_sms": sms - agent_sms, "split": how,
+                                        "agent_us": p0.elapsed_time(p1) * 1e3 / reps})
         overlap.append(rec)
     print(json.dumps({
         "extra": "k-step-off pipeline (Algorithm 1) driven from comem_kstep_plan; eq. 5 vs measured",

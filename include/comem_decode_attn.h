@@ -59,6 +59,26 @@ enum {
 #define COMEM_MAX_BATCH 4096
 
 /*
+ * Per-call launch options of the attention entry points (last argument of every *_async attention call; NULL = the
+ * process defaults below).  They change WHERE and HOW the kernel is launched, never its result bits' validity: the
+ * split-KV schedule is a function of (seq_lens, num_kv_heads, grid_ctas), so a given grid_ctas reproduces its own
+ * bits exactly and any value is within the parity tolerance.
+ *   grid_ctas            > 0: size of this call's persistent decode grid (its share of the SMs: the agent batch and
+ *                        the memory-model batch of the k-step-off pipeline, run side by side when their
+ *                        grids sum to the SM count; comem_sm_partition picks the split).  0: the default
+ *                        (comem_set_grid_ctas' value if set, else one CTA per SM).  Ignored by the prefill kernel.
+ *   programmatic_launch  1 / 0: launch with / without programmatic stream serialization (the next launch of the
+ *                        stream starts its prologue on SMs the previous one has released: shortest back-to-back steps,
+ *                        but a stream's NEXT kernel then parks on every free SM; use 0 with an SM partition).
+ *                        -1: the default (comem_set_programmatic_launch's value, initially 1).
+ * Two host threads may enqueue concurrently with different options; nothing here is process state.
+ */
+typedef struct {
+    int grid_ctas;
+    int programmatic_launch;
+} comem_launch_opts;
+
+/*
  * comem_decode_attn_async — enqueue one decode-attention step on `cuda_stream`.
  *
  * Enqueue-only: no host synchronisation, no device->host copy, no allocation;
@@ -93,7 +113,7 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                             int num_q_heads, int num_kv_heads, int head_dim, int page_size,
                             float softmax_scale, void *out, int batch, int max_pages_per_seq,
                             int64_t num_pages, float *lse_out, void *workspace,
-                            size_t workspace_bytes, void *cuda_stream);
+                            size_t workspace_bytes, void *cuda_stream, const comem_launch_opts *opts);
 
 /*
  * comem_workspace_init_async — zero the arrival counters at the head of `workspace`
@@ -121,7 +141,7 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
                                    float softmax_scale, void *out, int batch,
                                    int max_pages_per_seq, int64_t num_pages, float *lse_out,
                                    void *workspace, size_t workspace_bytes, void *cuda_stream,
-                                   int phases);
+                                   int phases, const comem_launch_opts *opts);
 
 /*
  * comem_decode_attn_window_async — the byte-reducing variant the paper calls orthogonal (sliding
@@ -138,7 +158,7 @@ int comem_decode_attn_window_async(const void *q, const void *k_pages, const voi
                                    float softmax_scale, void *out, int batch,
                                    int max_pages_per_seq, int64_t num_pages, float *lse_out,
                                    void *workspace, size_t workspace_bytes, void *cuda_stream,
-                                   int window, int sink_tokens);
+                                   int window, int sink_tokens, const comem_launch_opts *opts);
 
 /*
  * comem_decode_attn_fp8_async — the same step over an FP8 KV cache, the other byte-reducing variant
@@ -167,7 +187,7 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 float softmax_scale, void *out, int batch, int max_pages_per_seq,
                                 int64_t num_pages, float *lse_out, void *workspace,
                                 size_t workspace_bytes, void *cuda_stream, int window, int sink_tokens,
-                                int kv_layout);
+                                int kv_layout, const comem_launch_opts *opts);
 
 /*
  * comem_kv_append_fp8_async — comem_kv_append_async for the FP8 cache of comem_decode_attn_fp8_async (P:L61 for
@@ -249,7 +269,7 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
                              const int32_t *block_table, const int32_t *seq_lens, const int32_t *q_start,
                              int num_q_heads, int num_kv_heads, int head_dim, int page_size,
                              float softmax_scale, void *out, int batch, int total_q, int max_pages_per_seq,
-                             int64_t num_pages, float *lse_out, void *cuda_stream);
+                             int64_t num_pages, float *lse_out, void *cuda_stream, const comem_launch_opts *opts);
 
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
@@ -329,21 +349,25 @@ int comem_validate_inputs(const int32_t *block_table, const int32_t *seq_lens, i
                           int max_pages_per_seq, int page_size, int64_t num_pages, void *workspace,
                           size_t workspace_bytes, void *cuda_stream);
 
-/* Persistent-grid size (CTAs) the split kernel uses on the current device, or a
- * negative COMEM_ERR_* value.  comem_set_grid_ctas(n > 0) overrides it for later
- * calls from this process (n <= 0 restores the default); used to give each of two
- * concurrently running batches a share of the SMs. */
+/* Persistent-grid size (CTAs) the split kernel uses on the current device, or a negative COMEM_ERR_* value. */
 int comem_grid_ctas(int head_dim);
-int comem_set_grid_ctas(int n);
 
 /*
- * comem_set_programmatic_launch — process-wide launch policy, read at enqueue time (default 1).  With 1 the
- * attention kernel is launched with programmatic stream serialization: the next launch on the same stream
- * starts its prologue on SMs the previous one has released, which shortens back-to-back steps (config 2) but
- * also means a stream's NEXT kernel occupies every free SM while it waits.  Set 0 while two streams share the
- * GPU by SM partition (comem_set_grid_ctas per enqueue: agent and memory-model grids that sum to the SM
- * count), so that the other stream's kernel can be resident at the same time.
+ * comem_sm_partition — launch policy for two batches that share one GPU (the agent's decode step and the memory
+ * model's, P:L130-176 / P:L245): split num_sms CTAs in proportion to the bytes each batch has to
+ * stream, so that both persistent grids are resident together and finish together (the path is HBM-bound and an SM
+ * pulls a fixed rate); each side gets at least min_ctas.  Pass the results as comem_launch_opts.grid_ctas with
+ * programmatic_launch = 0.  Host arithmetic only.  *ctas_a + *ctas_b == num_sms.
  */
+int comem_sm_partition(double bytes_a, double bytes_b, int num_sms, int min_ctas, int *ctas_a, int *ctas_b);
+
+/*
+ * DEPRECATED process-wide defaults, read at enqueue time by calls whose comem_launch_opts is NULL (or leaves the
+ * field at its "default" value).  Two threads that need different settings must pass comem_launch_opts instead.
+ * comem_set_grid_ctas(n > 0) overrides the default grid (n <= 0 restores one CTA per SM);
+ * comem_set_programmatic_launch(0 / 1) switches programmatic stream serialization off / on (default 1).
+ */
+int comem_set_grid_ctas(int n);
 int comem_set_programmatic_launch(int enabled);
 
 const char *comem_status_string(int status);

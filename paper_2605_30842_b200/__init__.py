@@ -33,6 +33,8 @@ from .binding import (  # noqa: F401
     comem_kv_append_fp8_async,
     comem_schedule_host,
     comem_set_grid_ctas,
+    comem_sm_partition,
+    LaunchOpts,
     comem_set_programmatic_launch,
     comem_validate_inputs,
     comem_status_string,

@@ -47,19 +47,19 @@ def load_library():
     c = ctypes
     vp, i32, i64, f32, sz = c.c_void_p, c.c_int, c.c_int64, c.c_float, c.c_size_t
     lib.comem_decode_attn_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
-                                            i64, vp, vp, sz, vp]
+                                            i64, vp, vp, sz, vp, vp]
     lib.comem_decode_attn_async.restype = i32
     lib.comem_decode_attn_phases_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
-                                                   i32, i64, vp, vp, sz, vp, i32]
+                                                   i32, i64, vp, vp, sz, vp, i32, vp]
     lib.comem_decode_attn_phases_async.restype = i32
     lib.comem_decode_attn_window_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
-                                                   i32, i64, vp, vp, sz, vp, i32, i32]
+                                                   i32, i64, vp, vp, sz, vp, i32, i32, vp]
     lib.comem_decode_attn_window_async.restype = i32
     lib.comem_decode_attn_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
-                                                i32, i64, vp, vp, sz, vp, i32, i32, i32]
+                                                i32, i64, vp, vp, sz, vp, i32, i32, i32, vp]
     lib.comem_decode_attn_fp8_async.restype = i32
     lib.comem_prefill_attn_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i32,
-                                             i64, vp, vp]
+                                             i64, vp, vp, vp]
     lib.comem_prefill_attn_async.restype = i32
     lib.comem_decode_attn.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i64,
                                       vp, vp, sz]
@@ -92,6 +92,8 @@ def load_library():
     lib.comem_schedule_host.restype = i32
     lib.comem_grid_ctas.argtypes = [i32]
     lib.comem_grid_ctas.restype = i32
+    lib.comem_sm_partition.argtypes = [f64, f64, i32, i32, vp, vp]
+    lib.comem_sm_partition.restype = i32
     lib.comem_set_grid_ctas.argtypes = [i32]
     lib.comem_set_grid_ctas.restype = i32
     lib.comem_set_programmatic_launch.argtypes = [i32]
@@ -116,6 +118,30 @@ def comem_grid_ctas(head_dim: int) -> int:
     if g < 0:
         raise ComemError(-g, "comem_grid_ctas")
     return g
+
+
+class LaunchOpts(ctypes.Structure):
+    """comem_launch_opts: per-call grid size (0 = default) and programmatic launch (-1 = default)."""
+    _fields_ = [("grid_ctas", ctypes.c_int), ("programmatic_launch", ctypes.c_int)]
+
+
+def _opts(grid_ctas, programmatic_launch):
+    """None when both are defaults, else a pointer to a comem_launch_opts (the library reads it during the call)."""
+    if grid_ctas is None and programmatic_launch is None:
+        return None
+    o = LaunchOpts(int(grid_ctas or 0), -1 if programmatic_launch is None else (1 if programmatic_launch else 0))
+    return ctypes.cast(ctypes.pointer(o), ctypes.c_void_p)
+
+
+def comem_sm_partition(bytes_a: float, bytes_b: float, num_sms: int, min_ctas: int = 8):
+    """(ctas_a, ctas_b): the library's SM split for two batches sharing the GPU, proportional to their bytes."""
+    a, b = ctypes.c_int(0), ctypes.c_int(0)
+    st = load_library().comem_sm_partition(float(bytes_a), float(bytes_b), int(num_sms), int(min_ctas),
+                                           ctypes.cast(ctypes.byref(a), ctypes.c_void_p),
+                                           ctypes.cast(ctypes.byref(b), ctypes.c_void_p))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_sm_partition")
+    return a.value, b.value
 
 
 def comem_set_grid_ctas(n: int) -> None:
@@ -240,7 +266,8 @@ COMEM_PHASE_COMBINE = 2
 
 def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
                                    workspace, lse_out=None, stream=None,
-                                   phases: int = COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) -> None:
+                                   phases: int = COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
+                                   grid_ctas=None, programmatic_launch=None) -> None:
     """Enqueue the selected kernels of one decode-attention step on ``stream``; returns at once."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -248,13 +275,14 @@ def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, s
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream), int(phases))
+        workspace.numel() * workspace.element_size(), _stream(stream), int(phases),
+        _opts(grid_ctas, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_phases_async")
 
 
 def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
-                            workspace, lse_out=None, stream=None) -> None:
+                            workspace, lse_out=None, stream=None, grid_ctas=None, programmatic_launch=None) -> None:
     """Enqueue one decode-attention step (1 fused kernel launch) on ``stream``; returns at once."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -262,13 +290,14 @@ def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream))
+        workspace.numel() * workspace.element_size(), _stream(stream), _opts(grid_ctas, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_async")
 
 
 def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
-                                   workspace, window: int, sink_tokens: int, lse_out=None, stream=None) -> None:
+                                   workspace, window: int, sink_tokens: int, lse_out=None, stream=None,
+                                   grid_ctas=None, programmatic_launch=None) -> None:
     """Sliding-window + attention-sink decode attention (one fused launch on ``stream``)."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -276,14 +305,16 @@ def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, s
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens))
+        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens),
+        _opts(grid_ctas, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_window_async")
 
 
 def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
                                 softmax_scale: float, out, workspace, window: int = 0, sink_tokens: int = 0,
-                                lse_out=None, stream=None, kv_layout: str = "NHD") -> None:
+                                lse_out=None, stream=None, kv_layout: str = "NHD", grid_ctas=None,
+                                programmatic_launch=None) -> None:
     """Decode attention over an FP8 (E4M3 bytes + fp32 page scales) KV cache; one fused launch.
     kv_layout "NHD": pools [P, page_size, Hkv, D]; "HND": pools [P, Hkv, page_size, D]."""
     assert kv_layout in ("NHD", "HND")
@@ -303,7 +334,8 @@ def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_tab
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(k_scale), _ptr(v_scale), _ptr(block_table), _ptr(seq_lens),
         q.shape[1], hkv, q.shape[2], page_size, ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens), 1 if hnd else 0)
+        workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens), 1 if hnd else 0,
+        _opts(grid_ctas, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_fp8_async")
 
@@ -327,7 +359,7 @@ def comem_kv_append_fp8_async(k_pages, v_pages, k_scale, v_scale, block_table, s
 
 
 def comem_prefill_attn_async(q, k_pages, v_pages, block_table, seq_lens, q_start, softmax_scale: float, out,
-                             lse_out=None, stream=None) -> None:
+                             lse_out=None, stream=None, programmatic_launch=None) -> None:
     """Causal prefill attention of each sequence's last q_start[b+1] - q_start[b] tokens over the paged cache
     (one tcgen05 kernel on ``stream``).  q, out: bf16 [total_q, Hq, D]; q_start: int32 [batch + 1] on the device."""
     assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.dim() == 3
@@ -343,7 +375,8 @@ def comem_prefill_attn_async(q, k_pages, v_pages, block_table, seq_lens, q_start
     st = load_library().comem_prefill_attn_async(
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), _ptr(q_start), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
-        block_table.shape[0], q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _stream(stream))
+        block_table.shape[0], q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _stream(stream),
+        _opts(None, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_prefill_attn_async")
 

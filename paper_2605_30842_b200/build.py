@@ -39,18 +39,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-TRACE_LIB = os.path.join(HERE, "libcomem_decode_trace.so")
-
-
-def build_trace() -> str:
-    """Development variant with -DCOMEM_TRACE: the split kernel stamps %globaltimer at its stage
-    boundaries into a buffer set with comem_set_trace (see stage_trace.py).  Never loaded by the
-    binding, the tests or bench.py."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    subprocess.run([nvcc] + NVCC_FLAGS + ["-DCOMEM_TRACE", "-o", TRACE_LIB] +
-                   [os.path.join(CSRC, f) for f in SOURCES], check=True)
-    return TRACE_LIB
-
-
 if __name__ == "__main__":
-    print(build_trace() if "--trace" in sys.argv else build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

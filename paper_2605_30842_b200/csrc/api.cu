@@ -206,14 +206,22 @@ int make_q_tensor_map(const void *q, int64_t total_q, int hq, int d, int group, 
     return r == CUDA_SUCCESS ? COMEM_OK : COMEM_ERR_CUDA;
 }
 
-int grid_for(int head_dim, int *grid)
+constexpr int kMaxDevices = 64;
+
+// Persistent-grid size: the call's own option, else the process default override, else one CTA per SM of the
+// CURRENT device (cached per device ordinal).
+int grid_for(int head_dim, int *grid, const comem_launch_opts *opts = nullptr)
 {
+    (void)head_dim;
     static std::mutex mu;
-    static int cached[2] = {0, 0};
-    const int ov = g_grid_override.load();
+    static int cached[kMaxDevices] = {};
+    const int ov = (opts && opts->grid_ctas > 0) ? opts->grid_ctas : g_grid_override.load();
     if (ov > 0) { *grid = ov < kMaxGridCtas ? ov : kMaxGridCtas; return COMEM_OK; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) { cudaGetLastError(); return COMEM_ERR_CUDA; }
     std::lock_guard<std::mutex> lock(mu);
-    int &c = cached[head_dim == 128 ? 1 : 0];
+    int uncached = 0;
+    int &c = dev < kMaxDevices ? cached[dev] : uncached;
     if (c == 0) {
         int g = 0;
         if (split_default_grid(head_dim, &g) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
@@ -221,6 +229,13 @@ int grid_for(int head_dim, int *grid)
     }
     *grid = c;
     return COMEM_OK;
+}
+
+// programmatic stream serialization for this call: its own option (0 / 1), else the process default
+bool pdl_for(const comem_launch_opts *opts)
+{
+    if (opts && opts->programmatic_launch >= 0) return opts->programmatic_launch != 0;
+    return g_pdl.load() != 0;
 }
 
 #ifdef COMEM_TRACE
@@ -337,6 +352,24 @@ int comem_set_programmatic_launch(int enabled)
     return COMEM_OK;
 }
 
+int comem_sm_partition(double bytes_a, double bytes_b, int num_sms, int min_ctas, int *ctas_a, int *ctas_b)
+{
+    if (!ctas_a || !ctas_b || num_sms < 2 || !(bytes_a >= 0.0) || !(bytes_b >= 0.0) || !std::isfinite(bytes_a) ||
+        !std::isfinite(bytes_b))
+        return COMEM_ERR_INVALID_ARG;
+    if (min_ctas < 1) min_ctas = 1;
+    if (2 * min_ctas > num_sms) min_ctas = num_sms / 2;
+    // shares proportional to the bytes each batch must stream (the path is HBM-bound and an SM pulls a fixed
+    // rate), so both grids finish together; round to nearest, then keep at least min_ctas on each side
+    const double tot = bytes_a + bytes_b;
+    int a = tot > 0.0 ? (int)(bytes_a / tot * num_sms + 0.5) : num_sms / 2;
+    if (a < min_ctas) a = min_ctas;
+    if (a > num_sms - min_ctas) a = num_sms - min_ctas;
+    *ctas_a = a;
+    *ctas_b = num_sms - a;
+    return COMEM_OK;
+}
+
 int comem_grid_ctas(int head_dim)
 {
     if (head_dim != 64 && head_dim != 128) return -COMEM_ERR_UNSUPPORTED;
@@ -380,8 +413,8 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
                             void *out, int batch, int max_pages_per_seq, int64_t num_pages,
                             float *lse_out, void *workspace, size_t workspace_bytes,
                             void *cuda_stream, int phases, int window, int sink_tokens,
-                            const float *k_scale = nullptr, const float *v_scale = nullptr, bool kv_fp8 = false,
-                            int kv_layout = COMEM_KV_LAYOUT_NHD)
+                            const comem_launch_opts *opts, const float *k_scale = nullptr,
+                            const float *v_scale = nullptr, bool kv_fp8 = false, int kv_layout = COMEM_KV_LAYOUT_NHD)
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
     if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
@@ -408,7 +441,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.k_scale = kv_fp8 ? k_scale : nullptr;
     p.v_scale = kv_fp8 ? v_scale : nullptr;
     p.kv_hnd = hnd;
-    p.no_pdl = g_pdl.load() ? 0 : 1;
+    p.no_pdl = pdl_for(opts) ? 0 : 1;
     p.q = static_cast<const __nv_bfloat16 *>(q);
     p.block_table = block_table;
     p.seq_lens = seq_lens;
@@ -433,7 +466,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.scale_log2 = softmax_scale * kLog2e;
     p.window = window > 0 ? window : 0;
     p.sinks = window > 0 ? sink_tokens : 0;
-    if ((st = grid_for(head_dim, &p.grid_ctas)) != COMEM_OK) return st;
+    if ((st = grid_for(head_dim, &p.grid_ctas, opts)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8) != cudaSuccess) {
@@ -452,11 +485,11 @@ int comem_decode_attn_phases_async(const void *q, const void *k_pages, const voi
                                    int num_kv_heads, int head_dim, int page_size, float softmax_scale,
                                    void *out, int batch, int max_pages_per_seq, int64_t num_pages,
                                    float *lse_out, void *workspace, size_t workspace_bytes,
-                                   void *cuda_stream, int phases)
+                                   void *cuda_stream, int phases, const comem_launch_opts *opts)
 {
     return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
                             page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
-                            workspace, workspace_bytes, cuda_stream, phases, 0, 0);
+                            workspace, workspace_bytes, cuda_stream, phases, 0, 0, opts);
 }
 
 int comem_decode_attn_window_async(const void *q, const void *k_pages, const void *v_pages,
@@ -464,12 +497,12 @@ int comem_decode_attn_window_async(const void *q, const void *k_pages, const voi
                                    int num_kv_heads, int head_dim, int page_size, float softmax_scale,
                                    void *out, int batch, int max_pages_per_seq, int64_t num_pages,
                                    float *lse_out, void *workspace, size_t workspace_bytes,
-                                   void *cuda_stream, int window, int sink_tokens)
+                                   void *cuda_stream, int window, int sink_tokens, const comem_launch_opts *opts)
 {
     return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
                             page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
                             workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
-                            window, sink_tokens);
+                            window, sink_tokens, opts);
 }
 
 int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *v_pages, const float *k_scale,
@@ -477,30 +510,33 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 int num_q_heads, int num_kv_heads, int head_dim, int page_size,
                                 float softmax_scale, void *out, int batch, int max_pages_per_seq,
                                 int64_t num_pages, float *lse_out, void *workspace, size_t workspace_bytes,
-                                void *cuda_stream, int window, int sink_tokens, int kv_layout)
+                                void *cuda_stream, int window, int sink_tokens, int kv_layout,
+                                const comem_launch_opts *opts)
 {
     return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim,
                             page_size, softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out,
                             workspace, workspace_bytes, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
-                            window, sink_tokens, k_scale, v_scale, true, kv_layout);
+                            window, sink_tokens, opts, k_scale, v_scale, true, kv_layout);
 }
 
 int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pages,
                             const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
                             int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
                             int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
-                            void *workspace, size_t workspace_bytes, void *cuda_stream)
+                            void *workspace, size_t workspace_bytes, void *cuda_stream,
+                            const comem_launch_opts *opts)
 {
     return comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads,
                                           head_dim, page_size, softmax_scale, out, batch, max_pages_per_seq,
                                           num_pages, lse_out, workspace, workspace_bytes, cuda_stream,
-                                          COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
+                                          COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE, opts);
 }
 
 int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,
                              const int32_t *seq_lens, const int32_t *q_start, int num_q_heads, int num_kv_heads,
                              int head_dim, int page_size, float softmax_scale, void *out, int batch, int total_q,
-                             int max_pages_per_seq, int64_t num_pages, float *lse_out, void *cuda_stream)
+                             int max_pages_per_seq, int64_t num_pages, float *lse_out, void *cuda_stream,
+                             const comem_launch_opts *opts)
 {
     if (!q || !k_pages || !v_pages || !block_table || !seq_lens || !q_start || !out) return COMEM_ERR_INVALID_ARG;
     if (batch <= 0 || total_q <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || max_pages_per_seq <= 0 || num_pages <= 0)
@@ -543,7 +579,7 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
     const int64_t items = ((int64_t)total_q / pair_pos + (batch < total_q ? batch : total_q)) * num_kv_heads;
     if (items >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
     if (launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, (int)items, static_cast<cudaStream_t>(cuda_stream),
-                            g_pdl.load() != 0) != cudaSuccess) {
+                            pdl_for(opts)) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }
@@ -563,7 +599,7 @@ int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages, c
     const int st = comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, num_q_heads,
                                            num_kv_heads, head_dim, page_size, softmax_scale, out, batch,
                                            max_pages_per_seq, num_pages, lse_out, workspace,
-                                           workspace_bytes, nullptr);
+                                           workspace_bytes, nullptr, nullptr);
     if (st != COMEM_OK) return st;
     if (cudaStreamSynchronize(nullptr) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
     return COMEM_OK;
@@ -664,7 +700,7 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
             st = comem_decode_attn_async(ws + wl.q, k_pages, v_pages, block_table, seq_lens, num_q_heads,
                                          num_kv_heads, head_dim, page_size, softmax_scale, dout, batch,
                                          max_pages_per_seq, num_pages, static_cast<float *>(dlse), workspace,
-                                         workspace_bytes, cuda_stream);
+                                         workspace_bytes, cuda_stream, nullptr);
             if (st != COMEM_OK) return st;
             if (cudaStreamSynchronize(stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
             return COMEM_OK;
@@ -684,7 +720,7 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
     st = comem_decode_attn_async(ws + wl.q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads,
                                  head_dim, page_size, softmax_scale, ws + wl.out, batch, max_pages_per_seq,
                                  num_pages, lse_host ? reinterpret_cast<float *>(ws + wl.lse) : nullptr,
-                                 workspace, workspace_bytes, cuda_stream);
+                                 workspace, workspace_bytes, cuda_stream, nullptr);
     if (st != COMEM_OK) return st;
     ok = cudaMemcpyAsync(out_host, ws + wl.out, q_bytes, cudaMemcpyDeviceToHost, stream) == cudaSuccess;
     if (ok && lse_host)

@@ -111,16 +111,15 @@ cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t str
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    static const cudaError_t cfg128 = cudaFuncSetAttribute(combine_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         MergeCfg<128>::kStageBytes);
-    static const cudaError_t cfg64 = cudaFuncSetAttribute(combine_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                        MergeCfg<64>::kStageBytes);
+    static PerDeviceOnce once128, once64;
     if (head_dim == 128) {
-        if (cfg128 != cudaSuccess) return cfg128;
+        const cudaError_t e = set_max_smem_once(combine_kernel<128>, MergeCfg<128>::kStageBytes, once128);
+        if (e != cudaSuccess) return e;
         cfg.dynamicSmemBytes = MergeCfg<128>::kStageBytes;
         return cudaLaunchKernelEx(&cfg, combine_kernel<128>, p);
     }
-    if (cfg64 != cudaSuccess) return cfg64;
+    const cudaError_t e = set_max_smem_once(combine_kernel<64>, MergeCfg<64>::kStageBytes, once64);
+    if (e != cudaSuccess) return e;
     cfg.dynamicSmemBytes = MergeCfg<64>::kStageBytes;
     return cudaLaunchKernelEx(&cfg, combine_kernel<64>, p);
 }

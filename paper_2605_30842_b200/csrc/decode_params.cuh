@@ -1,5 +1,6 @@
 // decode_params.cuh — kernel argument block shared by the split and combine launchers.
 #pragma once
+#include <atomic>
 #include <cstdint>
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -37,6 +38,25 @@ struct DecodeParams {
     int no_pdl;                  // host-side only: launch without programmatic stream serialization (comem_set_programmatic_launch)
     int kv_hnd;                  // FP8 cache only: pools laid out [P][Hkv][ps][D] (a tile is 2 KiB contiguous) instead of [P][ps][Hkv][D]
 };
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-DEVICE setting: remember, per kernel instantiation,
+// the device ordinals it has been applied on (a process may drive the agent model on one GPU and the memory
+// model on another).
+struct PerDeviceOnce {
+    std::atomic<unsigned char> done[64];
+};
+template <typename Kernel>
+inline cudaError_t set_max_smem_once(Kernel kernel, int bytes, PerDeviceOnce &once)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && once.done[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess && tracked) once.done[dev].store(1, std::memory_order_release);
+    return e;
+}
 
 // launchers (defined in decode_split.cu / combine.cu / kv_append.cu)
 // kv_fp8: the pools hold E4M3 bytes and p.k_scale / p.v_scale are set

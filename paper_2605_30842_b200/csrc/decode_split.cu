@@ -899,10 +899,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 template <int D, bool kFp8>
 cudaError_t configure_once()
 {
-    static cudaError_t status = cudaFuncSetAttribute(decode_split_kernel<D, kFp8>,
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                     (int)smem_bytes_for<D, kFp8>(kMaxBatch));
-    return status;
+    static PerDeviceOnce once;
+    return set_max_smem_once(decode_split_kernel<D, kFp8>, (int)smem_bytes_for<D, kFp8>(kMaxBatch), once);
 }
 
 }  // namespace

@@ -402,9 +402,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 template <int D>
 cudaError_t configure_prefill()
 {
-    static cudaError_t status = cudaFuncSetAttribute(prefill_attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                     PfCfg<D>::kSmemBytes);
-    return status;
+    static PerDeviceOnce once;
+    return set_max_smem_once(prefill_attn_kernel<D>, PfCfg<D>::kSmemBytes, once);
 }
 
 template <int D>

@@ -365,6 +365,34 @@ def make_prefill_batch(seq_lens: Sequence[int], q_lens: Sequence[int], num_q_hea
                         seq_lens=base.seq_lens, softmax_scale=base.softmax_scale, name=name)
 
 
+def sink_batch(seq_len: int, num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int, seed: int,
+               device="cpu", *, sink_nats: float = 13.0, v_mean: float = 0.3, v_std: float = 0.1,
+               k_scale: float = 0.05) -> DecodeBatch:
+    """Stress recipe for low-precision P (input preparation only): one sequence whose token 0 is an attention sink
+    `sink_nats` above a flat tail (k ~ k_scale * N(0,1)), values with a NONZERO mean (v ~ N(v_mean, v_std^2), so the
+    tail's mass matters to the output and an FP8 page scale amax/448 is ~2e-3).  The G heads of a group get the same
+    query, so every head sees the same sink logit: k_0 = sink_nats / (scale * |q|^2) * q."""
+    b = make_batch([seq_len], num_q_heads, num_kv_heads, head_dim, page_size, seed, device, k_scale=k_scale,
+                   poison_unused=True)
+    g = num_q_heads // num_kv_heads
+    q = b.q.view(1, num_kv_heads, g, head_dim)
+    q[:] = q[:, :, :1, :]
+    gen = torch.Generator(device=b.q.device)
+    gen.manual_seed(seed + 1)
+    npg = pages_needed(seq_len, page_size)
+    ids = b.block_table[0, :npg].long()
+    v = torch.randn((npg, page_size, num_kv_heads, head_dim), generator=gen, device=b.q.device) * v_std + v_mean
+    v = v.to(torch.bfloat16)
+    tail = npg * page_size - seq_len
+    if tail:
+        v.view(-1, num_kv_heads, head_dim)[seq_len:] = float("nan")
+    b.v_pages[ids] = v
+    qf = b.q[0].float().view(num_kv_heads, g, head_dim)[:, 0, :]
+    k0 = qf * (sink_nats / (b.softmax_scale * (qf * qf).sum(-1, keepdim=True)))
+    b.k_pages[int(b.block_table[0, 0]), 0] = k0.to(torch.bfloat16)
+    return b
+
+
 # ---------------------------------------------------------------------------
 # BASELINE.json configs (C1..C5), concrete per SURVEY.md §8(d)
 # ---------------------------------------------------------------------------

@@ -59,7 +59,7 @@ def _call(lib, **over):
     return lib.comem_decode_attn_async(a["q"], a["k"], a["v"], a["bt"], a["sl"], a["hq"], a["hkv"],
                                        a["d"], a["ps"], ctypes.c_float(a["scale"]), a["out"],
                                        a["batch"], a["maxp"], a["npages"], a["lse"], a["ws"], a["wsb"],
-                                       a["stream"])
+                                       a["stream"], None)
 
 
 def test_argument_validation(lib):
@@ -138,7 +138,7 @@ def test_fp8_entry_point_validates_before_any_launch(lib):
 
     def call(ks=d, vs=d, head_dim=128, layout=0, sinks=0):
         return lib.comem_decode_attn_fp8_async(d, d, d, ks, vs, d, d, 64, 8, head_dim, 16, ctypes.c_float(0.088), d, 1,
-                                               2048, 4096, None, d, 1 << 30, None, 0, sinks, layout)
+                                               2048, 4096, None, d, 1 << 30, None, 0, sinks, layout, None)
 
     assert call(ks=None) == comem.COMEM_ERR_INVALID_ARG
     assert call(vs=None) == comem.COMEM_ERR_INVALID_ARG

@@ -81,6 +81,30 @@ def test_fp8_long_ragged_grids_and_permutation(oracle):
         comem.comem_set_grid_ctas(0)
 
 
+@pytest.mark.parametrize("nats,v_mean", [(12.0, 0.3), (13.0, 0.3), (14.0, 0.15), (13.0, 0.05)])
+def test_fp8_sink_token_small_v_scale(oracle, nats, v_mean):
+    """One sink token 12-14 nats above a flat 32K tail, V with a nonzero mean, page scales amax/448 <= 2e-3: the
+    tail's p * v_scale would fall into the fp16 subnormals (below 2^-14) and drop out of the numerator while the
+    normaliser still counts it.  The kernel keeps only the scale's mantissa (times a power of two relative to the
+    running largest exponent) on p and the power of two on the accumulator."""
+    f = W.quantize_batch_fp8(W.sink_batch(32768, 32, 8, 128, 16, seed=530, device=DEV, sink_nats=nats, v_mean=v_mean,
+                                          v_std=v_mean / 3))
+    assert float(f.v_scale[f.block_table[0, :2048].long()].max()) <= 2e-3
+    check(oracle, f, f"sink {nats} nats, v mean {v_mean}")
+    check(oracle, W.to_hnd(f), f"sink {nats} nats, v mean {v_mean}, HND")
+
+
+def test_fp8_mixed_page_scales(oracle):
+    """Page scales spread over 2^-12 .. 2^6 within one sequence (the running reference exponent moves up and down)."""
+    b = W.make_batch([3000, 777], 32, 8, 128, 16, seed=531, device=DEV, poison_unused=True)
+    gen = torch.Generator(device=DEV)
+    gen.manual_seed(5)
+    expo = torch.randint(-12, 7, (b.v_pages.shape[0], 1, 8, 1), generator=gen, device=DEV).float()
+    b.v_pages.copy_((b.v_pages.float() * torch.exp2(expo)).to(torch.bfloat16))
+    f = W.quantize_batch_fp8(b)
+    check(oracle, f, "mixed page scales")
+
+
 def test_fp8_single_long_sequence_aligned_schedule(oracle):
     """one 32K sequence x 8 kv heads: the segment-aligned schedule (18-19 CTAs per head) and the fused merge"""
     f = fp8_batch([32768], 64, 8, 16, seed=522, k_scale=0.5)
@@ -209,7 +233,7 @@ def test_fp8_rejects_unknown_layout_and_null_scales():
     p = lambda t: ctypes.c_void_p(t.data_ptr())
     args = lambda ks, layout: (p(b.q), p(k8), p(k8), ks, p(sc), p(b.block_table), p(b.seq_lens), 8, 2, 128, 16,
                                ctypes.c_float(0.1), p(out), 1, b.block_table.shape[1], b.num_pages, None, p(ws),
-                               ws.numel(), None, 0, 0, layout)
+                               ws.numel(), None, 0, 0, layout, None)
     assert lib.comem_decode_attn_fp8_async(*args(None, 0)) == comem.COMEM_ERR_INVALID_ARG
     assert lib.comem_decode_attn_fp8_async(*args(p(sc), 5)) == comem.COMEM_ERR_INVALID_ARG
     assert lib.comem_decode_attn_fp8_async(*args(p(sc), 0)) == comem.COMEM_OK

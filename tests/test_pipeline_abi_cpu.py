@@ -41,3 +41,19 @@ def test_latency_model_matches_oracle_and_case_study():
         for y in (10.0, 1000.0):
             assert comem.comem_net_speedup(y, l_full, l_sum, 2e-4, 2000.0, 3000.0) == \
                    KP.net_speedup(y, l_full, l_sum, 2e-4, 2000.0, 3000.0)
+
+
+def test_sm_partition_policy():
+    """comem_sm_partition: shares proportional to the bytes, a floor on each side, always the whole GPU."""
+    assert comem.comem_sm_partition(1.0, 1.0, 148, 8) == (74, 74)
+    assert comem.comem_sm_partition(4.83e9, 3.22e9, 148, 8) == (89, 59)          # config 5: agent C3 + memory batch
+    assert comem.comem_sm_partition(1e9, 0.0, 148, 8) == (140, 8)
+    assert comem.comem_sm_partition(0.0, 0.0, 148, 8) == (74, 74)
+    assert comem.comem_sm_partition(1.0, 1e6, 148, 200) == (74, 74)              # a floor above half is clamped to half
+    for a, b in ((1.0, 3.0), (5.0, 2.0), (1e12, 7.0)):
+        x, y = comem.comem_sm_partition(a, b, 148, 8)
+        assert x + y == 148 and min(x, y) >= 8
+        assert abs(x - 148 * a / (a + b)) <= max(1.0, 8 - 148 * min(a, b) / (a + b) + 1)
+    for bad in ((-1.0, 1.0, 148, 8), (1.0, float("nan"), 148, 8), (1.0, 1.0, 1, 1)):
+        with pytest.raises(comem.ComemError):
+            comem.comem_sm_partition(*bad)
