@@ -370,6 +370,17 @@ int comem_sm_partition(double bytes_a, double bytes_b, int num_sms, int min_ctas
 int comem_set_grid_ctas(int n);
 int comem_set_programmatic_launch(int enabled);
 
+/*
+ * comem_read_ceiling_async — measurement aid: a hand-written read-only sum-reduction over `bytes`
+ * bytes of device memory at `buf` (128-byte aligned, >= 8 KiB; use >= 8 GiB so that nothing is served from L2), the
+ * ceiling eq. 5's W can reach on this part for a kernel that reads every byte once.  variant 0: 16-byte
+ * vector loads, 2 x 1024 threads per SM; variant 1: the attention kernel's own transport (one CTA per SM, TMA bulk
+ * copies into a 16-stage shared-memory ring, 128 KiB in flight per SM).  `sink`: device, COMEM_READ_CEILING_SINK_WORDS
+ * 64-bit words that receive per-CTA sums (so no load can be elided).  Enqueue-only; time it with events on the stream.
+ */
+#define COMEM_READ_CEILING_SINK_WORDS 1024
+int comem_read_ceiling_async(const void *buf, size_t bytes, unsigned long long *sink, int variant, void *cuda_stream);
+
 const char *comem_status_string(int status);
 int comem_version(void);
 

@@ -34,6 +34,8 @@ from .binding import (  # noqa: F401
     comem_schedule_host,
     comem_set_grid_ctas,
     comem_sm_partition,
+    comem_read_ceiling_async,
+    COMEM_READ_CEILING_SINK_WORDS,
     LaunchOpts,
     comem_set_programmatic_launch,
     comem_validate_inputs,

@@ -92,6 +92,8 @@ def load_library():
     lib.comem_schedule_host.restype = i32
     lib.comem_grid_ctas.argtypes = [i32]
     lib.comem_grid_ctas.restype = i32
+    lib.comem_read_ceiling_async.argtypes = [vp, sz, vp, i32, vp]
+    lib.comem_read_ceiling_async.restype = i32
     lib.comem_sm_partition.argtypes = [f64, f64, i32, i32, vp, vp]
     lib.comem_sm_partition.restype = i32
     lib.comem_set_grid_ctas.argtypes = [i32]
@@ -142,6 +144,19 @@ def comem_sm_partition(bytes_a: float, bytes_b: float, num_sms: int, min_ctas: i
     if st != COMEM_OK:
         raise ComemError(st, "comem_sm_partition")
     return a.value, b.value
+
+
+COMEM_READ_CEILING_SINK_WORDS = 1024
+
+
+def comem_read_ceiling_async(buf: torch.Tensor, sink: torch.Tensor, variant: int = 0, stream=None, nbytes=None) -> None:
+    """Measurement aid: enqueue the read-only sum-reduction over `buf` (variant 0: vector loads, 1: TMA ring)."""
+    assert buf.is_cuda and buf.is_contiguous() and sink.is_cuda and sink.dtype == torch.int64
+    assert sink.numel() >= COMEM_READ_CEILING_SINK_WORDS
+    n = buf.numel() * buf.element_size() if nbytes is None else int(nbytes)
+    st = load_library().comem_read_ceiling_async(_ptr(buf), n, _ptr(sink), int(variant), _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_read_ceiling_async")
 
 
 def comem_set_grid_ctas(n: int) -> None:

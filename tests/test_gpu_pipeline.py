@@ -30,7 +30,7 @@ def test_sm_partitioned_streams_match_serial_and_oracle(oracle):
     ws_m = comem.alloc_workspace(memory.q, memory.k_pages, memory.block_table, stream=sb)
     sms = comem.comem_grid_ctas(128)
     ga, gm = comem.comem_sm_partition(agent.algorithmic_bytes(), memory.algorithmic_bytes(), sms)
-    assert ga + gm == sms and ga > gm >= 8        # the agent batch (64 query heads' Q, same KV bytes) is no smaller
+    assert ga + gm == sms and ga >= gm >= 8       # the agent batch (64 query heads' Q, same KV bytes) is no smaller
     steps = [t for t in range(12) if mem[t]]
     assert steps, "the plan launches memory jobs"
 
