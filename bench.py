@@ -44,11 +44,33 @@ UNIT = "GB/s"
 FALLBACK_PEAK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES_NOMINAL = 126e6
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE split-KV launch from the committed
-# `ncu --set full` capture (profiles/r1_b_fused.md names the command; c2 re-captured in profiles/r1_c_fp8_pipeline.md).
-NCU_TRAFFIC_BYTES = {"c2": 137_713_664, "c3": 4_838_226_768, "c4": 8_595_141_560}  # profiles/r1_b_fused.md
-# same for the FP8 kernel (profiles/r1_c_fp8_pipeline.md section 3): (workload, layout) -> bytes
-NCU_TRAFFIC_BYTES_FP8 = {("c4", "NHD"): 4_324_995_000 + 3_796_224, ("c4", "HND"): 4_301_188_000 + 3_680_768}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+
+
+def kernel_source_sha() -> str:
+    """sha256 over the kernel sources a traffic capture belongs to (the attention kernels and what they include)."""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2605_30842_b200", "csrc")
+    for f in ("decode_split.cu", "merge.cuh", "schedule.cuh", "ptx.cuh", "decode_params.cuh", "prefill_attn.cu", "tcgen05.cuh"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the workload's kernel from the committed
+    `ncu --set full` capture recorded in profiles/ncu_traffic.json -- or None when that capture was taken on other
+    kernel sources than the ones in the tree (a stale number is worse than none)."""
+    try:
+        with open(TRAFFIC_FILE) as fh:
+            t = json.load(fh)
+        if t.get("kernel_source_sha") != kernel_source_sha():
+            return None
+        return t["traffic_bytes_per_launch"].get(key)
+    except Exception:  # noqa: BLE001
+        return None
 
 
 def parse_args():
@@ -70,6 +92,10 @@ def parse_args():
     ap.add_argument("--pipeline", type=int, default=0, metavar="K",
                     help="extra: drive 64 agent steps of the k-step-off pipeline (Algorithm 1) from comem_kstep_plan "
                          "and check eq. 5 against the measured decode-attention times")
+    ap.add_argument("--prefill", action="store_true",
+                    help="extra: time comem_prefill_attn_async (paged causal prefill, tcgen05) and print its own line")
+    ap.add_argument("--primary-only", action="store_true",
+                    help="default run without the C3 / C4 / C5 / prefill / read-ceiling blocks of the JSON line")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
@@ -126,6 +152,7 @@ class ClockSampler:
 
     def __init__(self, uuid: str, index: int):
         self.samples, self.reasons, self.active = [], set(), False
+        self.warm_samples, self.warm = [], False   # `warm`: the run-up under the same load as the timed region
         self.max_mhz, self.err = None, None
         self._stop = threading.Event()
         try:
@@ -146,17 +173,18 @@ class ClockSampler:
 
     def _run(self):
         while not self._stop.is_set():
-            if self.active and self.nv is not None:
+            if (self.active or self.warm) and self.nv is not None:
                 try:
                     mhz = int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
                     r = int(self._reasons_fn(self.h))
-                    self.samples.append(mhz)
+                    (self.samples if self.active else self.warm_samples).append(mhz)
                     for bit, nm in self.REASONS.items():
                         if r & bit:
                             self.reasons.add(nm)
                 except Exception as e:  # noqa: BLE001
                     self.err = repr(e)
-            time.sleep(0.002)
+            # a timed region may last half a millisecond: wake often enough to see its start, poll fast inside it
+            time.sleep(0.00005 if self.active else 0.0002)
 
     def start(self):
         self.t.start()
@@ -165,10 +193,15 @@ class ClockSampler:
         self._stop.set()
         self.t.join(timeout=1.0)
 
+    def reset(self):
+        self.samples, self.warm_samples, self.reasons = [], [], set()
+
     def summary(self) -> dict:
         s = sorted(self.samples)
-        out = {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
-               "reasons": sorted(self.reasons), "samples": len(s)}
+        w = sorted(self.warm_samples)
+        use = s if s else w
+        out = {"sm_mhz": (use[len(use) // 2] if use else None), "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(self.reasons), "samples": len(s), "samples_run_up_same_load": len(w)}
         if self.err:
             out["error"] = self.err
         return out
@@ -180,7 +213,9 @@ class ClockSampler:
 def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, phases, use_graph, sampler,
                 device):
     """`warmup` untimed steps, then EXACTLY `steps` steps on `stream`, bracketed by barrier +
-    synchronize on both sides; CUDA events on that stream.  Returns this rank's milliseconds."""
+    synchronize on both sides; CUDA events on that stream.  With graphs (the default) every timed step is
+    replayed from a CUDA graph whatever `steps` is: steps = a * R + r runs as a replays of an R-step graph and one
+    replay of an r-step graph (R = number of rotating pools).  Returns this rank's milliseconds."""
     R = len(pools)
 
     def enqueue(first, n):
@@ -189,27 +224,37 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
             comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
                                                  b.softmax_scale, outs[i % R], ws, stream=stream, phases=phases)
 
+    def capture(first, n):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            enqueue(first, n)
+        return g
+
     with torch.cuda.stream(stream):
         enqueue(0, max(warmup, 3))
         stream.synchronize()
-        graph = None
-        if use_graph and steps >= R:
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph, stream=stream):
-                enqueue(0, R)
-            graph.replay()
-            stream.synchronize()
+        a, r = divmod(steps, R) if use_graph else (0, 0)
+        g_full = capture(0, R) if a else None
+        g_rest = capture(a * R, r) if r else None
+        sampler.warm = True          # the run-up: same kernels, same rate as the timed region
+        for g in (g_full, g_rest):
+            if g is not None:
+                for _ in range(3):
+                    g.replay()
+        stream.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         replicas.barrier()
         torch.cuda.synchronize(device)
+        sampler.warm = False
         sampler.active = True
         e0.record(stream)
-        done = 0
-        if graph is not None:
-            for _ in range(steps // R):
-                graph.replay()
-            done = (steps // R) * R
-        enqueue(done, steps - done)
+        if use_graph:
+            for _ in range(a):
+                g_full.replay()
+            if g_rest is not None:
+                g_rest.replay()
+        else:
+            enqueue(0, steps)
         e1.record(stream)
         torch.cuda.synchronize(device)
         sampler.active = False
@@ -411,20 +456,13 @@ def run_reference(args, rank: int) -> int:
     return 0
 
 
-def run_c5(args) -> int:
+def measure_c5(args, torch, comem, device, reps=None) -> dict:
     """BASELINE.json configs[4]: the agent batch (C3) and the memory-model batch on two CUDA streams,
-    64 successive decode steps each (append one token per sequence, then attend).  Reports each stream
-    alone, both overlapped, and the aggregate GB/s over the overlapped window.  1 GPU only."""
-    import torch
-    import paper_2605_30842_b200 as comem
-    from paper_2605_30842_b200 import build as cuda_build
+    64 successive decode steps each (append one token per sequence, then attend).  Each stream alone, both
+    overlapped with full grids (time sharing), both overlapped under the library's SM-partition policy
+    (comem_sm_partition + per-call launch options), and the aggregate GB/s over the overlapped window."""
     from paper_2605_30842_b200 import workloads as W
 
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
-    device = torch.device("cuda", 0)
-    torch.cuda.set_device(device)
-    cuda_build.build()
-    comem.load_library()
     n_steps = 64
     agent = W.config3_agent_ragged(device, spare_tokens=n_steps)
     memory = W.config5_memory_ragged(device, spare_tokens=n_steps)
@@ -444,14 +482,19 @@ def run_c5(args) -> int:
         return sum((l0 + (i + 1) * b.batch) * per_tok + b.batch * b.num_q_heads * b.head_dim * 2
                    for i in range(n_steps))
 
-    def enqueue(j, i):
+    by_a, by_m = nbytes(jobs[0]), nbytes(jobs[1])
+    sms = comem.comem_grid_ctas(128)
+    part = comem.comem_sm_partition(by_a, by_m, sms)
+
+    def enqueue(j, i, grid=None):
         b, st = j["b"], j["stream"]
         q, nk, nv = j["rows"][i]
         comem.comem_kv_append_async(b.k_pages, b.v_pages, b.block_table, b.seq_lens, nk, nv, stream=st)
         comem.comem_decode_attn_async(q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale,
-                                      j["out"], j["ws"], stream=st)
+                                      j["out"], j["ws"], stream=st, grid_ctas=grid,
+                                      programmatic_launch=None if grid is None else False)
 
-    def run(which):
+    def run(which, grids=None):
         for j in jobs:
             j["b"].seq_lens.copy_(j["len0"])
         torch.cuda.synchronize(device)
@@ -463,34 +506,63 @@ def run_c5(args) -> int:
             ev[k][0].record(jobs[k]["stream"])
         for i in range(n_steps):
             for k in which:
-                enqueue(jobs[k], i)
+                enqueue(jobs[k], i, None if grids is None else grids[k])
         for k in which:
             ev[k][1].record(jobs[k]["stream"])
         torch.cuda.synchronize(device)
         return {k: (t0.elapsed_time(ev[k][1]), ev[k][0].elapsed_time(ev[k][1])) for k in which}
 
     run([0, 1])  # warm-up
-    reps = max(1, min(5, args.steps // n_steps if args.steps >= n_steps else 1))
+    if reps is None:
+        reps = max(1, min(5, args.steps // n_steps if args.steps >= n_steps else 1))
     alone_a = min(run([0])[0][1] for _ in range(reps))
     alone_m = min(run([1])[1][1] for _ in range(reps))
     both = [run([0, 1]) for _ in range(reps)]
     best = min(both, key=lambda r: max(r[0][0], r[1][0]))
     window = max(best[0][0], best[1][0])
-    by_a, by_m = nbytes(jobs[0]), nbytes(jobs[1])
-    line = {"metric": METRIC, "value": (by_a + by_m) / (window * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
-            "steps": n_steps, "warmup": n_steps, "ms_per_step": window / n_steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+    pboth = [run([0, 1], grids=part) for _ in range(reps)]
+    pbest = min(pboth, key=lambda r: max(r[0][0], r[1][0]))
+    pwindow = max(pbest[0][0], pbest[1][0])
+    share_a = part[0] / sms
+    return {"n_steps": n_steps, "bytes_agent": by_a, "bytes_memory": by_m, "window_ms": window,
+            "aggregate_gbs": (by_a + by_m) / (window * 1e-3) / 1e9,
+            "agent_alone_us_per_step": alone_a / n_steps * 1e3, "memory_alone_us_per_step": alone_m / n_steps * 1e3,
+            "overlapped_window_us_per_step": window / n_steps * 1e3,
+            "agent_overlapped_us_per_step": best[0][1] / n_steps * 1e3,
+            "memory_overlapped_us_per_step": best[1][1] / n_steps * 1e3,
+            "agent_slowdown": best[0][1] / alone_a, "memory_slowdown": best[1][1] / alone_m,
+            "agent_alone_gbs": by_a / (alone_a * 1e-3) / 1e9, "memory_alone_gbs": by_m / (alone_m * 1e-3) / 1e9,
+            "serial_sum_us_per_step": (alone_a + alone_m) / n_steps * 1e3,
+            "sm_partition": {"policy": "comem_sm_partition (proportional to bytes), per-call launch options, PDL off",
+                             "agent_ctas": part[0], "memory_ctas": part[1],
+                             "window_us_per_step": pwindow / n_steps * 1e3,
+                             "aggregate_gbs": (by_a + by_m) / (pwindow * 1e-3) / 1e9,
+                             "agent_us_per_step": pbest[0][1] / n_steps * 1e3,
+                             "memory_us_per_step": pbest[1][1] / n_steps * 1e3,
+                             "agent_slowdown": pbest[0][1] / alone_a, "memory_slowdown": pbest[1][1] / alone_m,
+                             "agent_sm_share": share_a,
+                             "agent_slowdown_bound_1_over_share": 1.0 / share_a}}
+
+
+def run_c5(args) -> int:
+    """--workload c5: the config-5 measurement as its own JSON line (1 GPU only)."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    c5 = measure_c5(args, torch, comem, device)
+    line = {"metric": METRIC, "value": c5["aggregate_gbs"], "unit": UNIT, "n_gpus": 1,
+            "steps": c5["n_steps"], "warmup": c5["n_steps"], "ms_per_step": c5["window_ms"] / c5["n_steps"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": "C5 k-step-off overlap: C3 agent batch + memory batch (8 x U[65536,131072], 32q/8kv) "
                                    "on two streams, 64 append+attend steps each",
                        "l2": "cold: each step reads 4.5 + 3.0 GiB of KV >> L2", "launch": "host launches, 2 kernels per step per stream"},
-            "c5": {"agent_alone_us_per_step": alone_a / n_steps * 1e3, "memory_alone_us_per_step": alone_m / n_steps * 1e3,
-                   "overlapped_window_us_per_step": window / n_steps * 1e3,
-                   "agent_overlapped_us_per_step": best[0][1] / n_steps * 1e3,
-                   "memory_overlapped_us_per_step": best[1][1] / n_steps * 1e3,
-                   "agent_slowdown": best[0][1] / alone_a, "memory_slowdown": best[1][1] / alone_m,
-                   "agent_alone_gbs": by_a / (alone_a * 1e-3) / 1e9, "memory_alone_gbs": by_m / (alone_m * 1e-3) / 1e9,
-                   "serial_sum_us_per_step": (alone_a + alone_m) / n_steps * 1e3},
-            "gpu_launches": 4 * n_steps}
+            "c5": c5, "gpu_launches": 4 * c5["n_steps"]}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -732,7 +804,7 @@ def run_fp8(args) -> int:
                       "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128, 1>", "achieved": gbs,
                                    "peak": peaks["hbm_gbs"], "unit": UNIT, "frac": gbs / peaks["hbm_gbs"],
                                    "us_per_launch": us,
-                                   "traffic": NCU_TRAFFIC_BYTES_FP8.get((args.workload, pools[0].kv_layout))},
+                                   "traffic": ncu_traffic("fp8_%s_%s" % (args.workload, pools[0].kv_layout.lower()))},
                       "gpu_launches": replays * per_graph, "parity": parity, "oracle_seconds_one_sequence": oracle_s,
                       "bf16_cache_bytes_same_tokens": bf16_bytes,
                       "equivalent_bf16_gbs": bf16_bytes / us / 1e3, "clocks": sampler.summary(),
@@ -882,6 +954,190 @@ def run_pipeline(args) -> int:
     return 0
 
 
+def load_peaks():
+    peaks = {"hbm_gbs": FALLBACK_PEAK_GBS, "hbm_src": "fallback (B200_PROFILING.md)",
+             "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "tf_src": "fallback (B200_PROFILING.md)"}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            m = json.load(f)
+        peaks.update({"hbm_gbs": float(m["hbm_gbs"]), "hbm_src": "measured (MEASURED_PEAKS.json hbm_gbs, copy)",
+                      "bf16_tflops": float(m["bf16_tflops"]), "bf16_tflops_sustained": float(m["bf16_tflops_sustained"]),
+                      "tf_src": "measured (MEASURED_PEAKS.json)"})
+    except Exception:  # noqa: BLE001
+        pass
+    return peaks
+
+
+def measure_read_ceiling(torch, comem, device, stream, buf=None) -> dict:
+    """what a read-only stream gets on this part -- the library's two hand-written sum-reductions
+    (comem_read_ceiling_async) over >= 8 GiB, best of 5 each, CUDA events on the launch stream."""
+    own = buf is None
+    if own:
+        buf = torch.empty(8 << 30, dtype=torch.uint8, device=device)
+        buf.random_(0, 255)
+    nbytes = (buf.numel() * buf.element_size()) // 8192 * 8192
+    sink = torch.zeros(comem.COMEM_READ_CEILING_SINK_WORDS, dtype=torch.int64, device=device)
+    out = {"bytes": nbytes}
+    with torch.cuda.stream(stream):
+        for variant, name in ((0, "vector_loads"), (1, "tma_ring")):
+            ts = []
+            for i in range(7):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                comem.comem_read_ceiling_async(buf, sink, variant, stream=stream, nbytes=nbytes)
+                e1.record(stream)
+                stream.synchronize()
+                if i >= 2:
+                    ts.append(e0.elapsed_time(e1))
+            out[name + "_gbs"] = nbytes / min(ts) / 1e6
+            out[name + "_gbs_median"] = nbytes / sorted(ts)[len(ts) // 2] / 1e6
+    out["read_ceiling_gbs"] = max(out["vector_loads_gbs"], out["tma_ring_gbs"])
+    return out
+
+
+def measure_decode(ctx, name, steps, warmup, *, primary):
+    """One decode workload: the timed K steps (graph replays), and -- for the primary workload -- the split-only
+    timing, the isolated-step spread, a sustained run and the end-to-end leg."""
+    torch, comem, replicas, args = ctx["torch"], ctx["comem"], ctx["replicas"], ctx["args"]
+    device, rank, world, stream = ctx["device"], ctx["rank"], ctx["world"], ctx["stream"]
+    R_spare = 8 if name == "c2" else 1
+    spare = ((steps + max(warmup, 3)) // R_spare + 8) if primary else 0
+    pools = make_pools(name, device, rank, spare)
+    R = len(pools)
+    outs = [torch.empty_like(b.q) for b in pools]
+    ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream)
+    step_bytes = [b.algorithmic_bytes() for b in pools]
+    kv_pool_bytes = sum(int(b.seq_lens.sum().item()) * b.num_kv_heads * b.head_dim * 4 for b in pools)
+    sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), ctx["local_rank"])
+    sampler.start()
+    both = comem.COMEM_PHASE_SPLIT | comem.COMEM_PHASE_COMBINE
+    use_graph = not args.no_graph
+    with torch.cuda.stream(stream):   # one checked step on pool 0 first (feeds the parity block)
+        comem.comem_decode_attn_async(pools[0].q, pools[0].k_pages, pools[0].v_pages, pools[0].block_table,
+                                      pools[0].seq_lens, pools[0].softmax_scale, outs[0], ws, stream=stream)
+    stream.synchronize()
+    first_out = outs[0].clone()
+
+    ms = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, both, use_graph, sampler, device)
+    clocks = sampler.summary()
+    bytes_k_steps = sum(step_bytes[i % R] for i in range(steps))
+    ms_max = replicas.max_over_ranks(ms, device)
+    total_bytes = replicas.sum_over_ranks(bytes_k_steps, device)
+    res = {"pools": pools, "ws": ws, "R": R, "ms_max": ms_max, "total_bytes": total_bytes, "bytes_k_steps": bytes_k_steps,
+           "kv_pool_bytes": kv_pool_bytes, "clocks": clocks, "first_out": first_out, "steps": steps}
+    if primary:
+        ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup,
+                               comem.COMEM_PHASE_SPLIT, use_graph, sampler, device)
+        res["ms_split_max"] = replicas.max_over_ranks(ms_split, device)
+        res["dist"] = step_distribution(torch, comem, pools, outs, ws, stream, 200 if name == "c2" else 20, both)
+        # a sustained run of the same steps (seconds-scale thermals and the power cap show only here)
+        long_steps = max(steps, 8192 if name == "c2" else 256)
+        if long_steps != steps:
+            sampler.reset()
+            ms_long = timed_steps(torch, comem, replicas, pools, outs, ws, stream, long_steps, 3, both, use_graph,
+                                  sampler, device)
+            res["sustained"] = {"steps": long_steps, "us_per_step": replicas.max_over_ranks(ms_long, device) / long_steps * 1e3,
+                                "clocks": sampler.summary()}
+    sampler.stop()
+    return res
+
+
+def measure_prefill(ctx, peaks, with_parity=True) -> dict:
+    """the paged causal prefill kernel (tcgen05) on the agent geometry -- an uncached full prefill
+    of one 32 768-token context (Alg. 1 line 12) and a cached 512-token chunk over the same prefix (line 10).
+    TFLOP/s = causal flops (4 D per (query, key <= pos) pair and query head) / CUDA-event time, against the measured
+    sustained bf16 peak."""
+    torch, comem, stream = ctx["torch"], ctx["comem"], ctx["stream"]
+    from paper_2605_30842_b200 import workloads as W
+
+    out = {}
+    for key, lens, qn in (("uncached_32k", [32768], [32768]), ("cached_chunk_512_over_32k", [32768], [512]),
+                          ("batch8_uncached_8k", [8192] * 8, [8192] * 8)):
+        pb = W.make_prefill_batch(lens, qn, 64, 8, 128, 16, seed=2001, device=ctx["device"], k_scale=0.5)
+        o = torch.empty_like(pb.q)
+        reps = 3 if key == "uncached_32k" else 10
+        with torch.cuda.stream(stream):
+            f = lambda: comem.comem_prefill_attn_async(pb.q, pb.k_pages, pb.v_pages, pb.block_table, pb.seq_lens,  # noqa: E731
+                                                       pb.q_start, pb.softmax_scale, o, stream=stream)
+            for _ in range(3):
+                f()
+            stream.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                f()
+            e1.record(stream)
+            stream.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        fl = pb.algorithmic_flops()
+        rec = {"ms": ms, "algorithmic_flops": fl, "tflops": fl / ms / 1e9,
+               "frac_of_sustained_peak": fl / ms / 1e9 / peaks["bf16_tflops_sustained"],
+               "frac_of_burst_peak": fl / ms / 1e9 / peaks["bf16_tflops"]}
+        if key == "uncached_32k":
+            rec["tokens_per_s"] = 32768 / (ms * 1e-3)
+        if with_parity and key != "batch8_uncached_8k":
+            rec["parity"] = prefill_parity_sampled(pb, o)
+        out[key] = rec
+        del pb, o
+    return out
+
+
+def prefill_parity_sampled(pb, gpu_out, n_rows=6):
+    """Oracle on sampled query rows of a prefill batch, all query heads: row i of sequence 0 is, by the prefill
+    oracle's own definition (pin PF2), the decode oracle on the cache truncated at its position."""
+    import numpy as np
+    import torch
+    import oracle
+
+    oracle.build()
+    L, n = int(pb.seq_lens[0]), int(pb.q_start[1])
+    rows = sorted({0, 1, n // 3, n // 2 + 5, n - 2, n - 1} & set(range(n)))[:n_rows]
+    ps = pb.page_size
+    npg = (L + ps - 1) // ps
+    ids = pb.block_table[0, :npg].long()
+    kp, vp = pb.k_pages[ids].cpu(), pb.v_pages[ids].cpu()
+    bt = torch.arange(npg, dtype=torch.int32).view(1, npg).repeat(len(rows), 1)
+    sl = torch.tensor([L - n + i + 1 for i in rows], dtype=torch.int32)
+    q = pb.q[rows].cpu().contiguous()
+    ref, _ = oracle.decode_attn(q, kp, vp, bt, sl, pb.softmax_scale)
+    got = gpu_out[rows].double().cpu().numpy()
+    d = np.abs(got - ref)
+    par = {"rows": len(rows) * pb.num_q_heads, "max_abs": float(d.max()), "mean_abs": float(d.mean()),
+           "rel_l2": float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300))}
+    par["ok"] = bool(par["max_abs"] <= 2e-2 and par["mean_abs"] <= 2e-3 and par["rel_l2"] <= 5e-3)
+    return par
+
+
+def run_prefill(args) -> int:
+    """--prefill: the prefill kernel's own JSON line (extra; metric TFLOP/s against the measured bf16 peak)."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    peaks = load_peaks()
+    ctx = {"torch": torch, "comem": comem, "device": device, "stream": torch.cuda.Stream(device)}
+    sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), 0)
+    sampler.start()
+    sampler.active = True
+    pf = measure_prefill(ctx, peaks, with_parity=not args.no_cpu_baseline)
+    sampler.active = False
+    sampler.stop()
+    top = pf["uncached_32k"]
+    print(json.dumps({"extra": "paged causal prefill attention (tcgen05)", "metric": "prefill_attn_tflops",
+                      "value": top["tflops"], "unit": "TFLOP/s", "dtype": "bf16", "data": "synthetic",
+                      "config": {"workload": "uncached full prefill: batch 1, 64q/8kv, D128, 32768 tokens, page 16"},
+                      "roofline": {"bound": "tensor", "kernel": "prefill_attn_kernel<128>", "achieved": top["tflops"],
+                                   "peak": peaks["bf16_tflops_sustained"], "peak_source": peaks["tf_src"] + " bf16_tflops_sustained",
+                                   "unit": "TFLOP/s", "frac": top["frac_of_sustained_peak"],
+                                   "traffic": ncu_traffic("prefill_uncached_32k")},
+                      "prefill": pf, "clocks": sampler.summary()}), flush=True)
+    return 0
+
+
 def main() -> int:
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -895,6 +1151,8 @@ def main() -> int:
         return run_fp8(args) if rank == 0 else 0
     if args.affine:
         return run_affine(args) if rank == 0 else 0
+    if args.prefill:
+        return run_prefill(args) if rank == 0 else 0
     if args.workload == "c5":
         return run_c5(args) if rank == 0 else 0
 
@@ -912,83 +1170,109 @@ def main() -> int:
         cuda_build.build()
     replicas.barrier()
     comem.load_library()
-
-    R_spare = 8 if args.workload == "c2" else 1
-    spare = (args.steps + max(args.warmup, 3)) // R_spare + 8
-    pools = make_pools(args.workload, device, rank, spare)
-    R = len(pools)
-    outs = [torch.empty_like(b.q) for b in pools]
+    peaks = load_peaks()
     stream = torch.cuda.Stream(device)
-    ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream)
-    step_bytes = [b.algorithmic_bytes() for b in pools]
-    kv_pool_bytes = sum(int(b.seq_lens.sum().item()) * b.num_kv_heads * b.head_dim * 4 for b in pools)
-    sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), local_rank)
-    sampler.start()
+    ctx = {"torch": torch, "comem": comem, "replicas": replicas, "args": args, "device": device, "rank": rank,
+           "local_rank": local_rank, "world": world, "stream": stream}
 
-    both = comem.COMEM_PHASE_SPLIT | comem.COMEM_PHASE_COMBINE
-    # one checked step on pool 0 first (also feeds the parity block)
-    with torch.cuda.stream(stream):
-        comem.comem_decode_attn_async(pools[0].q, pools[0].k_pages, pools[0].v_pages, pools[0].block_table,
-                                      pools[0].seq_lens, pools[0].softmax_scale, outs[0], ws, stream=stream)
-    stream.synchronize()
-    first_out = outs[0].clone()
-
-    ms = timed_steps(torch, comem, replicas, pools, outs, ws, stream, args.steps, args.warmup, both,
-                     not args.no_graph, sampler, device)
-    ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, args.steps, args.warmup,
-                           comem.COMEM_PHASE_SPLIT, not args.no_graph, sampler, device)
-    dist = step_distribution(torch, comem, pools, outs, ws, stream, 200 if args.workload == "c2" else 20, both)
-    bytes_k_steps = sum(step_bytes[i % R] for i in range(args.steps))
-    ms_max = replicas.max_over_ranks(ms, device)
-    ms_split_max = replicas.max_over_ranks(ms_split, device)
-    total_bytes = replicas.sum_over_ranks(bytes_k_steps, device)
-
+    prim = measure_decode(ctx, args.workload, args.steps, args.warmup, primary=True)
+    pools, ws, R = prim["pools"], prim["ws"], prim["R"]
     cpu_base, parity = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_base, parity = cpu_baseline_and_parity(pools[0], first_out)
-
+        cpu_base, parity = cpu_baseline_and_parity(pools[0], prim["first_out"])
+    e2e_sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), local_rank)
+    e2e_sampler.start()
     e2e_ms, e2e_bytes, h2d, d2h = timed_e2e(torch, comem, replicas, pools, ws, stream, args.steps, args.warmup,
-                                            sampler, device, 5000 + 1000 * rank)
+                                            e2e_sampler, device, 5000 + 1000 * rank)
+    e2e_sampler.stop()
     e2e_ms_max = replicas.max_over_ranks(e2e_ms, device)
     e2e_total = replicas.sum_over_ranks(e2e_bytes, device)
-    sampler.stop()
+    checks = pools[0].checksums()
+    del pools, ws
+    prim["pools"] = prim["ws"] = None
+    torch.cuda.empty_cache()
+
+    # The other workloads the metric is quoted on ("at 32K-128K ctx"): C3, C4, C5's aggregate, the prefill kernel and
+    # the read-only ceiling, inside the same JSON line (1 GPU, default workload only; --primary-only skips them).
+    extra = {}
+    ceiling = None
+    if rank == 0 and world == 1 and args.workload == "c2" and not args.primary_only:
+        for name in ("c3", "c4"):
+            k = max(3, min(args.steps, 100))
+            r = measure_decode(ctx, name, k, 3, primary=False)
+            us = r["ms_max"] / k * 1e3
+            gbs = (r["bytes_k_steps"] / k) / us / 1e3
+            rec = {"workload": workload_desc(name)["workload"], "steps": k, "us_per_step": us, "achieved": gbs,
+                   "unit": UNIT, "frac": gbs / peaks["hbm_gbs"], "frac_of_8TBps": gbs / 8000.0,
+                   "algorithmic_bytes_per_step": r["bytes_k_steps"] // k, "traffic": ncu_traffic(name),
+                   "launch": "CUDA graph, replayed", "clocks": r["clocks"]}
+            if not args.no_cpu_baseline:
+                cb, par = cpu_baseline_and_parity(r["pools"][0], r["first_out"], budget_s=6.0)
+                rec["parity"] = par
+                rec["oracle_gbs"] = cb["value"]
+            extra[name] = rec
+            r["pools"] = r["ws"] = None
+            del r
+            torch.cuda.empty_cache()
+        ceiling = measure_read_ceiling(torch, comem, device, stream)   # its own 8 GiB buffer
+        torch.cuda.empty_cache()
+        for rec in extra.values():
+            rec["frac_of_read_ceiling"] = rec["achieved"] / ceiling["read_ceiling_gbs"]
+        c5 = measure_c5(args, torch, comem, device, reps=2)
+        c5["frac_of_8TBps"] = c5["aggregate_gbs"] / 8000.0
+        c5["frac_of_read_ceiling"] = c5["aggregate_gbs"] / ceiling["read_ceiling_gbs"]
+        extra["c5"] = c5
+        torch.cuda.empty_cache()
+        extra["prefill"] = measure_prefill(ctx, peaks, with_parity=not args.no_cpu_baseline)
+        torch.cuda.empty_cache()
 
     if rank == 0:
-        peak, peak_src = FALLBACK_PEAK_GBS, "fallback (B200_PROFILING.md)"
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-                peak, peak_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
-        except Exception:  # noqa: BLE001
-            pass
-        value = total_bytes / (ms_max * 1e-3) / 1e9
-        achieved = (bytes_k_steps / args.steps) / (ms_max / args.steps * 1e-3) / 1e9
+        peak, peak_src = peaks["hbm_gbs"], peaks["hbm_src"]
+        ms_max, steps = prim["ms_max"], args.steps
+        value = prim["total_bytes"] / (ms_max * 1e-3) / 1e9
+        achieved = (prim["bytes_k_steps"] / steps) / (ms_max / steps * 1e-3) / 1e9
         cfg = workload_desc(args.workload)
-        cfg.update({"l2": (f"cold: steps rotate over {R} disjoint KV pools ({kv_pool_bytes / 2**30:.2f} GiB) > L2"
-                           if R > 1 else f"cold: one step reads {kv_pool_bytes / 2**30:.2f} GiB of KV >> L2"),
-                    "launch": "CUDA graph of %d steps, replayed" % R if not args.no_graph else "host launches",
-                    "algorithmic_bytes_per_step": bytes_k_steps // args.steps,
+        kvp = prim["kv_pool_bytes"]
+        a, r_ = divmod(steps, R)
+        cfg.update({"l2": (f"cold: steps rotate over {R} disjoint KV pools ({kvp / 2**30:.2f} GiB) > L2"
+                           if R > 1 else f"cold: one step reads {kvp / 2**30:.2f} GiB of KV >> L2"),
+                    "launch": ("CUDA graphs only: %d replays of a %d-step graph + one %d-step graph" % (a, R, r_))
+                    if not args.no_graph else "host launches",
+                    "algorithmic_bytes_per_step": prim["bytes_k_steps"] // steps,
                     "grid_ctas": comem.comem_grid_ctas(cfg["head_dim"]),
                     "replicas": world})
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "us_per_step": ms_max / args.steps * 1e3,
+        roof = {"bound": "hbm", "kernel": "decode_split_kernel<128, 0>", "achieved": achieved,
+                "peak": peak, "peak_source": peak_src, "unit": UNIT, "frac": achieved / peak,
+                "us_per_launch": ms_max / steps * 1e3,
+                "split_only_us": prim["ms_split_max"] / steps * 1e3,
+                "traffic": ncu_traffic(args.workload), "traffic_source": "profiles/ncu_traffic.json (null when the capture predates the kernel sources)"}
+        if ceiling is not None:
+            roof["read_ceiling_gbs"] = ceiling["read_ceiling_gbs"]
+            roof["frac_of_read_ceiling"] = achieved / ceiling["read_ceiling_gbs"]
+            roof["read_ceiling"] = ceiling
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+                "warmup": args.warmup, "ms_per_step": ms_max / steps, "us_per_step": ms_max / steps * 1e3,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
                 "data": "synthetic", "config": cfg,
                 "frac_of_8TBps": value / world / 8000.0,
-                "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128, 0>", "achieved": achieved,
-                             "peak": peak, "peak_source": peak_src, "unit": UNIT, "frac": achieved / peak,
-                             "us_per_launch": ms_max / args.steps * 1e3,
-                             "split_only_us": ms_split_max / args.steps * 1e3,
-                             "traffic": NCU_TRAFFIC_BYTES.get(args.workload)},
+                "roofline": roof,
                 "e2e": {"value": e2e_total / (e2e_ms_max * 1e-3) / 1e9, "unit": UNIT,
                         "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                        "us_per_step": e2e_ms_max / args.steps * 1e3,
+                        "us_per_step": e2e_ms_max / steps * 1e3,
                         "api": "comem_decode_step_host, pinned host buffers: K3 reads the q,k,v rows over the host link and appends -> fused split+combine stores out into host memory -> stream synchronize (2 launches, no copy engine)"},
-                "isolated_step_us": dist, "input_checksums": pools[0].checksums(),
-                "gpu_launches": args.steps,
-                "clocks": sampler.summary()}
+                "isolated_step_us": prim["dist"], "input_checksums": checks,
+                "gpu_launches": steps,
+                "clocks": prim["clocks"]}
+        if "sustained" in prim:
+            s_ = prim["sustained"]
+            s_["achieved"] = (prim["bytes_k_steps"] / steps) / s_["us_per_step"] / 1e3
+            s_["frac"] = s_["achieved"] / peak
+            line["sustained"] = s_
         if cpu_base is not None:
             line["cpu_baseline"] = cpu_base
             line["parity"] = parity
+        if extra:
+            line["workloads"] = extra
         print(json.dumps(line), flush=True)
     replicas.finalize()
     return 0
