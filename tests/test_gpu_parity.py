@@ -317,3 +317,84 @@ def test_randomised_shapes(oracle, case):
         assert torch.equal(bits(out), bits(out2)) and torch.equal(lse.nan_to_num(neginf=-1e30), lse2.nan_to_num(neginf=-1e30))
     finally:
         comem.comem_set_grid_ctas(0)
+
+
+# ---- the paper's batch sizes (Fig. 2: batch 1 / 16 / 64; L257 section 4.4: 32 -> 256; L463-470 Table 7:
+# concurrency up to 128) and the ABI's limit: the strided prefix sum of the scheduler's prologue (batch > 32), the
+# shared-memory prefix table at COMEM_MAX_BATCH, the linear schedule with thousands of segments, K2 at large batch ----
+def _ragged(rng, batch, hi, zero_frac=0.1):
+    special = [0, 1, 15, 16, 17, 31, 32, 33]
+    return [0 if rng.random() < zero_frac else (int(rng.choice(special)) if rng.random() < 0.2 else int(rng.integers(1, hi)))
+            for _ in range(batch)]
+
+
+@pytest.mark.parametrize("batch,hi", [(33, 3000), (64, 2500), (128, 1200), (256, 700), (4096, 90)])
+@pytest.mark.parametrize("G,ps", [(8, 16), (4, 32)])
+def test_large_batches(oracle, batch, hi, G, ps):
+    rng = np.random.default_rng(7000 + batch + G)
+    lens = _ragged(rng, batch, hi)
+    lens[batch // 2] = 4 * hi                      # one long sequence among the short ones: cut by several CTAs
+    b = W.make_batch(lens, G * 8, 8, 128, ps, seed=7100 + batch + G, device=DEV, poison_unused=True)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    base = None
+    for grid in (None, 1, 37, 148, 1024):
+        out = torch.full_like(b.q, float("nan"))
+        lse = torch.full((b.batch, b.num_q_heads), float("nan"), dtype=torch.float32, device=DEV)
+        comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, out, ws,
+                                      lse_out=lse, grid_ctas=grid)
+        torch.cuda.synchronize()
+        if base is None:
+            pairs = all_pairs(b) if batch <= 256 else [(x, h) for x in range(0, batch, 7) for h in range(0, G * 8, 5)] + \
+                [(batch // 2, h) for h in range(G * 8)]
+            ref, ref_lse = oracle_rows(oracle, b, pairs)
+            base = (out, lse)
+        assert_parity(errors(out, ref, pairs), f"batch {batch} grid {grid}")
+        glse = np.array([float(lse[x, h]) for x, h in pairs])
+        assert np.array_equal(np.isneginf(glse), np.isneginf(ref_lse))
+        empty = (b.seq_lens == 0).nonzero().flatten().tolist()
+        assert all(float(out[e].abs().max()) == 0.0 for e in empty[:8])
+    # run to run and under a page permutation: bit-identical (default grid)
+    o2, l2 = gpu_run(b, workspace=ws)
+    o3, l3 = gpu_run(W.permute_pages(b, seed=batch))
+    assert torch.equal(bits(base[0]), bits(o2)) and torch.equal(bits(base[0]), bits(o3))
+    assert torch.equal(base[1].nan_to_num(neginf=-1e30), l3.nan_to_num(neginf=-1e30))
+    # the two-call form (K1 un-fused, then the stand-alone K2) at this batch
+    two = torch.full_like(b.q, float("nan"))
+    for ph in (comem.COMEM_PHASE_SPLIT, comem.COMEM_PHASE_COMBINE):
+        comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale,
+                                             two, ws, phases=ph)
+    torch.cuda.synchronize()
+    assert_parity(errors(two, ref, pairs), f"batch {batch} two-phase")
+
+
+def test_max_batch_fp8_and_window(oracle):
+    """COMEM_MAX_BATCH with the FP8 cache and with a sliding window (the same prologue, other tile maps)."""
+    rng = np.random.default_rng(7999)
+    lens = _ragged(rng, 4096, 70)
+    b = W.make_batch(lens, 16, 4, 128, 16, seed=7998, device=DEV, poison_unused=True)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    out = torch.full_like(b.q, float("nan"))
+    comem.comem_decode_attn_window_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, out,
+                                         ws, 24, 2)
+    torch.cuda.synchronize()
+    c = b.to("cpu")
+    ref, _ = oracle.decode_attn_window(c.q, c.k_pages, c.v_pages, c.block_table, c.seq_lens, c.softmax_scale, 24, 2)
+    assert_parity(_err_dense(out, ref), "window at max batch")
+    f = W.quantize_batch_fp8(b)
+    out8 = torch.full_like(f.q, float("nan"))
+    comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                      f.softmax_scale, out8, ws)
+    torch.cuda.synchronize()
+    cf = f.to("cpu")
+    ref8, _ = oracle.decode_attn_fp8(cf.q, cf.k_pages, cf.v_pages, cf.k_scale, cf.v_scale, cf.block_table, cf.seq_lens,
+                                     cf.softmax_scale)
+    assert_parity(_err_dense(out8, ref8), "fp8 at max batch")
+
+
+def _err_dense(gpu_out, ref):
+    g = gpu_out.double().cpu().numpy().reshape(-1, gpu_out.shape[-1])
+    r = np.asarray(ref).reshape(-1, gpu_out.shape[-1])
+    d = np.abs(g - r)
+    return {"max_abs": float(d.max()), "mean_abs": float(d.mean()),
+            "rel_l2": float(np.linalg.norm(g - r) / max(np.linalg.norm(r), 1e-300)),
+            "max_ref": float(np.abs(r).max()), "finite": bool(np.isfinite(g).all())}
