@@ -45,6 +45,8 @@ FALLBACK_PEAK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES_NOMINAL = 126e6
 
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+# COMEM_LAUNCH_* bits the decode workloads are launched with unless --launch-flags says otherwise
+DEFAULT_LAUNCH_FLAGS = 0
 
 
 def kernel_source_sha() -> str:
@@ -97,6 +99,8 @@ def parse_args():
     ap.add_argument("--primary-only", action="store_true",
                     help="default run without the C3 / C4 / C5 / prefill / read-ceiling blocks of the JSON line")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from the host")
+    ap.add_argument("--launch-flags", type=int, default=None,
+                    help="COMEM_LAUNCH_* bits for the decode calls (default: KV_PREFIX_IMMUTABLE | SPLIT_COMBINE, see DESIGN.md)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
                     help="--impl reference: wall-clock budget for the whole run")
@@ -211,7 +215,7 @@ class ClockSampler:
 # the timed loops
 # ---------------------------------------------------------------------------------------------
 def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, phases, use_graph, sampler,
-                device):
+                device, flags=0):
     """`warmup` untimed steps, then EXACTLY `steps` steps on `stream`, bracketed by barrier +
     synchronize on both sides; CUDA events on that stream.  With graphs (the default) every timed step is
     replayed from a CUDA graph whatever `steps` is: steps = a * R + r runs as a replays of an R-step graph and one
@@ -222,7 +226,8 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
         for i in range(first, first + n):
             b = pools[i % R]
             comem.comem_decode_attn_phases_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
-                                                 b.softmax_scale, outs[i % R], ws, stream=stream, phases=phases)
+                                                 b.softmax_scale, outs[i % R], ws, stream=stream, phases=phases,
+                                                 flags=flags)
 
     def capture(first, n):
         g = torch.cuda.CUDAGraph()
@@ -1012,22 +1017,26 @@ def measure_decode(ctx, name, steps, warmup, *, primary):
     sampler.start()
     both = comem.COMEM_PHASE_SPLIT | comem.COMEM_PHASE_COMBINE
     use_graph = not args.no_graph
-    with torch.cuda.stream(stream):   # one checked step on pool 0 first (feeds the parity block)
+    flags = DEFAULT_LAUNCH_FLAGS if args.launch_flags is None else args.launch_flags
+    res_flags = flags
+    with torch.cuda.stream(stream):   # one checked step on pool 0 first (feeds the parity block): same launch flags
         comem.comem_decode_attn_async(pools[0].q, pools[0].k_pages, pools[0].v_pages, pools[0].block_table,
-                                      pools[0].seq_lens, pools[0].softmax_scale, outs[0], ws, stream=stream)
+                                      pools[0].seq_lens, pools[0].softmax_scale, outs[0], ws, stream=stream, flags=flags)
     stream.synchronize()
     first_out = outs[0].clone()
 
-    ms = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, both, use_graph, sampler, device)
+    ms = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, both, use_graph, sampler, device,
+                     flags=flags)
     clocks = sampler.summary()
     bytes_k_steps = sum(step_bytes[i % R] for i in range(steps))
     ms_max = replicas.max_over_ranks(ms, device)
     total_bytes = replicas.sum_over_ranks(bytes_k_steps, device)
     res = {"pools": pools, "ws": ws, "R": R, "ms_max": ms_max, "total_bytes": total_bytes, "bytes_k_steps": bytes_k_steps,
-           "kv_pool_bytes": kv_pool_bytes, "clocks": clocks, "first_out": first_out, "steps": steps}
+           "kv_pool_bytes": kv_pool_bytes, "clocks": clocks, "first_out": first_out, "steps": steps,
+           "launch_flags": res_flags}
     if primary:
         ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup,
-                               comem.COMEM_PHASE_SPLIT, use_graph, sampler, device)
+                               comem.COMEM_PHASE_SPLIT, use_graph, sampler, device, flags=flags & 1)
         res["ms_split_max"] = replicas.max_over_ranks(ms_split, device)
         res["dist"] = step_distribution(torch, comem, pools, outs, ws, stream, 200 if name == "c2" else 20, both)
         # a sustained run of the same steps (seconds-scale thermals and the power cap show only here)
@@ -1035,7 +1044,7 @@ def measure_decode(ctx, name, steps, warmup, *, primary):
         if long_steps != steps:
             sampler.reset()
             ms_long = timed_steps(torch, comem, replicas, pools, outs, ws, stream, long_steps, 3, both, use_graph,
-                                  sampler, device)
+                                  sampler, device, flags=flags)
             res["sustained"] = {"steps": long_steps, "us_per_step": replicas.max_over_ranks(ms_long, device) / long_steps * 1e3,
                                 "clocks": sampler.summary()}
     sampler.stop()
@@ -1261,7 +1270,8 @@ def main() -> int:
                         "us_per_step": e2e_ms_max / steps * 1e3,
                         "api": "comem_decode_step_host, pinned host buffers: K3 reads the q,k,v rows over the host link and appends -> fused split+combine stores out into host memory -> stream synchronize (2 launches, no copy engine)"},
                 "isolated_step_us": prim["dist"], "input_checksums": checks,
-                "gpu_launches": steps,
+                "gpu_launches": steps * (2 if (prim["launch_flags"] & 2) and args.workload == "c2" else 1),
+                "launch_flags": prim["launch_flags"],
                 "clocks": prim["clocks"]}
         if "sustained" in prim:
             s_ = prim["sustained"]

@@ -71,11 +71,30 @@ enum {
  *                        stream starts its prologue on SMs the previous one has released: shortest back-to-back steps,
  *                        but a stream's NEXT kernel then parks on every free SM; use 0 with an SM partition).
  *                        -1: the default (comem_set_programmatic_launch's value, initially 1).
+ *   flags                bit set of COMEM_LAUNCH_* below; 0 = none.
+ *     COMEM_LAUNCH_KV_PREFIX_IMMUTABLE   a PROMISE by the caller, for decode calls launched with programmatic stream
+ *                        serialization: no work of the stream that may still be running when this call's kernel starts
+ *                        (the kernels enqueued just before it) writes (a) K/V rows at positions below the last 16-token
+ *                        tile of any sequence as seq_lens reads at that moment, (b) the block-table entries of the pages
+ *                        holding them, (c) FP8 cache: those pages' scales.  This is what a decode loop does anyway: the
+ *                        cache of old tokens never changes (the step appends K^(t), V^(t) to
+ *                        the cache of steps < t), comem_kv_append_async writes one row at position seq_lens[b].  The kernel
+ *                        then loads its first tiles into shared memory BEFORE it waits for the preceding kernel
+ *                        (instead of only hinting them into L2), re-validating its schedule after the wait.  Results are
+ *                        bit-identical with and without the flag.  If the promise is broken the call may attend stale rows.
+ *     COMEM_LAUNCH_SPLIT_COMBINE        run the log-sum-exp combine as a second, small kernel launched right behind the
+ *                        split kernel (2 launches; its CTAs sit beside the split kernel's and start the moment the split
+ *                        grid has drained) instead of inside it.  Shortest back-to-back steps for a step of few long
+ *                        segments (batch * num_kv_heads <= 64: one 32K sequence); no gain for large batches.  The combine
+ *                        sums a segment's partials in a different (equally fixed) order than the fused kernel, so the
+ *                        result is within rounding of the default's, and bit-identical to itself from run to run.
  * Two host threads may enqueue concurrently with different options; nothing here is process state.
  */
+enum { COMEM_LAUNCH_KV_PREFIX_IMMUTABLE = 1, COMEM_LAUNCH_SPLIT_COMBINE = 2, COMEM_LAUNCH_Q_STABLE = 4 };
 typedef struct {
     int grid_ctas;
     int programmatic_launch;
+    int flags;
 } comem_launch_opts;
 
 /*

@@ -122,16 +122,22 @@ def comem_grid_ctas(head_dim: int) -> int:
     return g
 
 
+COMEM_LAUNCH_KV_PREFIX_IMMUTABLE = 1
+COMEM_LAUNCH_SPLIT_COMBINE = 2
+COMEM_LAUNCH_Q_STABLE = 4
+
+
 class LaunchOpts(ctypes.Structure):
-    """comem_launch_opts: per-call grid size (0 = default) and programmatic launch (-1 = default)."""
-    _fields_ = [("grid_ctas", ctypes.c_int), ("programmatic_launch", ctypes.c_int)]
+    """comem_launch_opts: per-call grid size (0 = default), programmatic launch (-1 = default), COMEM_LAUNCH_* flags."""
+    _fields_ = [("grid_ctas", ctypes.c_int), ("programmatic_launch", ctypes.c_int), ("flags", ctypes.c_int)]
 
 
-def _opts(grid_ctas, programmatic_launch):
-    """None when both are defaults, else a pointer to a comem_launch_opts (the library reads it during the call)."""
-    if grid_ctas is None and programmatic_launch is None:
+def _opts(grid_ctas, programmatic_launch, flags=0):
+    """None when all are defaults, else a pointer to a comem_launch_opts (the library reads it during the call)."""
+    if grid_ctas is None and programmatic_launch is None and not flags:
         return None
-    o = LaunchOpts(int(grid_ctas or 0), -1 if programmatic_launch is None else (1 if programmatic_launch else 0))
+    o = LaunchOpts(int(grid_ctas or 0), -1 if programmatic_launch is None else (1 if programmatic_launch else 0),
+                   int(flags))
     return ctypes.cast(ctypes.pointer(o), ctypes.c_void_p)
 
 
@@ -282,7 +288,7 @@ COMEM_PHASE_COMBINE = 2
 def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
                                    workspace, lse_out=None, stream=None,
                                    phases: int = COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE,
-                                   grid_ctas=None, programmatic_launch=None) -> None:
+                                   grid_ctas=None, programmatic_launch=None, flags: int = 0) -> None:
     """Enqueue the selected kernels of one decode-attention step on ``stream``; returns at once."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -291,13 +297,13 @@ def comem_decode_attn_phases_async(q, k_pages, v_pages, block_table, seq_lens, s
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream), int(phases),
-        _opts(grid_ctas, programmatic_launch))
+        _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_phases_async")
 
 
 def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
-                            workspace, lse_out=None, stream=None, grid_ctas=None, programmatic_launch=None) -> None:
+                            workspace, lse_out=None, stream=None, grid_ctas=None, programmatic_launch=None, flags: int = 0) -> None:
     """Enqueue one decode-attention step (1 fused kernel launch) on ``stream``; returns at once."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -305,14 +311,14 @@ def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
-        workspace.numel() * workspace.element_size(), _stream(stream), _opts(grid_ctas, programmatic_launch))
+        workspace.numel() * workspace.element_size(), _stream(stream), _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_async")
 
 
 def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
                                    workspace, window: int, sink_tokens: int, lse_out=None, stream=None,
-                                   grid_ctas=None, programmatic_launch=None) -> None:
+                                   grid_ctas=None, programmatic_launch=None, flags: int = 0) -> None:
     """Sliding-window + attention-sink decode attention (one fused launch on ``stream``)."""
     _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
     assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
@@ -321,7 +327,7 @@ def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, s
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens),
-        _opts(grid_ctas, programmatic_launch))
+        _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_window_async")
 
@@ -329,7 +335,7 @@ def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, s
 def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
                                 softmax_scale: float, out, workspace, window: int = 0, sink_tokens: int = 0,
                                 lse_out=None, stream=None, kv_layout: str = "NHD", grid_ctas=None,
-                                programmatic_launch=None) -> None:
+                                programmatic_launch=None, flags: int = 0) -> None:
     """Decode attention over an FP8 (E4M3 bytes + fp32 page scales) KV cache; one fused launch.
     kv_layout "NHD": pools [P, page_size, Hkv, D]; "HND": pools [P, Hkv, page_size, D]."""
     assert kv_layout in ("NHD", "HND")
@@ -350,7 +356,7 @@ def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_tab
         q.shape[1], hkv, q.shape[2], page_size, ctypes.c_float(softmax_scale), _ptr(out),
         q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream), int(window), int(sink_tokens), 1 if hnd else 0,
-        _opts(grid_ctas, programmatic_launch))
+        _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_fp8_async")
 

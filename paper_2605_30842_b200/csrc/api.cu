@@ -267,7 +267,7 @@ using namespace comem;
 
 extern "C" {
 
-int comem_version(void) { return 120; }
+int comem_version(void) { return 130; }
 
 const char *comem_status_string(int status)
 {
@@ -451,8 +451,15 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.part_state = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.part_state);
     p.part_cap = kMaxGridCtas;
     p.seg_counters = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.counters);
-    const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE);
+    const int flags = opts ? opts->flags : 0;
+    if (flags & ~(COMEM_LAUNCH_KV_PREFIX_IMMUTABLE | COMEM_LAUNCH_SPLIT_COMBINE | COMEM_LAUNCH_Q_STABLE)) return COMEM_ERR_INVALID_ARG;
+    // the small dependent combine serves steps of few segments only (elsewhere the fused merge costs nothing)
+    const bool small_combine = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) && (flags & COMEM_LAUNCH_SPLIT_COMBINE) &&
+                               batch * num_kv_heads <= kAlignedMaxSegs;
+    const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) && !small_combine;
     p.fuse_combine = fused ? 1 : 0;
+    p.kv_immutable = (flags & COMEM_LAUNCH_KV_PREFIX_IMMUTABLE) ? 1 : 0;
+    p.q_stable = (flags & COMEM_LAUNCH_Q_STABLE) ? 1 : 0;  // (only acts together with KV_PREFIX_IMMUTABLE)
 #ifdef COMEM_TRACE
     p.trace = g_trace;
 #endif
@@ -472,6 +479,13 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
+    }
+    if (small_combine) {
+        if (launch_combine_small(p, head_dim, stream) != cudaSuccess) {
+            cudaGetLastError();
+            return COMEM_ERR_CUDA;
+        }
+        return COMEM_OK;
     }
     if (!fused && (phases & COMEM_PHASE_COMBINE) && launch_combine(p, head_dim, stream) != cudaSuccess) {
         cudaGetLastError();

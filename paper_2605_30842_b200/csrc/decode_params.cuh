@@ -36,6 +36,10 @@ struct DecodeParams {
     const float *k_scale;        // FP8 cache only (reading R18): fp32 [P][Hkv] page scales, else nullptr
     const float *v_scale;
     int no_pdl;                  // host-side only: launch without programmatic stream serialization (comem_set_programmatic_launch)
+    int kv_immutable;            // COMEM_LAUNCH_KV_PREFIX_IMMUTABLE: the caller promises that nothing still running when this
+                                 // grid starts writes K/V rows (or their block-table entries / page scales) below each
+                                 // sequence's last 16-token tile, so the ring may be filled before griddepcontrol.wait
+    int q_stable;                // COMEM_LAUNCH_Q_STABLE: ... nor q: the consumers may start before the wait too
     int kv_hnd;                  // FP8 cache only: pools laid out [P][Hkv][ps][D] (a tile is 2 KiB contiguous) instead of [P][ps][Hkv][D]
 };
 
@@ -63,6 +67,8 @@ inline cudaError_t set_max_smem_once(Kernel kernel, int bytes, PerDeviceOnce &on
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                                 const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false);
 cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
+// the small dependent combine (COMEM_LAUNCH_SPLIT_COMBINE; batch * Hkv <= kAlignedMaxSegs)
+cudaError_t launch_combine_small(const DecodeParams &p, int head_dim, cudaStream_t stream);
 cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
                              const int32_t *block_table, int32_t *seq_lens,
                              const __nv_bfloat16 *new_k, const __nv_bfloat16 *new_v, int row_elems,

@@ -82,19 +82,22 @@ struct Cfg {
     static constexpr int kStateOff = kMaxGroup * kRowPitch;       // m[8], l[8], lx[8] follow the rows
     static constexpr int kScratchFloatsPerWarp = kStateOff + 3 * kMaxGroup;
     // the scratch area doubles as merge.cuh's staging area (never live at the same time)
+    static constexpr int kS6ScratchBytes = kConsumerWarps * kScratchFloatsPerWarp * 4;
     static constexpr int kScratchBytes =
-        kConsumerWarps * kScratchFloatsPerWarp * 4 > MergeCfg<D>::kStageBytes
-            ? kConsumerWarps * kScratchFloatsPerWarp * 4 : MergeCfg<D>::kStageBytes;
+        kS6ScratchBytes > MergeCfg<D>::kStageBytes ? kS6ScratchBytes : MergeCfg<D>::kStageBytes;
     static constexpr int kKSteps = D / 16;  // QK^T k-steps == PV m-tiles
     static constexpr int kTilesPerPass = kFp8 ? COMEM_FP8_TILES_PER_PASS : 1;  // tiles a consumer warp takes per online-softmax update
 };
 
+// `fused`: the kernel also merges (S7) and needs merge.cuh's staging area; un-fused (the merge runs as the small
+// dependent kernel of combine.cu) it leaves that shared memory free, so that kernel's CTAs fit beside this one's.
 template <int D, bool kFp8>
-__host__ __device__ constexpr size_t smem_bytes_for(int batch)
+__host__ __device__ constexpr size_t smem_bytes_for(int batch, bool fused = true)
 {
     using C = Cfg<D, kFp8>;
-    return 1024 /* alignment slack */ + (size_t)C::kStages * C::kStageBytes + (size_t)C::kScratchBytes +
-           (2 * C::kStages + 1) * 8 + C::kScaleBytes + ((size_t)batch + 1) * 4 + 16;
+    return 1024 /* alignment slack */ + (size_t)C::kStages * C::kStageBytes +
+           (size_t)(fused ? C::kScratchBytes : C::kS6ScratchBytes) +
+           (2 * C::kStages + 2) * 8 + C::kScaleBytes + ((size_t)batch + 1) * 4 + 16;
 }
 
 struct SegPos {
@@ -132,12 +135,14 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     const uint32_t ring = (raw + 1023u) & ~1023u;  // 1024-aligned: the 128B-swizzle atom
     uint8_t *ring_ptr = smem_raw + (ring - raw);
     float *scratch = reinterpret_cast<float *>(ring_ptr + C::kStages * C::kStageBytes);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(scratch) + C::kScratchBytes);
-    const uint32_t scales0 = smem_u32(bars + 2 * C::kStages + 1);  // FP8 only: float2 per ring stage
-    int *prefix = reinterpret_cast<int *>(reinterpret_cast<uint8_t *>(bars + 2 * C::kStages + 1) + C::kScaleBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(scratch) +
+                                                  (p.fuse_combine ? C::kScratchBytes : C::kS6ScratchBytes));
+    const uint32_t scales0 = smem_u32(bars + 2 * C::kStages + 2);  // FP8 only: float2 per ring stage
+    int *prefix = reinterpret_cast<int *>(reinterpret_cast<uint8_t *>(bars + 2 * C::kStages + 2) + C::kScaleBytes);
     const uint32_t full0 = smem_u32(bars);
     const uint32_t empty0 = full0 + 8 * C::kStages;
     const uint32_t merge_bar = empty0 + 8 * C::kStages;  // completion of merge.cuh's bulk copies
+    const uint32_t verdict_bar = merge_bar + 8;          // early mode: the schedule guess has been validated (or not)
 
     // A CTA cuts at most two segments: its first (slot 0) and its last (slot 1; slot 0 if it has one segment only).
     // Per slot: {this CTA merges?, first record's kind, i_first, nsplit, arrival counter index, first output row}.
@@ -162,6 +167,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             mbar_init(empty0 + 8 * s, 1);
         }
         mbar_init(merge_bar, 1);
+        mbar_init(verdict_bar, 1);
         fence_mbar_init();
     }
     if (warp == kConsumerWarps && lane == 0) {  // first producer warp
@@ -281,54 +287,73 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         }
     };
     compute_schedule();  // speculative
-    // Still before the wait: ask the TMA unit to pull this CTA's first tiles into L2.  Cached KV rows
-    // of old tokens are immutable, so a prefetch from the guessed schedule and the block table as it
-    // reads now is at worst useless (the page index is clamped to the table row, a bad page id is an
-    // out-of-range tensor coordinate: both harmless for a hint).  HBM is idle while the previous
-    // kernel drains its tail; the first real loads after the wait then hit L2.
-    if (warp == kConsumerWarps && c0 < c1 && p.window <= 0) {  // (identity tile map only)
-        const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
-        const int64_t rem = c1 - c0;
-        int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
-        cnt = cnt < C::kPrefetch ? cnt : C::kPrefetch;
-        if (lane < cnt) {
-            const int jj = sp.j + lane;
-            int page = jj >> p.page_tile_shift;
-            page = page < p.max_pages ? page : p.max_pages - 1;
-            const int pid = __ldcg(p.block_table + (int64_t)sp.b * p.max_pages + page);
-            const int slot0 = (jj & ((1 << p.page_tile_shift) - 1)) << kTileShift;
-            // tensor coordinates of the tile: {d, token row, -, kv head}, or {d, slot, kv head, page} for the HND layout
-            const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid * p.page_size + slot0;
-            const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid : sp.kvh;
-            tma_prefetch_tile_4d(&tm_k, 0, c1, c2, c3);
-            tma_prefetch_tile_4d(&tm_v, 0, c1, c2, c3);
+    // EARLY MODE (COMEM_LAUNCH_KV_PREFIX_IMMUTABLE, p.kv_immutable): the caller has PROMISED that nothing still running
+    // writes the cached rows below each sequence's last tile, their block-table entries or their page scales.  Then
+    // this CTA does not sit in griddepcontrol.wait while the previous kernel drains: its producers stream those tiles
+    // NOW, from the guessed schedule, and -- with COMEM_LAUNCH_Q_STABLE (q is not being written either) -- its consumers
+    // fold them as they land.  The wait moves to the first point where the CTA needs something the previous kernel may
+    // still write or must not yet see written: a sequence's LAST tile (the append kernel's row), seq_lens itself, and
+    // any global store (S6).  That point is CTA-local tile index X: the sequence-last tile if the CTA's first segment
+    // portion ends with it, else the end of that portion (= the end of the CTA's range).  There, one producer warp
+    // waits for the previous grid, re-reads seq_lens, compares the tile counts with the guess and publishes the
+    // verdict on an mbarrier; everybody else picks it up when they get to X.  A wrong guess (a length crossed a tile
+    // boundary: once in 16 decode steps per sequence) aborts the attempt: what was streamed is dropped, the barriers
+    // are re-initialised and the CTA runs again in the classic order below.  Bits are the same in both modes: the
+    // schedule, the tile -> warp map and every reduction order are unchanged.
+    bool early = p.kv_immutable != 0 && p.window <= 0 && c0 < c1;
+    __shared__ int s_abort;
+    if (!early) {
+        // Classic order.  Still before the wait: ask the TMA unit to pull this CTA's first tiles into L2.  Cached KV
+        // rows of old tokens are immutable, so a prefetch from the guessed schedule and the block table as it reads
+        // now is at worst useless (the page index is clamped to the table row, a bad page id is an out-of-range
+        // tensor coordinate: both harmless for a hint).  HBM is idle while the previous kernel drains its tail; the
+        // first real loads after the wait then hit L2.
+        if (warp == kConsumerWarps && c0 < c1 && p.window <= 0) {  // (identity tile map only)
+            const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
+            const int64_t rem = c1 - c0;
+            int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
+            cnt = cnt < C::kPrefetch ? cnt : C::kPrefetch;
+            if (lane < cnt) {
+                const int jj = sp.j + lane;
+                int page = jj >> p.page_tile_shift;
+                page = page < p.max_pages ? page : p.max_pages - 1;
+                const int pid = __ldcg(p.block_table + (int64_t)sp.b * p.max_pages + page);
+                const int slot0 = (jj & ((1 << p.page_tile_shift) - 1)) << kTileShift;
+                // tensor coordinates of the tile: {d, token row, -, kv head}, or {d, slot, kv head, page} for the HND layout
+                const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid * p.page_size + slot0;
+                const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid : sp.kvh;
+                tma_prefetch_tile_4d(&tm_k, 0, c1, c2, c3);
+                tma_prefetch_tile_4d(&tm_v, 0, c1, c2, c3);
+            }
         }
-    }
-    pdl_wait_prior_grid();
-    COMEM_STAMP(1);
-    if (warp == 0) {  // validate the guess against the lengths as they are now
-        bool same = true;
+        pdl_wait_prior_grid();
+        COMEM_STAMP(1);
+        if (warp == 0) {  // validate the guess against the lengths as they are now
+            bool same = true;
 #pragma unroll 1
-        for (int b = lane; b < p.batch; b += 32)
-            same = same && seq_tiles(__ldcg(p.seq_lens + b), p.window, p.sinks) == prefix[b + 1] - prefix[b];
-        same = __all_sync(kFull, same);
-        if (lane == 0) s_valid = same ? 1 : 0;
-    }
+            for (int b = lane; b < p.batch; b += 32)
+                same = same && seq_tiles(__ldcg(p.seq_lens + b), p.window, p.sinks) == prefix[b + 1] - prefix[b];
+            same = __all_sync(kFull, same);
+            if (lane == 0) s_valid = same ? 1 : 0;
+        }
 #ifdef COMEM_TRACE
-    if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
-    if (p.trace && threadIdx.x == kConsumerThreads) p.trace[blockIdx.x * 16 + 12] = globaltimer_ns();
-    if (p.trace && threadIdx.x == 32) p.trace[blockIdx.x * 16 + 13] = globaltimer_ns();
+        if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
+        if (p.trace && threadIdx.x == kConsumerThreads) p.trace[blockIdx.x * 16 + 12] = globaltimer_ns();
+        if (p.trace && threadIdx.x == 32) p.trace[blockIdx.x * 16 + 13] = globaltimer_ns();
 #endif
-    __syncthreads();
-    if (!s_valid) {
-        __syncthreads();  // everyone has read s_valid and the old tables before warp 0 rewrites them
-        compute_schedule();
+        __syncthreads();
+        if (!s_valid) {
+            __syncthreads();  // everyone has read s_valid and the old tables before warp 0 rewrites them
+            compute_schedule();
+        }
     }
     pdl_launch_dependents();
     COMEM_STAMP(2);
 
+  for (;;) {  // one pass, or two when an early attempt is aborted
     // S8: rows of empty sequences (reading R9): +0.0 and lse = -inf, dealt round-robin to the CTAs.
-    if (p.fuse_combine) {
+    auto write_empty_rows = [&]() {
+        if (!p.fuse_combine) return;
         for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
             if (prefix[b + 1] != prefix[b]) continue;
             const int64_t row0 = (int64_t)b * p.num_q_heads;
@@ -336,8 +361,24 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             if (p.lse_out)
                 for (int h = threadIdx.x; h < p.num_q_heads; h += kThreads) p.lse_out[row0 + h] = -INFINITY;
         }
+    };
+    if (!early) {
+        write_empty_rows();
+        if (c0 >= c1) return;  // nothing to stream (no tiles at all, or more CTAs than the schedule uses)
     }
-    if (c0 >= c1) return;  // nothing to stream (no tiles at all, or more CTAs than the schedule uses)
+    // early mode: CTA-local index of the first tile that needs the wait (producers: xp, consumers: xc)
+    int xp = 0, xc = 0;
+    if (early) {
+        const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
+        const int64_t rem = c1 - c0;
+        const int cnt0 = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
+        const int x_wait = (sp.j + cnt0 == sp.T) ? cnt0 - 1 : cnt0;
+        // without COMEM_LAUNCH_Q_STABLE the consumers cannot start before the wait: the producers fill the ring once
+        // (no stage is reused, so they never block on the consumers) and ask for the verdict
+        xc = p.q_stable ? x_wait : 0;
+        xp = p.q_stable ? x_wait : (x_wait < C::kStages ? x_wait : C::kStages);
+    }
+    bool early_pending = early, aborted = false;
 
     if (warp >= kConsumerWarps) {
         // ------------------------------ S2: page-gather producers -----------------------------
@@ -354,83 +395,117 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         const int tiles_per_page_mask = (1 << p.page_tile_shift) - 1;
         int tl0 = 0;  // CTA-local index of the current segment's first tile
         int64_t x = c0;
-        while (x < c1) {
+        // Early mode: the wait, the validation of the guessed schedule and the verdict (see above).  Producer warp 0
+        // decides, the others read its verdict.
+        auto verdict = [&]() {
+            if (pw == 0) {
+                pdl_wait_prior_grid();
+                bool same = true;
+#pragma unroll 1
+                for (int b = lane; b < p.batch; b += 32)
+                    same = same && seq_tiles(__ldcg(p.seq_lens + b), p.window, p.sinks) == prefix[b + 1] - prefix[b];
+                same = __all_sync(kFull, same);
+                if (lane == 0) {
+                    *reinterpret_cast<volatile int *>(&s_abort) = same ? 0 : 1;
+                    mbar_arrive(verdict_bar);  // release: s_abort is visible to whoever waits on the barrier
+                }
+                aborted = !same;
+            } else {
+                mbar_wait(verdict_bar, 0u);
+                pdl_wait_prior_grid();
+                aborted = *reinterpret_cast<volatile int *>(&s_abort) != 0;
+            }
+            early_pending = false;
+#ifdef COMEM_TRACE
+            if (p.trace && threadIdx.x == kConsumerThreads) p.trace[blockIdx.x * 16 + 14] = globaltimer_ns();
+#endif
+        };
+        while (x < c1 && !aborted) {
             const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
             const int64_t rem = c1 - x;
             const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
             const int32_t *bt = p.block_table + (int64_t)sp.b * p.max_pages;
             // sequence tile index -> logical tile (identity unless a sliding window is set)
             const WinTiles wt = win_tiles(p.window > 0 ? __ldcg(p.seq_lens + sp.b) : 0, p.window, p.sinks);
-            // The per-tile metadata (block-table entry, then -- FP8 -- the page's two scales, which depend on it)
-            // is fetched 32 tiles at a time, one tile per lane, and kept TWO batches ahead of the tiles being
-            // issued: a batch's loads are in flight while the previous batches' TMAs are issued, so the dependent
-            // round trips to L2 / DRAM never stop the issue loop (they did: half of the producers' samples).
-            auto load_pid = [&](int base) -> int {
-                if (base + lane >= cnt) return 0;
-                return __ldg(bt + (win_logical_tile(wt, sp.j + base + lane) >> p.page_tile_shift));
-            };
-            auto load_scales = [&](int base, int pid, float &ks, float &vs) {
-                ks = vs = 0.f;
-                if constexpr (kFp8) {
-                    if (base + lane < cnt) {
-                        ks = __ldg(p.k_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
-                        vs = __ldg(p.v_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
-                    }
-                }
-            };
-            // (bf16: one L2-latency load per 32 tiles of 8 KiB is covered by the ring, and a short CTA -- config 2
-            // has ~110 tiles -- is better off with the shortest path to its first TMA: measured, so not pipelined.)
-            constexpr bool kMetaAhead = kFp8;
-            int pid = kMetaAhead ? load_pid(0) : 0, pid_next = kMetaAhead ? load_pid(32) : 0;
-            float ks = 0.f, vs = 0.f;  // FP8: the page's scales for this kv head
-            if constexpr (kMetaAhead) load_scales(0, pid, ks, vs);
-            for (int base = 0; base < cnt; base += 32) {
-                float ks_next = 0.f, vs_next = 0.f;
-                int pid_next2 = 0;
-                if constexpr (kMetaAhead) {
-                    load_scales(base + 32, pid_next, ks_next, vs_next);
-                    pid_next2 = load_pid(base + 64);
-                } else {
-                    pid = load_pid(base);
-                }
-                const int jj = win_logical_tile(wt, sp.j + base + lane);
-                const int m = cnt - base < 32 ? cnt - base : 32;
-                for (int i = (pw - (tl0 + base)) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
-                    const int tl = tl0 + base + i;
-                    const int stage = tl & (C::kStages - 1);
-                    const uint32_t phase = (uint32_t)(tl >> kStageShift) & 1u;
-                    mbar_wait(empty0 + 8 * stage, phase ^ 1u);
-                    const int pid_i = __shfl_sync(kFull, pid, i);
-                    const int jj_i = __shfl_sync(kFull, jj, i);
-                    float ks_i = 0.f, vs_i = 0.f;
+            // issue the segment's tiles [lo, hi) (indices within this CTA's portion of the segment)
+            auto issue_range = [&](const int lo, const int hi) {
+                // The per-tile metadata (block-table entry, then -- FP8 -- the page's two scales, which depend on it)
+                // is fetched 32 tiles at a time, one tile per lane, and kept TWO batches ahead of the tiles being
+                // issued: a batch's loads are in flight while the previous batches' TMAs are issued, so the dependent
+                // round trips to L2 / DRAM never stop the issue loop (they did: half of the producers' samples).
+                auto load_pid = [&](int base) -> int {
+                    if (base + lane >= hi) return 0;
+                    return __ldg(bt + (win_logical_tile(wt, sp.j + base + lane) >> p.page_tile_shift));
+                };
+                auto load_scales = [&](int base, int pid, float &ks, float &vs) {
+                    ks = vs = 0.f;
                     if constexpr (kFp8) {
-                        ks_i = __shfl_sync(kFull, ks, i);
-                        vs_i = __shfl_sync(kFull, vs, i);
+                        if (base + lane < hi) {
+                            ks = __ldg(p.k_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
+                            vs = __ldg(p.v_scale + (int64_t)pid * p.num_kv_heads + sp.kvh);
+                        }
                     }
-                    if (lane == 0) {
-                        const int slot0 = (jj_i & tiles_per_page_mask) << kTileShift;
-                        const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid_i * p.page_size + slot0;
-                        const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid_i : sp.kvh;
-                        const uint32_t dst = ring + stage * C::kStageBytes;
-                        const uint32_t bar = full0 + 8 * stage;
-                        if constexpr (kFp8)  // ordered before the consumers' wait by the arrive below (release) and their wait (acquire)
-                            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(scales0 + 8 * stage), "f"(ks_i), "f"(vs_i) : "memory");
-                        mbar_arrive_expect_tx(bar, C::kStageBytes);
-                        tma_load_4d_hint(dst, &tm_k, bar, 0, c1, c2, c3, stream_policy);
-                        tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, c1, c2, c3, stream_policy);
+                };
+                // (bf16: one L2-latency load per 32 tiles of 8 KiB is covered by the ring, and a short CTA -- config 2
+                // has ~110 tiles -- is better off with the shortest path to its first TMA: measured, so not pipelined.)
+                constexpr bool kMetaAhead = kFp8;
+                int pid = kMetaAhead ? load_pid(lo) : 0, pid_next = kMetaAhead ? load_pid(lo + 32) : 0;
+                float ks = 0.f, vs = 0.f;  // FP8: the page's scales for this kv head
+                if constexpr (kMetaAhead) load_scales(lo, pid, ks, vs);
+                for (int base = lo; base < hi; base += 32) {
+                    float ks_next = 0.f, vs_next = 0.f;
+                    int pid_next2 = 0;
+                    if constexpr (kMetaAhead) {
+                        load_scales(base + 32, pid_next, ks_next, vs_next);
+                        pid_next2 = load_pid(base + 64);
+                    } else {
+                        pid = load_pid(base);
                     }
+                    const int jj = win_logical_tile(wt, sp.j + base + lane);
+                    const int m = hi - base < 32 ? hi - base : 32;
+                    for (int i = (pw - (tl0 + base)) & (kProducerWarps - 1); i < m; i += kProducerWarps) {
+                        const int tl = tl0 + base + i;
+                        const int stage = tl & (C::kStages - 1);
+                        const uint32_t phase = (uint32_t)(tl >> kStageShift) & 1u;
+                        mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                        const int pid_i = __shfl_sync(kFull, pid, i);
+                        const int jj_i = __shfl_sync(kFull, jj, i);
+                        float ks_i = 0.f, vs_i = 0.f;
+                        if constexpr (kFp8) {
+                            ks_i = __shfl_sync(kFull, ks, i);
+                            vs_i = __shfl_sync(kFull, vs, i);
+                        }
+                        if (lane == 0) {
+                            const int slot0 = (jj_i & tiles_per_page_mask) << kTileShift;
+                            const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid_i * p.page_size + slot0;
+                            const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid_i : sp.kvh;
+                            const uint32_t dst = ring + stage * C::kStageBytes;
+                            const uint32_t bar = full0 + 8 * stage;
+                            if constexpr (kFp8)  // ordered before the consumers' wait by the arrive below (release) and their wait (acquire)
+                                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(scales0 + 8 * stage), "f"(ks_i), "f"(vs_i) : "memory");
+                            mbar_arrive_expect_tx(bar, C::kStageBytes);
+                            tma_load_4d_hint(dst, &tm_k, bar, 0, c1, c2, c3, stream_policy);
+                            tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, c1, c2, c3, stream_policy);
+                        }
+                    }
+                    pid = pid_next;
+                    pid_next = pid_next2;
+                    ks = ks_next;
+                    vs = vs_next;
                 }
-                pid = pid_next;
-                pid_next = pid_next2;
-                ks = ks_next;
-                vs = vs_next;
+            };
+            int lo = 0;
+            if (early_pending) {  // (first segment only: xp lies inside it)
+                lo = xp - tl0 < cnt ? xp - tl0 : cnt;
+                issue_range(0, lo);
+                verdict();
+                if (aborted) break;
             }
+            issue_range(lo, cnt);
             x += cnt;
             tl0 += cnt;
         }
-        return;
-    }
-
+    } else {
     // ------------------------------ consumers: S3..S6 -----------------------------------------
     const int quad = lane >> 2;  // score row = query head within the group
     const int qlane = lane & 3;
@@ -478,6 +553,14 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             merge_partials<D>(p, warp, lane, s_seg[cur_slot][1], s_seg[cur_slot][2], s_seg[cur_slot][3],
                               (int64_t)s_seg[cur_slot][5], scratch, merge_bar, merge_phase);
     };
+    // early mode: pick up the producers' verdict (the previous grid has completed, the guessed schedule holds or not)
+    auto need_verdict = [&]() {
+        mbar_wait(verdict_bar, 0u);
+        pdl_wait_prior_grid();
+        aborted = *reinterpret_cast<volatile int *>(&s_abort) != 0;
+        early_pending = false;
+        COMEM_STAMP(1);
+    };
     int64_t x = c0;
     int n = 0;        // CTA-local index of the segment's first tile
     int t = warp;     // this warp's next tile (CTA-local index)
@@ -485,6 +568,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     uint32_t phase = 0;
 
     while (x < c1) {
+        if (early_pending && xc <= n) {  // nothing of this segment may be touched before the wait (q included)
+            need_verdict();
+            if (aborted) break;
+        }
         const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
         const int64_t rem = c1 - x;
         const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
@@ -506,8 +593,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             sg[4] = sp.b * p.num_kv_heads + sp.kvh;
             sg[5] = sp.b * p.num_q_heads + sp.kvh * p.group;
         }
-        const int seq_len = __ldcg(p.seq_lens + sp.b);
-        const WinTiles wt = win_tiles(seq_len, p.window, p.sinks);
+        // (early mode, before the verdict: possibly the length before the append -- it only decides the mask of the
+        // sequence's last tile, which is not touched until the verdict is in and the length re-read)
+        int seq_len = __ldcg(p.seq_lens + sp.b);
+        WinTiles wt = win_tiles(seq_len, p.window, p.sinks);
         const int head0 = sp.kvh * p.group;
 
         // Q fragments (A operand of S = Q K^T): row = head `quad`, rows 8..15 are zero padding.
@@ -553,6 +642,12 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // with half the bytes per tile, a single chain per warp is latency-bound below the HBM rate.
         auto tiles_pass = [&](auto nt_tag) {
             constexpr int NT = decltype(nt_tag)::value;
+            if (early_pending && t + (NT - 1) * kConsumerWarps >= xc) {
+                need_verdict();
+                if (aborted) return;
+                seq_len = __ldcg(p.seq_lens + sp.b);
+                wt = win_tiles(seq_len, p.window, p.sinks);
+            }
             uint32_t k_base[NT], v_base[NT];
             unsigned alive[NT];
             int stg[NT];
@@ -785,9 +880,11 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             t += NT * kConsumerWarps;
         };
         if constexpr (C::kTilesPerPass == 2) {
-            while (t + kConsumerWarps < n + cnt) tiles_pass(std::integral_constant<int, 2>{});
+            while (t + kConsumerWarps < n + cnt && !aborted) tiles_pass(std::integral_constant<int, 2>{});
         }
-        while (t < n + cnt) tiles_pass(std::integral_constant<int, 1>{});
+        while (t < n + cnt && !aborted) tiles_pass(std::integral_constant<int, 1>{});
+        if (early_pending) need_verdict();  // S6 stores to global memory
+        if (aborted) break;
 
         // S6: merge the consumer warps' states (warp-index order) and write the row or a partial.
         // Scratch layout per warp: acc as [head][D + 4] (the +4 pad makes both the fragment
@@ -893,7 +990,37 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         x += cnt;
         n += cnt;
     }
-    if (pending_first) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
+    if (pending_first && !aborted) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
+    if (aborted) {
+        // every tile the producers issued before the verdict must have landed before the barriers are re-initialised:
+        // this warp's share of them that it has not consumed
+        for (int tt = t; tt < xp; tt += kConsumerWarps)
+            mbar_wait(full0 + 8 * (tt & (C::kStages - 1)), (uint32_t)(tt / C::kStages) & 1u);
+    }
+    }  // consumers
+    if (!early) return;
+    // End of an early attempt: all threads meet; either it went through (the empty rows are still to write: global
+    // stores, so after the wait every thread has passed by now), or the guess was wrong and the CTA starts over in
+    // the classic order with fresh barriers and the real schedule.
+    __syncthreads();
+    if (*reinterpret_cast<volatile int *>(&s_abort) == 0) {
+        write_empty_rows();
+        return;
+    }
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_inval(full0 + 8 * s);
+            mbar_inval(empty0 + 8 * s);
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 1);
+        }
+        mbar_inval(merge_bar);
+        mbar_init(merge_bar, 1);
+        fence_mbar_init();
+    }
+    compute_schedule();  // (its barrier also publishes the fresh mbarriers)
+    early = false;
+  }  // attempts
 }
 
 template <int D, bool kFp8>
@@ -930,7 +1057,7 @@ static cudaError_t launch_variant(const CUtensorMap &tm_k, const CUtensorMap &tm
     const cudaError_t e = configure_once<D, kFp8>();
     if (e != cudaSuccess) return e;
     cfg.blockDim = dim3(Cfg<D, kFp8>::kThreads);
-    cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch);
+    cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch, p.fuse_combine != 0);
     return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8>, tm_k, tm_v, p);
 }
 

@@ -17,6 +17,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t arrivals)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(arrivals) : "memory");
 }
+__device__ __forceinline__ void mbar_inval(uint32_t bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void fence_mbar_init()
 {
     // make barrier initialisation visible to the async (TMA) proxy

@@ -16,7 +16,7 @@ from paper_2605_30842_b200 import workloads as W
 MAX_ABS, MEAN_ABS, REL_L2 = 2e-2, 2e-3, 5e-3
 
 
-def gpu_run(batch: W.DecodeBatch, want_lse: bool = True, stream=None, workspace=None):
+def gpu_run(batch: W.DecodeBatch, want_lse: bool = True, stream=None, workspace=None, flags: int = 0):
     """One decode-attention step through the C-ABI on the current device. Returns (out, lse) tensors."""
     assert batch.q.is_cuda
     out = torch.full_like(batch.q, float("nan"))
@@ -25,7 +25,7 @@ def gpu_run(batch: W.DecodeBatch, want_lse: bool = True, stream=None, workspace=
     ws = workspace if workspace is not None else comem.alloc_workspace(batch.q, batch.k_pages, batch.block_table,
                                                                         stream=stream)
     comem.comem_decode_attn_async(batch.q, batch.k_pages, batch.v_pages, batch.block_table,
-                                  batch.seq_lens, batch.softmax_scale, out, ws, lse_out=lse, stream=stream)
+                                  batch.seq_lens, batch.softmax_scale, out, ws, lse_out=lse, stream=stream, flags=flags)
     return out, lse
 
 
@@ -85,8 +85,8 @@ def assert_parity(err, what=""):
     assert err["max_abs"] <= 4 * 2.0 ** -9 * err["max_ref"] + 1e-6, (what, err)
 
 
-def check_batch(oracle, batch: W.DecodeBatch, pairs=None, what="", lse_tol=2e-4):
-    out, lse = gpu_run(batch)
+def check_batch(oracle, batch: W.DecodeBatch, pairs=None, what="", lse_tol=2e-4, flags: int = 0):
+    out, lse = gpu_run(batch, flags=flags)
     torch.cuda.synchronize()
     pairs = pairs if pairs is not None else all_pairs(batch)
     ref, ref_lse = oracle_rows(oracle, batch, pairs)
