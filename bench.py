@@ -46,7 +46,7 @@ L2_BYTES_NOMINAL = 126e6
 
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 # COMEM_LAUNCH_* bits the decode workloads are launched with unless --launch-flags says otherwise
-DEFAULT_LAUNCH_FLAGS = 0
+DEFAULT_LAUNCH_FLAGS = 5  # KV_PREFIX_IMMUTABLE | Q_STABLE: nothing in the timed loops writes the cache prefix or q
 
 
 def kernel_source_sha() -> str:
@@ -218,8 +218,8 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
                 device, flags=0):
     """`warmup` untimed steps, then EXACTLY `steps` steps on `stream`, bracketed by barrier +
     synchronize on both sides; CUDA events on that stream.  With graphs (the default) every timed step is
-    replayed from a CUDA graph whatever `steps` is: steps = a * R + r runs as a replays of an R-step graph and one
-    replay of an r-step graph (R = number of rotating pools).  Returns this rank's milliseconds."""
+    replayed from a CUDA graph whatever `steps` is: steps = a * C + r runs as a replays of a C-step graph and one
+    replay of an r-step graph, C = min(steps, 1024) (the pools rotate inside the graph).  Returns this rank's milliseconds."""
     R = len(pools)
 
     def enqueue(first, n):
@@ -238,9 +238,12 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
     with torch.cuda.stream(stream):
         enqueue(0, max(warmup, 3))
         stream.synchronize()
-        a, r = divmod(steps, R) if use_graph else (0, 0)
-        g_full = capture(0, R) if a else None
-        g_rest = capture(a * R, r) if r else None
+        # one graph for the whole timed region when it is short (no graph-launch boundary inside it: consecutive
+        # steps overlap through programmatic launch only inside a graph); 1 024-step graphs for long runs
+        chunk = min(steps, 1024)
+        a, r = divmod(steps, chunk) if use_graph else (0, 0)
+        g_full = capture(0, chunk) if a else None
+        g_rest = capture(a * chunk, r) if r else None
         sampler.warm = True          # the run-up: same kernels, same rate as the timed region
         for g in (g_full, g_rest):
             if g is not None:
@@ -1036,7 +1039,7 @@ def measure_decode(ctx, name, steps, warmup, *, primary):
            "launch_flags": res_flags}
     if primary:
         ms_split = timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup,
-                               comem.COMEM_PHASE_SPLIT, use_graph, sampler, device, flags=flags & 1)
+                               comem.COMEM_PHASE_SPLIT, use_graph, sampler, device, flags=flags & 5)
         res["ms_split_max"] = replicas.max_over_ranks(ms_split, device)
         res["dist"] = step_distribution(torch, comem, pools, outs, ws, stream, 200 if name == "c2" else 20, both)
         # a sustained run of the same steps (seconds-scale thermals and the power cap show only here)
