@@ -94,6 +94,8 @@ def parse_args():
     ap.add_argument("--pipeline", type=int, default=0, metavar="K",
                     help="extra: drive 64 agent steps of the k-step-off pipeline (Algorithm 1) from comem_kstep_plan "
                          "and check eq. 5 against the measured decode-attention times")
+    ap.add_argument("--offload", action="store_true",
+                    help="extra: decode attention over the two-tier (HBM + pinned host) cache; prints its own line")
     ap.add_argument("--prefill", action="store_true",
                     help="extra: time comem_prefill_attn_async (paged causal prefill, tcgen05) and print its own line")
     ap.add_argument("--primary-only", action="store_true",
@@ -676,6 +678,57 @@ def run_window(args) -> int:
     return 0
 
 
+def run_offload(args) -> int:
+    """Extra: decode attention over the two-tier cache.  The C3 agent batch
+    with the coldest 0 / 5 / 10 / 25 / 50 % of every sequence's pages in pinned host memory: us/step, and the rate at
+    which the host-resident bytes crossed the host link.  One JSON line; not the driver's bench line."""
+    import torch
+    import paper_2605_30842_b200 as comem
+    from paper_2605_30842_b200 import build as cuda_build
+    from paper_2605_30842_b200 import workloads as W
+
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(device)
+    cuda_build.build()
+    comem.load_library()
+    b = W.config3_agent_ragged(device)
+    stream = torch.cuda.Stream(device)
+    rows = []
+    ref_out = None
+    for frac in (0.0, 0.05, 0.10, 0.25, 0.50):
+        ob = W.offload_pages(b, frac, seed=11)
+        bb = ob.base
+        out = torch.empty_like(bb.q)
+        ws = comem.alloc_workspace(bb.q, bb.k_pages, bb.block_table, stream=stream)
+        with torch.cuda.stream(stream):
+            f = lambda: comem.comem_decode_attn_offload_async(bb.q, bb.k_pages, bb.v_pages, ob.k_host, ob.v_host,  # noqa: E731
+                                                              bb.block_table, bb.seq_lens, bb.softmax_scale, out, ws,
+                                                              stream=stream)
+            for _ in range(2):
+                f()
+            stream.synchronize()
+            n = max(3, min(args.steps, 10))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(n):
+                f()
+            e1.record(stream)
+            stream.synchronize()
+        us = e0.elapsed_time(e1) / n * 1e3
+        if ref_out is None:
+            ref_out = out.clone()
+        same = bool(torch.equal(out.view(torch.int16), ref_out.view(torch.int16)))
+        rows.append({"host_fraction": frac, "host_bytes_per_step": ob.host_bytes(), "us_per_step": us,
+                     "host_link_gbs": (ob.host_bytes() / us / 1e3) if ob.host_bytes() else None,
+                     "total_gbs": b.algorithmic_bytes() / us / 1e3, "bits_equal_all_hbm": same})
+        del ob, bb, out, ws
+    print(json.dumps({"extra": "two-tier cache (HBM + pinned host memory), C3 agent batch, coldest pages offloaded",
+                      "algorithmic_bytes_per_step": b.algorithmic_bytes(), "rows": rows,
+                      "note": "host-resident tiles are TMA-loaded over the host link straight into shared memory, once per step"}),
+          flush=True)
+    return 0
+
+
 def fp8_parity(fb, gpu_out, seq: int = 0):
     """Oracle (oracle.decode_attn_fp8, all host cores) on ONE whole sequence of the FP8 batch, all its query heads,
     from the same bytes and scales; returns (parity block, oracle seconds)."""
@@ -1157,6 +1210,8 @@ def main() -> int:
         return run_reference(args, rank)
     if args.window > 0:
         return run_window(args) if rank == 0 else 0
+    if args.offload:
+        return run_offload(args) if rank == 0 else 0
     if args.pipeline > 0:
         return run_pipeline(args) if rank == 0 else 0
     if args.kv_fp8:

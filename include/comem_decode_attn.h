@@ -209,6 +209,40 @@ int comem_decode_attn_fp8_async(const void *q, const void *k_pages, const void *
                                 int kv_layout, const comem_launch_opts *opts);
 
 /*
+ * comem_decode_attn_offload_async — the decode step over a TWO-TIER cache: part of the pages live in HBM, the cold part
+ * in pinned host memory ("part of the KV cache will be either emitted or offloaded to CPU ... CPU offload is often a
+ * better strategy"; every latency result of the paper is reported with and without CPU offloading, P:L245,
+ * Table 1).  Nothing is copied back first: the page-gather loader issues the same TMA tile load against a
+ * second tensor map over the host pool, so a host-resident page crosses the host link exactly once, straight into
+ * shared memory, interleaved with the HBM-resident pages of the same sequence.
+ *   k_pages_host, v_pages_host   bf16 [num_pages_host][page_size][num_kv_heads][head_dim], HOST pointers to pinned,
+ *                    device-mapped memory (cudaHostAlloc / cudaHostRegister; torch's pin_memory()), 128-byte aligned
+ *   block_table      entry e >= 0: physical page e of the device pool (k_pages / v_pages);
+ *                    entry e <  0: physical page -1 - e of the host pool
+ * Everything else -- q, out, lse_out, seq_lens, workspace, stream, launch options, determinism (bit-identical results
+ * wherever a page lives: placement never enters the arithmetic) and the error contract -- as comem_decode_attn_async.
+ * bf16 cache, full attention (no window) in this version.  COMEM_ERR_INVALID_ARG if a host pool is not pinned + mapped.
+ */
+int comem_decode_attn_offload_async(const void *q, const void *k_pages, const void *v_pages,
+                                    const void *k_pages_host, const void *v_pages_host,
+                                    const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                    int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
+                                    int batch, int max_pages_per_seq, int64_t num_pages, int64_t num_pages_host,
+                                    float *lse_out, void *workspace, size_t workspace_bytes, void *cuda_stream,
+                                    const comem_launch_opts *opts);
+
+/*
+ * comem_pages_copy_async — move whole pages between two pools of the same page shape (HBM <-> pinned host memory:
+ * offloading cold pages, bringing them back; or compaction inside one tier).  For i in [0, n_pages): page src_ids[i] of
+ * (k_src, v_src) is copied to page dst_ids[i] of (k_dst, v_dst); src_ids / dst_ids are device int32 arrays; pools may
+ * be device pointers or pinned, device-mapped host pointers; page_bytes = page_size * num_kv_heads * head_dim * element
+ * size, a multiple of 16.  One kernel on `cuda_stream` (it reads and writes host memory itself: no copy engine, no
+ * per-page cudaMemcpy); the caller updates the block table.  Destination pages must be distinct.
+ */
+int comem_pages_copy_async(const void *k_src, const void *v_src, void *k_dst, void *v_dst, const int32_t *src_ids,
+                           const int32_t *dst_ids, int n_pages, size_t page_bytes, void *cuda_stream);
+
+/*
  * comem_kv_append_fp8_async — comem_kv_append_async for the FP8 cache of comem_decode_attn_fp8_async (P:L61 for
  * reading R18's cache): the new token's bf16 K row of kv head h is stored as
  *     byte = e4m3( (float)new_k[b][h][d] / k_scale[pid][h] )      pid = block_table[b][seq_lens[b] / page_size]

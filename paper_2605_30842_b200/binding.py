@@ -58,6 +58,11 @@ def load_library():
     lib.comem_decode_attn_fp8_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                                 i32, i64, vp, vp, sz, vp, i32, i32, i32, vp]
     lib.comem_decode_attn_fp8_async.restype = i32
+    lib.comem_decode_attn_offload_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
+                                                    i64, i64, vp, vp, sz, vp, vp]
+    lib.comem_decode_attn_offload_async.restype = i32
+    lib.comem_pages_copy_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, sz, vp]
+    lib.comem_pages_copy_async.restype = i32
     lib.comem_prefill_attn_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i32,
                                              i64, vp, vp, vp]
     lib.comem_prefill_attn_async.restype = i32
@@ -359,6 +364,41 @@ def comem_decode_attn_fp8_async(q, k_pages, v_pages, k_scale, v_scale, block_tab
         _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_fp8_async")
+
+
+def comem_decode_attn_offload_async(q, k_pages, v_pages, k_host, v_host, block_table, seq_lens, softmax_scale: float,
+                                    out, workspace, lse_out=None, stream=None, grid_ctas=None,
+                                    programmatic_launch=None, flags: int = 0) -> None:
+    """Decode attention over a two-tier cache: block-table entries < 0 address pages of the pinned host pools
+    (k_host, v_host: CPU tensors from .pin_memory()), entries >= 0 the device pools.  One fused launch."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    for t in (k_host, v_host):
+        assert (not t.is_cuda) and t.is_pinned() and t.dtype == torch.bfloat16 and t.is_contiguous() and t.dim() == 4
+        assert tuple(t.shape[1:]) == tuple(k_pages.shape[1:])
+    assert k_host.shape == v_host.shape
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_offload_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(k_host), _ptr(v_host), _ptr(block_table), _ptr(seq_lens),
+        q.shape[1], k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], k_host.shape[0], _ptr(lse_out), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream), _opts(grid_ctas, programmatic_launch, flags))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_offload_async")
+
+
+def comem_pages_copy_async(k_src, v_src, k_dst, v_dst, src_ids, dst_ids, stream=None) -> None:
+    """Copy pages src_ids[i] of (k_src, v_src) to pages dst_ids[i] of (k_dst, v_dst); pools are CUDA tensors or pinned
+    CPU tensors of the same page shape; the id arrays are int32 CUDA tensors."""
+    for t in (k_src, v_src, k_dst, v_dst):
+        assert t.is_contiguous() and t.dim() == 4 and (t.is_cuda or t.is_pinned())
+        assert tuple(t.shape[1:]) == tuple(k_src.shape[1:]) and t.dtype == k_src.dtype
+    assert src_ids.is_cuda and dst_ids.is_cuda and src_ids.dtype == torch.int32 and dst_ids.dtype == torch.int32
+    assert src_ids.is_contiguous() and dst_ids.is_contiguous() and src_ids.shape == dst_ids.shape and src_ids.dim() == 1
+    page_bytes = k_src[0].numel() * k_src.element_size()
+    st = load_library().comem_pages_copy_async(_ptr(k_src), _ptr(v_src), _ptr(k_dst), _ptr(v_dst), _ptr(src_ids),
+                                               _ptr(dst_ids), src_ids.numel(), page_bytes, _stream(stream))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_pages_copy_async")
 
 
 def comem_kv_append_fp8_async(k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, new_k, new_v,

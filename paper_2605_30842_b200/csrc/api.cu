@@ -414,7 +414,9 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
                             float *lse_out, void *workspace, size_t workspace_bytes,
                             void *cuda_stream, int phases, int window, int sink_tokens,
                             const comem_launch_opts *opts, const float *k_scale = nullptr,
-                            const float *v_scale = nullptr, bool kv_fp8 = false, int kv_layout = COMEM_KV_LAYOUT_NHD)
+                            const float *v_scale = nullptr, bool kv_fp8 = false, int kv_layout = COMEM_KV_LAYOUT_NHD,
+                            const void *k_pages_host = nullptr, const void *v_pages_host = nullptr,
+                            int64_t num_pages_host = 0)
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
     if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
@@ -436,8 +438,20 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     const int hnd = kv_layout == COMEM_KV_LAYOUT_HND ? 1 : 0;
     if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k, elem_bytes, hnd)) != COMEM_OK) return st;
     if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v, elem_bytes, hnd)) != COMEM_OK) return st;
+    // second tier ("offloaded to CPU"): pools of the same layout in pinned, device-mapped host memory
+    CUtensorMap tm_kh, tm_vh;
+    const bool host_tier = k_pages_host != nullptr;
+    if (host_tier) {
+        if (kv_fp8 || !v_pages_host || num_pages_host <= 0 || phases != (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) return COMEM_ERR_INVALID_ARG;
+        if (num_pages_host * page_size >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
+        const void *dk = device_alias(k_pages_host), *dv = device_alias(v_pages_host);
+        if (!dk || !dv || !aligned(dk, 128) || !aligned(dv, 128)) return COMEM_ERR_INVALID_ARG;  // not pinned + mapped
+        if ((st = get_tensor_map(dk, num_pages_host, page_size, num_kv_heads, head_dim, &tm_kh)) != COMEM_OK) return st;
+        if ((st = get_tensor_map(dv, num_pages_host, page_size, num_kv_heads, head_dim, &tm_vh)) != COMEM_OK) return st;
+    }
 
     DecodeParams p;
+    p.host_tier = host_tier ? 1 : 0;
     p.k_scale = kv_fp8 ? k_scale : nullptr;
     p.v_scale = kv_fp8 ? v_scale : nullptr;
     p.kv_hnd = hnd;
@@ -476,7 +490,9 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     if ((st = grid_for(head_dim, &p.grid_ctas, opts)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    if ((phases & COMEM_PHASE_SPLIT) && launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8) != cudaSuccess) {
+    if ((phases & COMEM_PHASE_SPLIT) &&
+        launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8, host_tier ? &tm_kh : nullptr,
+                            host_tier ? &tm_vh : nullptr) != cudaSuccess) {
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }
@@ -544,6 +560,48 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                                           head_dim, page_size, softmax_scale, out, batch, max_pages_per_seq,
                                           num_pages, lse_out, workspace, workspace_bytes, cuda_stream,
                                           COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE, opts);
+}
+
+int comem_decode_attn_offload_async(const void *q, const void *k_pages, const void *v_pages, const void *k_pages_host,
+                                    const void *v_pages_host, const int32_t *block_table, const int32_t *seq_lens,
+                                    int num_q_heads, int num_kv_heads, int head_dim, int page_size, float softmax_scale,
+                                    void *out, int batch, int max_pages_per_seq, int64_t num_pages,
+                                    int64_t num_pages_host, float *lse_out, void *workspace, size_t workspace_bytes,
+                                    void *cuda_stream, const comem_launch_opts *opts)
+{
+    if (!k_pages_host || !v_pages_host) return COMEM_ERR_INVALID_ARG;
+    return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim, page_size,
+                            softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out, workspace, workspace_bytes,
+                            cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE, 0, 0, opts, nullptr, nullptr, false,
+                            COMEM_KV_LAYOUT_NHD, k_pages_host, v_pages_host, num_pages_host);
+}
+
+int comem_pages_copy_async(const void *k_src, const void *v_src, void *k_dst, void *v_dst, const int32_t *src_ids,
+                           const int32_t *dst_ids, int n_pages, size_t page_bytes, void *cuda_stream)
+{
+    if (!k_src || !v_src || !k_dst || !v_dst || !src_ids || !dst_ids || n_pages < 0 || page_bytes == 0 || page_bytes % 16)
+        return COMEM_ERR_INVALID_ARG;
+    if (n_pages == 0) return COMEM_OK;
+    if (n_pages > 65535 * 1024) return COMEM_ERR_UNSUPPORTED;
+    const int st = check_device();
+    if (st != COMEM_OK) return st;
+    // a pinned host pool is addressed through its device alias; a device pointer is used as it is
+    auto resolve = [](const void *p) -> void * {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        if (at.type == cudaMemoryTypeHost) return at.devicePointer;
+        if (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) return const_cast<void *>(p);
+        return nullptr;  // pageable host memory
+    };
+    void *ks = resolve(k_src), *vs = resolve(v_src), *kd = resolve(k_dst), *vd = resolve(v_dst);
+    if (!ks || !vs || !kd || !vd || !aligned(ks, 16) || !aligned(vs, 16) || !aligned(kd, 16) || !aligned(vd, 16))
+        return COMEM_ERR_INVALID_ARG;
+    if (launch_pages_copy(ks, vs, kd, vd, src_ids, dst_ids, n_pages, page_bytes,
+                          static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return COMEM_OK;
 }
 
 int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_pages, const int32_t *block_table,

@@ -40,6 +40,7 @@ struct DecodeParams {
                                  // grid starts writes K/V rows (or their block-table entries / page scales) below each
                                  // sequence's last 16-token tile, so the ring may be filled before griddepcontrol.wait
     int q_stable;                // COMEM_LAUNCH_Q_STABLE: ... nor q: the consumers may start before the wait too
+    int host_tier;               // a second pool in pinned host memory is addressed by block-table entries < 0 (bf16 only)
     int kv_hnd;                  // FP8 cache only: pools laid out [P][Hkv][ps][D] (a tile is 2 KiB contiguous) instead of [P][ps][Hkv][D]
 };
 
@@ -65,7 +66,8 @@ inline cudaError_t set_max_smem_once(Kernel kernel, int bytes, PerDeviceOnce &on
 // launchers (defined in decode_split.cu / combine.cu / kv_append.cu)
 // kv_fp8: the pools hold E4M3 bytes and p.k_scale / p.v_scale are set
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
-                                const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false);
+                                const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false,
+                                const CUtensorMap *tm_k_host = nullptr, const CUtensorMap *tm_v_host = nullptr);
 cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
 // the small dependent combine (COMEM_LAUNCH_SPLIT_COMBINE; batch * Hkv <= kAlignedMaxSegs)
 cudaError_t launch_combine_small(const DecodeParams &p, int head_dim, cudaStream_t stream);
@@ -79,6 +81,8 @@ cudaError_t launch_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float
                                  const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
                                  const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
                                  int max_pages, int hnd, cudaStream_t stream);
+cudaError_t launch_pages_copy(const void *k_src, const void *v_src, void *k_dst, void *v_dst, const int32_t *src_ids,
+                              const int32_t *dst_ids, int n_pages, size_t page_bytes, cudaStream_t stream);
 cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,
                             int page_size, int64_t num_pages, int *flag, cudaStream_t stream, int extra_tokens = 0);
 // occupancy-derived persistent grid for the split kernel on the current device

@@ -124,6 +124,7 @@ __device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch
 template <int D, bool kFp8>
 __global__ void __launch_bounds__((Cfg<D, kFp8>::kThreads), 1)
 decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
+                    const __grid_constant__ CUtensorMap tm_kh, const __grid_constant__ CUtensorMap tm_vh,
                     const DecodeParams p)
 {
     using C = Cfg<D, kFp8>;
@@ -173,6 +174,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     if (warp == kConsumerWarps && lane == 0) {  // first producer warp
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
+        if (p.host_tier) {  // second tier: a pool in pinned host memory (block-table entries < 0), bf16 only
+            tma_prefetch_desc(&tm_kh);
+            tma_prefetch_desc(&tm_vh);
+        }
     }
     // Nothing above touched global data.  The inputs may still be written by the kernel running
     // before this one (kv_append bumps seq_lens), so nothing read before the wait is trusted -- but
@@ -322,8 +327,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 // tensor coordinates of the tile: {d, token row, -, kv head}, or {d, slot, kv head, page} for the HND layout
                 const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid * p.page_size + slot0;
                 const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid : sp.kvh;
-                tma_prefetch_tile_4d(&tm_k, 0, c1, c2, c3);
-                tma_prefetch_tile_4d(&tm_v, 0, c1, c2, c3);
+                if (pid >= 0) {  // (a host-tier page is not worth a hint: it would cross the host link twice)
+                    tma_prefetch_tile_4d(&tm_k, 0, c1, c2, c3);
+                    tma_prefetch_tile_4d(&tm_v, 0, c1, c2, c3);
+                }
             }
         }
         pdl_wait_prior_grid();
@@ -477,15 +484,19 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                         }
                         if (lane == 0) {
                             const int slot0 = (jj_i & tiles_per_page_mask) << kTileShift;
-                            const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pid_i * p.page_size + slot0;
-                            const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pid_i : sp.kvh;
+                            // block-table entry e >= 0: page e of the device pool; e < 0: page -1 - e of the host tier
+                            const bool host_page = !kFp8 && pid_i < 0;
+                            const int pg = host_page ? -1 - pid_i : pid_i;
+                            const CUtensorMap *mk = host_page ? &tm_kh : &tm_k, *mv = host_page ? &tm_vh : &tm_v;
+                            const int c1 = (kFp8 && p.kv_hnd) ? slot0 : pg * p.page_size + slot0;
+                            const int c2 = (kFp8 && p.kv_hnd) ? sp.kvh : 0, c3 = (kFp8 && p.kv_hnd) ? pg : sp.kvh;
                             const uint32_t dst = ring + stage * C::kStageBytes;
                             const uint32_t bar = full0 + 8 * stage;
                             if constexpr (kFp8)  // ordered before the consumers' wait by the arrive below (release) and their wait (acquire)
                                 asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(scales0 + 8 * stage), "f"(ks_i), "f"(vs_i) : "memory");
                             mbar_arrive_expect_tx(bar, C::kStageBytes);
-                            tma_load_4d_hint(dst, &tm_k, bar, 0, c1, c2, c3, stream_policy);
-                            tma_load_4d_hint(dst + C::kTileBytes, &tm_v, bar, 0, c1, c2, c3, stream_policy);
+                            tma_load_4d_hint(dst, mk, bar, 0, c1, c2, c3, stream_policy);
+                            tma_load_4d_hint(dst + C::kTileBytes, mv, bar, 0, c1, c2, c3, stream_policy);
                         }
                     }
                     pid = pid_next;
@@ -1051,19 +1062,22 @@ cudaError_t split_default_grid(int head_dim, int *grid_ctas)
 }
 
 template <int D, bool kFp8>
-static cudaError_t launch_variant(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
-                                  cudaLaunchConfig_t &cfg)
+static cudaError_t launch_variant(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const CUtensorMap &tm_kh,
+                                  const CUtensorMap &tm_vh, const DecodeParams &p, cudaLaunchConfig_t &cfg)
 {
     const cudaError_t e = configure_once<D, kFp8>();
     if (e != cudaSuccess) return e;
     cfg.blockDim = dim3(Cfg<D, kFp8>::kThreads);
     cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch, p.fuse_combine != 0);
-    return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8>, tm_k, tm_v, p);
+    return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8>, tm_k, tm_v, tm_kh, tm_vh, p);
 }
 
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
-                                int head_dim, cudaStream_t stream, bool kv_fp8)
+                                int head_dim, cudaStream_t stream, bool kv_fp8, const CUtensorMap *tm_k_host,
+                                const CUtensorMap *tm_v_host)
 {
+    // without a host tier the two extra descriptors are never used: pass the device ones
+    const CUtensorMap &tm_kh = tm_k_host ? *tm_k_host : tm_k, &tm_vh = tm_v_host ? *tm_v_host : tm_v;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(p.grid_ctas);
     cfg.stream = stream;
@@ -1072,9 +1086,11 @@ cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = p.no_pdl ? 0 : 1;
-    if (kv_fp8) return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, p, cfg) : launch_variant<64, true>(tm_k, tm_v, p, cfg);
-    if (head_dim == 128) return launch_variant<128, false>(tm_k, tm_v, p, cfg);
-    return launch_variant<64, false>(tm_k, tm_v, p, cfg);
+    if (kv_fp8)
+        return head_dim == 128 ? launch_variant<128, true>(tm_k, tm_v, tm_kh, tm_vh, p, cfg)
+                               : launch_variant<64, true>(tm_k, tm_v, tm_kh, tm_vh, p, cfg);
+    if (head_dim == 128) return launch_variant<128, false>(tm_k, tm_v, tm_kh, tm_vh, p, cfg);
+    return launch_variant<64, false>(tm_k, tm_v, tm_kh, tm_vh, p, cfg);
 }
 
 }  // namespace comem

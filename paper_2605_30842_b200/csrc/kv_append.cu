@@ -107,7 +107,29 @@ validate_kernel(const int32_t *block_table, const int32_t *seq_lens, int max_pag
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicCAS(flag, 0, b + 1);
 }
 
+// comem_pages_copy_async: CTA (i, t) copies page src_ids[i] -> dst_ids[i] of the K pool (t = 0) or the V pool (t = 1)
+// with 16-byte accesses; either side may be pinned host memory (zero-copy over the host link).
+__global__ void __launch_bounds__(256)
+pages_copy_kernel(const uint4 *k_src, const uint4 *v_src, uint4 *k_dst, uint4 *v_dst, const int32_t *src_ids,
+                  const int32_t *dst_ids, size_t page_vecs)
+{
+    pdl_wait_prior_grid();
+    const int i = blockIdx.x;
+    const uint4 *src = (blockIdx.y ? v_src : k_src) + (size_t)src_ids[i] * page_vecs;
+    uint4 *dst = (blockIdx.y ? v_dst : k_dst) + (size_t)dst_ids[i] * page_vecs;
+    for (size_t e = threadIdx.x; e < page_vecs; e += blockDim.x) dst[e] = src[e];
+}
+
 }  // namespace
+
+cudaError_t launch_pages_copy(const void *k_src, const void *v_src, void *k_dst, void *v_dst, const int32_t *src_ids,
+                              const int32_t *dst_ids, int n_pages, size_t page_bytes, cudaStream_t stream)
+{
+    pages_copy_kernel<<<dim3(n_pages, 2), 256, 0, stream>>>(
+        static_cast<const uint4 *>(k_src), static_cast<const uint4 *>(v_src), static_cast<uint4 *>(k_dst),
+        static_cast<uint4 *>(v_dst), src_ids, dst_ids, page_bytes / 16);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,
                             int page_size, int64_t num_pages, int *flag, cudaStream_t stream, int extra_tokens)

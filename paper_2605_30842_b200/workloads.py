@@ -479,3 +479,70 @@ def permute_pages(batch: DecodeBatch, seed: int) -> DecodeBatch:
     valid = bt >= 0
     bt2 = torch.where(valid, perm[bt.clamp_min(0)], bt).to(torch.int32)
     return dataclasses.replace(batch, k_pages=k2, v_pages=v2, block_table=bt2.to(dev))
+
+
+# ---------------------------------------------------------------------------------------------
+# two-tier cache (PAPER.md L61 / L245: CPU offloading): input preparation only
+# ---------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class OffloadBatch:
+    """A DecodeBatch whose cold pages live in a second pool in pinned host memory.  block_table entry e >= 0 is page
+    e of (k_pages, v_pages) on the device, e < 0 is page -1 - e of (k_host, v_host)."""
+
+    base: DecodeBatch          # q, device pools, remapped block table, seq_lens
+    k_host: torch.Tensor       # bf16 [P_host, page_size, Hkv, D], pinned
+    v_host: torch.Tensor
+    host_tokens: int           # cached tokens that live in the host pool
+
+    def host_bytes(self) -> int:
+        return self.host_tokens * self.base.num_kv_heads * self.base.head_dim * 2 * 2
+
+
+def offload_pages(batch: DecodeBatch, frac: float, seed: int, coldest_first: bool = True) -> OffloadBatch:
+    """Move a fraction `frac` of every sequence's USED pages to a pinned host pool and rewrite the block table
+    (pure data movement, like permute_pages).  coldest_first: the oldest pages of each sequence go (what an engine
+    offloads); otherwise a seeded random subset.  The device copies of the moved pages are overwritten with NaN, so a
+    kernel that still read them would show it."""
+    assert batch.q.is_cuda and 0.0 <= frac <= 1.0
+    ps = batch.page_size
+    lens = batch.seq_lens.cpu().tolist()
+    bt = batch.block_table.cpu().clone()
+    g = torch.Generator(device="cpu")
+    g.manual_seed(seed)
+    moved, host_tokens = [], 0
+    for b, L in enumerate(lens):
+        n = pages_needed(int(L), ps)
+        k = int(round(frac * n))
+        if k == 0:
+            continue
+        pick = list(range(k)) if coldest_first else sorted(torch.randperm(n, generator=g)[:k].tolist())
+        for j in pick:
+            moved.append(int(bt[b, j]))
+            bt[b, j] = -1 - (len(moved) - 1)
+            host_tokens += min(ps, int(L) - j * ps)
+    n_host = max(1, len(moved))
+    shape = (n_host,) + tuple(batch.k_pages.shape[1:])
+    k_host = torch.zeros(shape, dtype=torch.bfloat16).pin_memory()
+    v_host = torch.zeros(shape, dtype=torch.bfloat16).pin_memory()
+    k_dev, v_dev = batch.k_pages.clone(), batch.v_pages.clone()
+    if moved:
+        ids = torch.tensor(moved, dtype=torch.int64, device=batch.k_pages.device)
+        k_host[: len(moved)].copy_(batch.k_pages[ids])
+        v_host[: len(moved)].copy_(batch.v_pages[ids])
+        k_dev[ids] = float("nan")
+        v_dev[ids] = float("nan")
+    base = dataclasses.replace(batch, k_pages=k_dev, v_pages=v_dev, block_table=bt.to(batch.block_table.device))
+    return OffloadBatch(base=base, k_host=k_host, v_host=v_host, host_tokens=host_tokens)
+
+
+def combined_pool_cpu(ob: OffloadBatch) -> DecodeBatch:
+    """The same logical cache as ONE pool on the CPU (device pool followed by the host pool, table entries e < 0
+    rewritten to P_dev - 1 - e): what the oracle, which knows one pool, is given.  Data movement only."""
+    b = ob.base
+    P = b.num_pages
+    k = torch.cat([b.k_pages.cpu(), ob.k_host], dim=0)
+    v = torch.cat([b.v_pages.cpu(), ob.v_host], dim=0)
+    bt = b.block_table.cpu().to(torch.int64)
+    bt = torch.where(bt < 0, P - 1 - bt, bt).to(torch.int32)
+    return DecodeBatch(q=b.q.cpu(), k_pages=k, v_pages=v, block_table=bt, seq_lens=b.seq_lens.cpu(),
+                       softmax_scale=b.softmax_scale, name=b.name, seed=b.seed)
