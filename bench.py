@@ -877,6 +877,69 @@ def run_fp8(args) -> int:
     return 0
 
 
+def pipeline_trajectory(torch, comem, W, device, K, T, TURN, SUMM, CONC, Y, YM):
+    """The whole trajectory through the library's scheduler (comem_kstep_step_async): per agent step the prefill
+    attention (cached or uncached, as Algorithm 1 says), Y decode tokens (append + decode attention), and the memory
+    model's jobs on the second stream with the SM-partition policy -- once under CoMem's plan (retain-turns K) and once
+    as the full-context baseline (no memory model: the plan of k > T never adopts or launches).  Eq. 6: the
+    net speed-up holds iff the decode time saved per cycle exceeds the uncached prefill it costs."""
+    max_ctx = T * TURN + max(Y, YM) + 16
+
+    def build(hq, seed, cap_tokens):
+        b = W.make_batch([max_ctx] * CONC, hq, 8, 128, 16, seed, device)
+        qp = torch.empty((CONC * cap_tokens, hq, 128), dtype=torch.bfloat16, device=device).normal_()
+        m = {"b": b, "qp": qp, "op": torch.empty_like(qp), "od": torch.empty_like(b.q),
+             "nk": torch.randn((CONC, 8, 128), device=device).to(torch.bfloat16),
+             "nv": torch.randn((CONC, 8, 128), device=device).to(torch.bfloat16),
+             "qs": torch.zeros(CONC + 1, dtype=torch.int32, device=device),
+             "ws": comem.alloc_workspace(b.q, b.k_pages, b.block_table)}
+        m["model"] = comem.kstep_model(b.q, m["od"], qp, m["op"], m["nk"], m["nv"], b.k_pages, b.v_pages, b.block_table,
+                                       b.seq_lens, m["qs"], m["ws"], b.softmax_scale)
+        return m
+
+    agent = build(64, 1301, SUMM + (K + 1) * TURN)   # CoMem never prefills more than summary + k + 1 turns at once
+    memory = build(32, 1302, T * TURN)               # the memory model prefills the whole trajectory so far
+    sa, sm = torch.cuda.Stream(device), torch.cuda.Stream(device)
+    ev_done, ev_step = torch.cuda.Event(), torch.cuda.Event()
+    ev_done.record(sm)
+    ev_step.record(sa)
+    torch.cuda.synchronize()
+    out = {}
+    # "comem_memory_elsewhere" is the paper's deployment (separate engines for the agent and the memory model,
+    # P:L245, L310): this GPU runs the agent's side of Algorithm 1 only; "comem_colocated" also runs every memory
+    # job (a full-trajectory prefill of the 32q/8kv model at the same concurrency) on this GPU's second stream.
+    for name, k_plan, mem in (("comem_memory_elsewhere", K, None), ("comem_colocated", K, memory),
+                              ("full_context", T + 1, None)):
+        arr, events = comem.comem_kstep_plan(T, k_plan, 0)
+        per_step, launches, partitioned = [], 0, 0
+        t0 = torch.cuda.Event(enable_timing=True)
+        t0.record(sa)
+        marks = []
+        for e in events:
+            st = comem.comem_kstep_step_async(e, TURN, SUMM, Y, YM, agent["model"], None if mem is None else mem["model"],
+                                              sa, sm, ev_done, ev_step)
+            launches += st.launches
+            partitioned += st.memory_in_flight
+            m = torch.cuda.Event(enable_timing=True)
+            m.record(sa)
+            marks.append(m)
+        torch.cuda.synchronize()
+        prev = t0
+        for m in marks:
+            per_step.append(prev.elapsed_time(m))
+            prev = m
+        unc = [per_step[i] for i, e in enumerate(events) if e.prefill_uncached and i > 0]
+        out[name] = {"agent_stream_ms": t0.elapsed_time(marks[-1]), "launches": launches,
+                     "steps_with_sm_partition": partitioned, "per_step_ms": [round(x, 3) for x in per_step],
+                     "uncached_prefill_steps": sum(int(e.prefill_uncached) for e in events),
+                     "mean_ms_steps_with_uncached_prefill": (sum(unc) / len(unc)) if unc else None}
+    out["speedup_agent_stream"] = out["full_context"]["agent_stream_ms"] / out["comem_memory_elsewhere"]["agent_stream_ms"]
+    out["speedup_agent_stream_colocated"] = out["full_context"]["agent_stream_ms"] / out["comem_colocated"]["agent_stream_ms"]
+    out["config"] = {"k": K, "steps": T, "turn_tokens": TURN, "summary_tokens": SUMM, "concurrency": CONC,
+                     "decode_tokens_per_step": Y, "memory_decode_tokens": YM}
+    return out
+
+
 def run_pipeline(args) -> int:
     """Extra: the k-step-off pipeline (Algorithm 1) over 64 agent steps
     (L261), shaped like the paper's crossover benchmark (section 4.5: fixed-length turns, concurrency 32,
@@ -999,8 +1062,28 @@ def run_pipeline(args) -> int:
             rec["sm_partition"].append({"agent_sms": agent_sms, "memory_sms": sms - agent_sms, "split": how,
                                         "agent_us": p0.elapsed_time(p1) * 1e3 / reps})
         overlap.append(rec)
+    del flush, out_a, out_m, ws_a, ws_m, agent, memory
+    torch.cuda.empty_cache()
+    # the whole trajectory through the library's scheduler, attention AND prefill per step; eq. 6 against it
+    Y, YM = 32, 32
+    traj = pipeline_trajectory(torch, comem, W, device, K, T, TURN, SUMM, CONC, Y, YM)
+    p_tok_s = None
+    unc_ms = traj["comem_memory_elsewhere"]["mean_ms_steps_with_uncached_prefill"]
+    if unc_ms:
+        # P of eq. 6: prompt tokens per second of the uncached prefill (summary + buffered turns, all sequences)
+        l_sum_tokens = statistics.mean(c for c, e in zip(ctx_comem, events) if e.prefill_uncached)
+        dec_ms = Y * statistics.mean(t_comem) / 1e3
+        p_tok_s = CONC * l_sum_tokens / max((unc_ms - dec_ms) * 1e-3, 1e-9)
+        l_full_mean, l_sum_mean = statistics.mean(ctx_full), statistics.mean(ctx_comem)
+        traj["eq6"] = {"P_tokens_per_s": p_tok_s, "W_gbs": w_gbs, "Y_tokens_per_cycle": Y * K * CONC,
+                       "L_full_mean": l_full_mean, "L_sum_mean": l_sum_mean,
+                       "predicted_net_speedup": bool(comem.comem_net_speedup(Y * K, l_full_mean, l_sum_mean, s_bytes / 1e9, w_gbs,
+                                                                             p_tok_s / CONC)),
+                       "measured_net_speedup": traj["speedup_agent_stream"] > 1.0,
+                       "max_compression_ratio_eq7": comem.comem_max_compression_ratio(w_gbs, Y * K, s_bytes / 1e9, p_tok_s / CONC)}
     print(json.dumps({
         "extra": "k-step-off pipeline (Algorithm 1) driven from comem_kstep_plan; eq. 5 vs measured",
+        "trajectory": traj,
         "k": K, "steps": T, "turn_tokens": TURN, "summary_tokens": SUMM, "concurrency": CONC,
         "uncached_prefills": sum(int(e.prefill_uncached) for e in events),
         "memory_launches": sum(int(e.launch_memory) for e in events),

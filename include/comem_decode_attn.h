@@ -295,6 +295,56 @@ double comem_max_compression_ratio(double w_gb_per_s, double y_tokens, double s_
                                    double p_tokens_per_s);
 
 /*
+ * comem_kstep_step_async — ONE agent step of Algorithm 1 as the library's host scheduler: everything
+ * the attention path does for step t is enqueued, on two streams, from the plan entry of comem_kstep_plan:
+ *   agent stream   lines 4-7   adopt a finished summary: the KV cache is invalid, the context becomes
+ *                              summary + raw buffer (eq. 4): seq_lens[b] <- ctx_t for every sequence
+ *                  lines 9-13  prefill attention (comem_prefill_attn_async) of the NEW tokens: the whole context
+ *                              when the plan says uncached ("a full uncached prefill is required"), else
+ *                              the last turn_tokens only (cached, incremental)
+ *                  line 15     decode_tokens times: comem_kv_append_async + comem_decode_attn_async
+ *   memory stream  lines 19-21 if the plan launches a memory job after this step: wait for the agent's step, then
+ *                              the memory model's uncached prefill over tau_{<=t} (t * turn_tokens tokens) and
+ *                              memory_decode_tokens decode steps (the summary it writes), behind an event
+ * Sharing the GPU: while a memory job is in flight (the scheduler asks the job's completion event, without blocking)
+ * both models' decode grids are sized by comem_sm_partition from the bytes each streams per step and launched without
+ * programmatic serialization, so an agent step never queues behind a whole memory step; otherwise the agent has
+ * every SM and programmatic launch.  This is the attention path of one layer: projections, MLPs and sampling are
+ * the serving engine's; K/V rows of prefilled tokens are whatever the pools hold (the engine writes them).
+ *
+ * comem_kstep_model describes one model's buffers (all device pointers, caller-owned, contiguous):
+ *   q_decode / out_decode   bf16 [batch][Hq][D];  new_k / new_v  bf16 [batch][Hkv][D] (the row each decode token appends)
+ *   q_prefill / out_prefill bf16 [prefill_cap][Hq][D], prefill_cap >= batch * (largest context this model prefills)
+ *   k_pages, v_pages, block_table, seq_lens, workspace: as comem_decode_attn_async;  q_start int32 [batch + 1]
+ * The call writes seq_lens and q_start (a small kernel), out_decode, out_prefill and the workspace; it never
+ * synchronizes.  stats (optional, host) reports what was enqueued.  COMEM_ERR_INVALID_ARG: a context that does not
+ * fit max_pages_per_seq * page_size or prefill_cap, null buffers, decode_tokens < 0.
+ */
+typedef struct {
+    void *q_decode, *out_decode, *q_prefill, *out_prefill, *new_k, *new_v;
+    void *k_pages, *v_pages;
+    int32_t *block_table, *seq_lens, *q_start;
+    void *workspace;
+    size_t workspace_bytes;
+    int64_t num_pages, prefill_cap;
+    int batch, num_q_heads, num_kv_heads, head_dim, page_size, max_pages_per_seq;
+    float softmax_scale;
+} comem_kstep_model;
+typedef struct {
+    int32_t agent_ctx;            /* tokens in the agent's context at this step (eq. 4) */
+    int32_t agent_prefill_tokens; /* per sequence: ctx if uncached, else turn_tokens */
+    int32_t memory_ctx;           /* tokens the memory job prefills (0 if none launched) */
+    int32_t agent_grid, memory_grid; /* decode grids used (0 = default: every SM) */
+    int32_t memory_in_flight;     /* 1 if the SM partition was applied to the agent's decode steps */
+    int32_t launches;             /* kernels enqueued by this call */
+} comem_kstep_step_stats;
+int comem_kstep_step_async(const comem_kstep_event *event, int turn_tokens, int summary_tokens, int decode_tokens,
+                           int memory_decode_tokens, const comem_kstep_model *agent,
+                           const comem_kstep_model *memory /* NULL: no memory model on this GPU */,
+                           void *agent_stream, void *memory_stream, void *memory_done_event /* cudaEvent_t */,
+                           void *agent_step_event /* cudaEvent_t */, comem_kstep_step_stats *stats);
+
+/*
  * comem_prefill_attn_async — causal prefill attention over the paged cache: the compute-bound
  * step of the path.  P:L149-156 (Algorithm 1 lines 9-13): "Prefill new tokens only" when the KV cache is valid
  * (cached, incremental prefill), "Prefill full context" after a summary adoption invalidated it (uncached);

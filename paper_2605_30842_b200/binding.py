@@ -63,6 +63,8 @@ def load_library():
     lib.comem_decode_attn_offload_async.restype = i32
     lib.comem_pages_copy_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, sz, vp]
     lib.comem_pages_copy_async.restype = i32
+    lib.comem_kstep_step_async.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.comem_kstep_step_async.restype = i32
     lib.comem_prefill_attn_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i32,
                                              i64, vp, vp, vp]
     lib.comem_prefill_attn_async.restype = i32
@@ -204,6 +206,56 @@ def comem_kstep_plan(num_steps: int, k: int, mem_delay: int = 0):
     if st != COMEM_OK:
         raise ComemError(st, "comem_kstep_plan")
     return ev, [ev[i] for i in range(num_steps)]
+
+
+class KstepModel(ctypes.Structure):
+    """comem_kstep_model (include/comem_decode_attn.h)."""
+    _fields_ = [(n, ctypes.c_void_p) for n in ("q_decode", "out_decode", "q_prefill", "out_prefill", "new_k", "new_v",
+                                               "k_pages", "v_pages", "block_table", "seq_lens", "q_start", "workspace")] + \
+               [("workspace_bytes", ctypes.c_size_t), ("num_pages", ctypes.c_int64), ("prefill_cap", ctypes.c_int64)] + \
+               [(n, ctypes.c_int) for n in ("batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size",
+                                            "max_pages_per_seq")] + [("softmax_scale", ctypes.c_float)]
+
+
+class KstepStepStats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("agent_ctx", "agent_prefill_tokens", "memory_ctx", "agent_grid",
+                                              "memory_grid", "memory_in_flight", "launches")]
+
+
+def kstep_model(q_decode, out_decode, q_prefill, out_prefill, new_k, new_v, k_pages, v_pages, block_table, seq_lens,
+                q_start, workspace, softmax_scale: float) -> KstepModel:
+    """Fill a comem_kstep_model from torch tensors (pointers only: keep the tensors alive)."""
+    m = KstepModel()
+    for name, t in (("q_decode", q_decode), ("out_decode", out_decode), ("q_prefill", q_prefill),
+                    ("out_prefill", out_prefill), ("new_k", new_k), ("new_v", new_v), ("k_pages", k_pages),
+                    ("v_pages", v_pages), ("block_table", block_table), ("seq_lens", seq_lens), ("q_start", q_start),
+                    ("workspace", workspace)):
+        assert t.is_cuda and t.is_contiguous()
+        setattr(m, name, t.data_ptr())
+    m.workspace_bytes = workspace.numel() * workspace.element_size()
+    m.num_pages, m.prefill_cap = k_pages.shape[0], q_prefill.shape[0]
+    m.batch, m.num_q_heads, m.head_dim = q_decode.shape
+    m.num_kv_heads, m.page_size, m.max_pages_per_seq = k_pages.shape[2], k_pages.shape[1], block_table.shape[1]
+    m.softmax_scale = float(softmax_scale)
+    return m
+
+
+def comem_kstep_step_async(event, turn_tokens: int, summary_tokens: int, decode_tokens: int, memory_decode_tokens: int,
+                           agent: KstepModel, memory, agent_stream, memory_stream=None, memory_done_event=None,
+                           agent_step_event=None) -> KstepStepStats:
+    """One agent step of Algorithm 1 enqueued by the library's scheduler (see the header).  `event`: one
+    comem_kstep_event of comem_kstep_plan's array; events: torch.cuda.Event objects that have been recorded once
+    (so that their CUDA handle exists), or None."""
+    stats = KstepStepStats()
+    ev = lambda e: None if e is None else ctypes.c_void_p(e.cuda_event)  # noqa: E731
+    st = load_library().comem_kstep_step_async(
+        ctypes.byref(event), int(turn_tokens), int(summary_tokens), int(decode_tokens), int(memory_decode_tokens),
+        ctypes.byref(agent), None if memory is None else ctypes.byref(memory), _stream(agent_stream),
+        None if memory_stream is None else _stream(memory_stream), ev(memory_done_event), ev(agent_step_event),
+        ctypes.byref(stats))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_kstep_step_async")
+    return stats
 
 
 def comem_kstep_context_lengths(events_array, num_steps: int, turn_tokens: int, summary_tokens: int):
