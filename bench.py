@@ -771,7 +771,7 @@ def run_fp8(args) -> int:
     cuda_build.build()
     comem.load_library()
     pools = []
-    for bf in make_pools(args.workload, device, 0, 0):
+    for bf in make_pools(args.workload, device, 0, 64):   # 64 spare tokens per sequence: room for the e2e leg's appends
         f8 = W.quantize_batch_fp8(bf)
         del bf
         pools.append(W.to_hnd(f8) if args.kv_layout == "hnd" else f8)
@@ -857,7 +857,41 @@ def run_fp8(args) -> int:
         step(0)
         stream.synchronize()
     parity, oracle_s = (None, None) if args.no_cpu_baseline else fp8_parity(pools[0], outs[0])
-    print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload),
+    # end to end through comem_decode_step_host_fp8: pinned host q / k / v rows in, quantising append, attention, host out
+    e2e = None
+    if pools[0].kv_layout in ("NHD", "HND"):
+        n_e2e = 32
+        rows = []
+        for j in range(4):
+            gq = torch.Generator(device=device)
+            gq.manual_seed(4242 + j)
+            b0_ = pools[0]
+            rows.append(tuple(torch.randn(sh, generator=gq, device=device).to(torch.bfloat16).cpu().pin_memory()
+                              for sh in (tuple(b0_.q.shape), (b0_.batch, b0_.num_kv_heads, b0_.head_dim),
+                                         (b0_.batch, b0_.num_kv_heads, b0_.head_dim))))
+        out_h = torch.empty(tuple(pools[0].q.shape), dtype=torch.bfloat16).pin_memory()
+        lens0 = [b.seq_lens.clone() for b in pools]
+
+        def e2e_step(i):
+            b = pools[i % len(pools)]
+            q, nk, nv = rows[i % 4]
+            comem.comem_decode_step_host_fp8(q, nk, nv, b.k_pages, b.v_pages, b.k_scale, b.v_scale, b.block_table,
+                                             b.seq_lens, b.softmax_scale, out_h, ws, stream=stream, kv_layout=b.kv_layout)
+        for i in range(3):
+            e2e_step(i)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for i in range(n_e2e):
+            e2e_step(3 + i)
+        t1 = time.perf_counter()
+        for b, l0 in zip(pools, lens0):
+            b.seq_lens.copy_(l0)
+        e2e_us = (t1 - t0) / n_e2e * 1e6
+        h2d = (rows[0][0].numel() + 2 * rows[0][1].numel()) * 2
+        e2e = {"value": nbytes / e2e_us / 1e3, "unit": UNIT, "us_per_step": e2e_us, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": out_h.numel() * 2, "steps": n_e2e,
+               "api": "comem_decode_step_host_fp8, pinned host buffers (host wall clock around the synchronous calls)"}
+    print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload), "e2e": e2e,
                       "kv_layout": pools[0].kv_layout,
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,

@@ -430,6 +430,20 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
                            void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * comem_decode_step_host_fp8 — comem_decode_step_host for the FP8 cache (reading R18): the new token's bf16 q, k, v rows
+ * come from host buffers, k / v are quantised into the E4M3 pools with the page's scales (comem_kv_append_fp8_async's
+ * arithmetic), seq_lens += 1, comem_decode_attn_fp8_async runs, out (and lse) go back to the host.  Same two paths
+ * (pinned + mapped: the kernels move the bytes, 2 launches + synchronize; pageable: cudaMemcpyAsync staging), same
+ * host-synchronous contract.  new_k_host / new_v_host are required (this call always appends).
+ */
+int comem_decode_step_host_fp8(const void *q_host, const void *new_k_host, const void *new_v_host, void *k_pages,
+                               void *v_pages, const float *k_scale, const float *v_scale,
+                               const int32_t *block_table, int32_t *seq_lens, int num_q_heads, int num_kv_heads,
+                               int head_dim, int page_size, float softmax_scale, void *out_host, int batch,
+                               int max_pages_per_seq, int64_t num_pages, float *lse_host, void *workspace,
+                               size_t workspace_bytes, void *cuda_stream, int kv_layout);
+
+/*
  * Split-KV schedule introspection (host arithmetic mirroring the device
  * scheduler; used by tests and DESIGN.md).  Given host copies of seq_lens,
  * writes for each CTA i in [0, *num_ctas) its half-open range of 16-token tiles

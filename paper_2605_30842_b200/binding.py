@@ -65,6 +65,9 @@ def load_library():
     lib.comem_pages_copy_async.restype = i32
     lib.comem_kstep_step_async.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.comem_kstep_step_async.restype = i32
+    lib.comem_decode_step_host_fp8.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
+                                               i64, vp, vp, sz, vp, i32]
+    lib.comem_decode_step_host_fp8.restype = i32
     lib.comem_prefill_attn_async.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32, i32,
                                              i64, vp, vp, vp]
     lib.comem_prefill_attn_async.restype = i32
@@ -548,3 +551,23 @@ def comem_decode_step_host(q_host, new_k_host, new_v_host, k_pages, v_pages, blo
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_step_host")
 
+
+
+def comem_decode_step_host_fp8(q_host, new_k_host, new_v_host, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
+                               softmax_scale: float, out_host, workspace, lse_host=None, stream=None,
+                               kv_layout: str = "NHD") -> None:
+    """comem_decode_step_host for the FP8 cache: host q / new k / new v rows in (bf16), quantising append, FP8 decode
+    attention, host out back (synchronous)."""
+    assert kv_layout in ("NHD", "HND")
+    hnd = kv_layout == "HND"
+    assert q_host.device.type == "cpu" and out_host.device.type == "cpu"
+    assert q_host.dtype == torch.bfloat16 and out_host.dtype == torch.bfloat16 and k_pages.dtype == torch.uint8
+    assert q_host.is_contiguous() and out_host.is_contiguous() and out_host.shape == q_host.shape
+    page_size, hkv = (k_pages.shape[2], k_pages.shape[1]) if hnd else (k_pages.shape[1], k_pages.shape[2])
+    st = load_library().comem_decode_step_host_fp8(
+        _ptr(q_host), _ptr(new_k_host), _ptr(new_v_host), _ptr(k_pages), _ptr(v_pages), _ptr(k_scale), _ptr(v_scale),
+        _ptr(block_table), _ptr(seq_lens), q_host.shape[1], hkv, q_host.shape[2], page_size,
+        ctypes.c_float(softmax_scale), _ptr(out_host), q_host.shape[0], block_table.shape[1], k_pages.shape[0],
+        _ptr(lse_host), _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream), 1 if hnd else 0)
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_step_host_fp8")

@@ -802,4 +802,66 @@ int comem_decode_step_host(const void *q_host, const void *new_k_host, const voi
     return COMEM_OK;
 }
 
+int comem_decode_step_host_fp8(const void *q_host, const void *new_k_host, const void *new_v_host, void *k_pages,
+                               void *v_pages, const float *k_scale, const float *v_scale, const int32_t *block_table,
+                               int32_t *seq_lens, int num_q_heads, int num_kv_heads, int head_dim, int page_size,
+                               float softmax_scale, void *out_host, int batch, int max_pages_per_seq, int64_t num_pages,
+                               float *lse_host, void *workspace, size_t workspace_bytes, void *cuda_stream, int kv_layout)
+{
+    if (!q_host || !out_host || !new_k_host || !new_v_host || !k_pages || !v_pages || !k_scale || !v_scale ||
+        !block_table || !seq_lens)
+        return COMEM_ERR_INVALID_ARG;
+    if (kv_layout != COMEM_KV_LAYOUT_NHD && kv_layout != COMEM_KV_LAYOUT_HND) return COMEM_ERR_INVALID_ARG;
+    int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
+    if (st != COMEM_OK) return st;
+    const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
+    if (!workspace || workspace_bytes < wl.total || !aligned(workspace, 256)) return COMEM_ERR_WORKSPACE;
+    if ((st = check_device()) != COMEM_OK) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    char *ws = static_cast<char *>(workspace);
+    const size_t q_bytes = (size_t)batch * num_q_heads * head_dim * 2;
+    const size_t kv_bytes = (size_t)batch * num_kv_heads * head_dim * 2;
+    const int hnd = kv_layout == COMEM_KV_LAYOUT_HND ? 1 : 0;
+    void *dq = device_alias(q_host), *dout = device_alias(out_host), *dk = device_alias(new_k_host),
+         *dv = device_alias(new_v_host), *dlse = lse_host ? device_alias(lse_host) : nullptr;
+    const bool mapped = dq && dout && dk && dv && (!lse_host || dlse) && aligned(dq, 16) && aligned(dout, 16) &&
+                        aligned(dk, 4) && aligned(dv, 4);
+    const void *nk = dk, *nv = dv;
+    const void *q_src = dq;
+    void *out_dst = dout;
+    float *lse_dst = static_cast<float *>(dlse);
+    bool ok = true;
+    if (!mapped) {  // pageable host memory: the copy engine stages the rows
+        ok = cudaMemcpyAsync(ws + wl.new_k, new_k_host, kv_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess &&
+             cudaMemcpyAsync(ws + wl.new_v, new_v_host, kv_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess &&
+             cudaMemcpyAsync(ws + wl.out, q_host, q_bytes, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+        nk = ws + wl.new_k;
+        nv = ws + wl.new_v;
+        q_src = ws + wl.out;  // (staged to wl.q by the append kernel like the mapped path; wl.out is free until the attention runs)
+        out_dst = ws + wl.out;
+        lse_dst = lse_host ? reinterpret_cast<float *>(ws + wl.lse) : nullptr;
+    }
+    // K3 (FP8): quantise + append the new row with the page's scales, bump seq_lens, stage q in the workspace
+    if (launch_kv_append_fp8(static_cast<uint8_t *>(k_pages), static_cast<uint8_t *>(v_pages), k_scale, v_scale,
+                             block_table, seq_lens, static_cast<const __nv_bfloat16 *>(nk),
+                             static_cast<const __nv_bfloat16 *>(nv), num_kv_heads, head_dim, page_size, batch,
+                             max_pages_per_seq, hnd, stream, static_cast<const __nv_bfloat16 *>(q_src),
+                             reinterpret_cast<__nv_bfloat16 *>(ws + wl.q), num_q_heads * head_dim) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    st = comem_decode_attn_fp8_async(ws + wl.q, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, num_q_heads,
+                                     num_kv_heads, head_dim, page_size, softmax_scale, out_dst, batch, max_pages_per_seq,
+                                     num_pages, lse_dst, workspace, workspace_bytes, cuda_stream, 0, 0, kv_layout, nullptr);
+    if (st != COMEM_OK) return st;
+    if (!mapped) {
+        ok = cudaMemcpyAsync(out_host, ws + wl.out, q_bytes, cudaMemcpyDeviceToHost, stream) == cudaSuccess;
+        if (ok && lse_host)
+            ok = cudaMemcpyAsync(lse_host, ws + wl.lse, (size_t)batch * num_q_heads * 4, cudaMemcpyDeviceToHost, stream) == cudaSuccess;
+    }
+    if (!ok || cudaStreamSynchronize(stream) != cudaSuccess) { cudaGetLastError(); return COMEM_ERR_CUDA; }
+    return COMEM_OK;
+}
+
 }  // extern "C"

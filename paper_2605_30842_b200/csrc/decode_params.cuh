@@ -80,7 +80,8 @@ cudaError_t launch_kv_append(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages,
 cudaError_t launch_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
                                  const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
                                  const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
-                                 int max_pages, int hnd, cudaStream_t stream);
+                                 int max_pages, int hnd, cudaStream_t stream, const __nv_bfloat16 *q_src = nullptr,
+                                 __nv_bfloat16 *q_dst = nullptr, int q_row_elems = 0);
 cudaError_t launch_pages_copy(const void *k_src, const void *v_src, void *k_dst, void *v_dst, const int32_t *src_ids,
                               const int32_t *dst_ids, int n_pages, size_t page_bytes, cudaStream_t stream);
 cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens, int batch, int max_pages,

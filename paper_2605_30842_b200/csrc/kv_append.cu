@@ -56,11 +56,17 @@ kv_append_kernel(__nv_bfloat16 *k_pages, __nv_bfloat16 *v_pages, const int32_t *
 __global__ void __launch_bounds__(128)
 kv_append_fp8_kernel(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
                      const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
-                     const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int max_pages, int hnd)
+                     const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int max_pages, int hnd,
+                     const __nv_bfloat16 *q_src, __nv_bfloat16 *q_dst, int q_row_elems)
 {
     pdl_launch_dependents();  // as in kv_append_kernel
     pdl_wait_prior_grid();
     const int b = blockIdx.x;
+    if (q_src != nullptr) {  // end-to-end path: stage sequence b's query rows (q_src may be pinned host memory)
+        const uint4 *s = reinterpret_cast<const uint4 *>(q_src + (int64_t)b * q_row_elems);
+        uint4 *d = reinterpret_cast<uint4 *>(q_dst + (int64_t)b * q_row_elems);
+        for (int i = threadIdx.x; i < q_row_elems / 8; i += blockDim.x) d[i] = s[i];
+    }
     const int t = seq_lens[b];
     const int page = t / page_size;
     const int slot = t - page * page_size;
@@ -143,10 +149,12 @@ cudaError_t launch_validate(const int32_t *block_table, const int32_t *seq_lens,
 cudaError_t launch_kv_append_fp8(uint8_t *k_pages, uint8_t *v_pages, const float *k_scale, const float *v_scale,
                                  const int32_t *block_table, int32_t *seq_lens, const __nv_bfloat16 *new_k,
                                  const __nv_bfloat16 *new_v, int num_kv_heads, int head_dim, int page_size, int batch,
-                                 int max_pages, int hnd, cudaStream_t stream)
+                                 int max_pages, int hnd, cudaStream_t stream, const __nv_bfloat16 *q_src,
+                                 __nv_bfloat16 *q_dst, int q_row_elems)
 {
     kv_append_fp8_kernel<<<batch, 128, 0, stream>>>(k_pages, v_pages, k_scale, v_scale, block_table, seq_lens, new_k,
-                                                   new_v, num_kv_heads, head_dim, page_size, max_pages, hnd);
+                                                   new_v, num_kv_heads, head_dim, page_size, max_pages, hnd, q_src, q_dst,
+                                                   q_row_elems);
     return cudaGetLastError();
 }
 

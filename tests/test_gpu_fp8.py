@@ -381,3 +381,40 @@ def test_fp8_two_streams_overlap_equals_serial():
             xf = x.view(torch.bfloat16).float()
             assert torch.isfinite(xf).all() and float(xf.abs().max()) < 16.0, (which, step, float(xf.abs().max()))
             assert torch.equal(x, y), (which, step)
+
+
+@pytest.mark.parametrize("layout", ["NHD", "HND"])
+@pytest.mark.parametrize("pinned", [True, False])
+def test_fp8_decode_step_host_equals_device_calls(oracle, layout, pinned):
+    """comem_decode_step_host_fp8 (host rows in, quantising append, FP8 attention, host out back) against the same
+    step made of comem_kv_append_fp8_async + comem_decode_attn_fp8_async on a twin cache: bytes, lengths and outputs
+    bit-identical, on the pinned (zero-copy) and the pageable (copy-engine) path; last step checked against the oracle."""
+    ps = 16
+    b = W.make_batch([ps - 2, 3000, 0, 129], 16, 4, 128, ps, seed=571, device=DEV, spare_tokens=24)
+    f = W.quantize_batch_fp8(b)
+    f.k_scale.copy_(torch.where(torch.isnan(f.k_scale) | (f.k_scale == 1.0), torch.full_like(f.k_scale, 0.011), f.k_scale))
+    f.v_scale.copy_(torch.where(torch.isnan(f.v_scale) | (f.v_scale == 1.0), torch.full_like(f.v_scale, 0.009), f.v_scale))
+    if layout == "HND":
+        f = W.to_hnd(f)
+    twin = dataclasses.replace(f, k_pages=f.k_pages.clone(), v_pages=f.v_pages.clone(), seq_lens=f.seq_lens.clone())
+    f = dataclasses.replace(f, seq_lens=f.seq_lens.clone())
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=layout)
+    ws2 = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=layout)
+    pin = (lambda t: t.cpu().pin_memory()) if pinned else (lambda t: t.cpu())
+    out_h = pin(torch.zeros_like(f.q))
+    lse_h = pin(torch.zeros((f.q.shape[0], f.q.shape[1]), dtype=torch.float32))
+    for step in range(20):
+        q, nk, nv = W.decode_step_rows(b, step, seed_base=7100)
+        comem.comem_decode_step_host_fp8(pin(q), pin(nk), pin(nv), f.k_pages, f.v_pages, f.k_scale, f.v_scale,
+                                         f.block_table, f.seq_lens, f.softmax_scale, out_h, ws, lse_host=lse_h,
+                                         kv_layout=layout)
+        comem.comem_kv_append_fp8_async(twin.k_pages, twin.v_pages, twin.k_scale, twin.v_scale, twin.block_table,
+                                        twin.seq_lens, nk, nv, kv_layout=layout)
+        out, lse = run8(dataclasses.replace(twin, q=q), ws=ws2)
+        torch.cuda.synchronize()
+        assert torch.equal(out_h.view(torch.int16), out.cpu().view(torch.int16)), step
+        assert torch.equal(lse_h.view(torch.int32), lse.cpu().view(torch.int32)), step
+        assert torch.equal(f.seq_lens, twin.seq_lens) and torch.equal(f.k_pages, twin.k_pages) and torch.equal(f.v_pages, twin.v_pages)
+    ref, ref_lse = oracle.decode_attn_fp8(q.cpu(), f.k_pages.cpu(), f.v_pages.cpu(), f.k_scale.cpu(), f.v_scale.cpu(),
+                                          f.block_table.cpu(), f.seq_lens.cpu(), f.softmax_scale, kv_layout=layout)
+    gate(out_h.double().numpy(), ref, lse_h.double().numpy(), ref_lse, f"host step {layout}")
