@@ -46,7 +46,7 @@ L2_BYTES_NOMINAL = 126e6
 
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 # COMEM_LAUNCH_* bits the decode workloads are launched with unless --launch-flags says otherwise
-DEFAULT_LAUNCH_FLAGS = 5  # KV_PREFIX_IMMUTABLE | Q_STABLE: nothing in the timed loops writes the cache prefix or q
+DEFAULT_LAUNCH_FLAGS = 7  # KV_PREFIX_IMMUTABLE | SPLIT_COMBINE | Q_STABLE: nothing in the timed loops writes the cache prefix or q
 
 
 def kernel_source_sha() -> str:
