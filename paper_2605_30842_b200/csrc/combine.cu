@@ -111,7 +111,10 @@ combine_kernel(const DecodeParams p)
 //     are taken against the segment's global maximum (known before any accumulation), each warp sums its records in
 //     index order and the four warp sums are added in warp order: a fixed order, a function of the schedule only.
 // K1 then needs neither fence nor ticket, and no CTA of it finishes later than the others because it merged.
-constexpr int kSmallThreads = 128;
+#ifndef COMEM_SMALL_THREADS
+#define COMEM_SMALL_THREADS 128
+#endif
+constexpr int kSmallThreads = COMEM_SMALL_THREADS;
 constexpr int kSmallStripes = kSmallThreads / 32;
 constexpr int kSmallBatch = 5;  // records per warp in flight
 

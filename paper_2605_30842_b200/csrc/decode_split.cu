@@ -209,8 +209,14 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // exclusive prefix of tiles per sequence (warp 0); kept small: no unrolling
         if (warp == 0) {
             if (p.batch <= 32) {
+#ifdef COMEM_TRACE
+                if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
+#endif
                 const int mine = lane < p.batch ? seq_tiles(__ldcg(p.seq_lens + lane), p.window, p.sinks) : 0;
                 int incl = mine;
+#ifdef COMEM_TRACE
+                if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 12] = globaltimer_ns() + (mine == -12345);
+#endif
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int v = __shfl_up_sync(kFull, incl, o);
@@ -264,6 +270,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             if (lane == 0) s_aligned = ok ? 1 : 0;
         }
         __syncthreads();
+#ifdef COMEM_TRACE
+        if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 13] = globaltimer_ns();
+#endif
         // this CTA's range [c0, c1) of the linearised tile space
         total = (int64_t)p.num_kv_heads * prefix[p.batch];
         aligned = s_aligned != 0;
