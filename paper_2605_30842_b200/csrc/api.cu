@@ -6,6 +6,7 @@
 
 #include <atomic>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -650,8 +651,10 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
     const int64_t pair_pos = 2 * (int64_t)p.rows_per_tile;
     const int64_t items = ((int64_t)total_q / pair_pos + (batch < total_q ? batch : total_q)) * num_kv_heads;
     if (items >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
-    if (launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, (int)items, static_cast<cudaStream_t>(cuda_stream),
-                            pdl_for(opts)) != cudaSuccess) {
+    const cudaError_t le = launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, (int)items,
+                                               static_cast<cudaStream_t>(cuda_stream), pdl_for(opts));
+    if (le != cudaSuccess) {
+        if (std::getenv("COMEM_DEBUG_ERRORS")) fprintf(stderr, "comem_prefill_attn_async: %s\n", cudaGetErrorString(le));
         cudaGetLastError();
         return COMEM_ERR_CUDA;
     }

@@ -29,6 +29,7 @@
 // Everything that decides an output bit is a function of the logical problem (positions, never page ids),
 // and a row is computed by one thread in a fixed order: results are bit-identical under page permutation.
 #include <cstdio>
+#include <type_traits>
 #include "decode_params.cuh"
 #include "prefill_params.cuh"
 #include "ptx.cuh"
@@ -80,7 +81,8 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void *tmap,
 // score column (S = Q K^T as issued: see the header) -> token of the 128-token block
 __host__ __device__ constexpr int col_token(int col) { return 16 * ((col & 63) >> 3) + 8 * (col >> 6) + (col & 7); }
 
-template <int D>
+template <int D, bool kLse>
+// (168 registers is the most ten warps can have: two of the SM's four sub-partitions hold three of them)
 __global__ void __launch_bounds__(PfCfg<D>::kThreads, 1)
 prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                     const __grid_constant__ CUtensorMap tm_v, const PrefillParams p)
@@ -314,9 +316,15 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     for (int c = 0; c < 128; ++c)
                         if (col_token(c) > pos_rel) s[c] = -INFINITY;
                 }
-                float mr = s[0];
+                // (eight independent chains, then a tree: one thread per row means the row's 128 scores are one
+                // thread's instruction stream, and a single 127-deep fmax chain is 127 dependent issue slots)
+                float mr8[8];
 #pragma unroll
-                for (int c = 1; c < 128; ++c) mr = fmaxf(mr, s[c]);
+                for (int i = 0; i < 8; ++i) mr8[i] = s[i];
+#pragma unroll
+                for (int c = 8; c < 128; ++c) mr8[c & 7] = fmaxf(mr8[c & 7], s[c]);
+                const float mr = fmaxf(fmaxf(fmaxf(mr8[0], mr8[1]), fmaxf(mr8[2], mr8[3])),
+                                       fmaxf(fmaxf(mr8[4], mr8[5]), fmaxf(mr8[6], mr8[7])));
                 const float mx = (mr == -INFINITY) ? -INFINITY : mr * p.scale_log2;
                 const bool grow = mx > m_used + kRescaleThreshold;  // also the first block (m_used = -inf)
                 float factor = 1.f;
@@ -338,31 +346,39 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         tmem_st32(o_addr + 32 * c, o);
                     }
                 }
-                // p = 2^(s * scale - m), rounded to bf16; P word i holds tokens 2i, 2i+1 of the block
+                // p = 2^(s * scale - m), rounded to bf16; P word i holds tokens 2i, 2i+1 of the block.  Two copies of the
+                // loop, chosen once per block: only the blocks on the diagonal carry the per-element mask test (a
+                // predicated-off FSEL still takes its issue slot, and this loop is what the tensor pipe waits for), and
+                // the unrounded sum is kept only when the caller wants lse_out.
                 const float neg_m = -m_used;
-                float rsum = 0.f, xsum = 0.f;
+                auto exp_pass = [&](auto masked_tag) {
+                    constexpr bool kMasked = decltype(masked_tag)::value;
+                    float rs4[4] = {0.f, 0.f, 0.f, 0.f}, xs4[4] = {0.f, 0.f, 0.f, 0.f};  // independent partial sums (fixed order)
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    uint32_t pw[32];
+                    for (int h = 0; h < 2; ++h) {
+                        uint32_t pw[32];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const int w = 32 * h + i;                      // P word: tile w / 8, token pair (w % 8)
-                        const int tile = w >> 3, q = w & 7;
-                        const int col = (q >> 2) * 64 + tile * 8 + 2 * (q & 3);   // score column of token 16 tile + 2 q
-                        float e0 = ex2(fmaf(s[col], p.scale_log2, neg_m));
-                        float e1 = ex2(fmaf(s[col + 1], p.scale_log2, neg_m));
-                        if (masked) {  // (s = -inf and scale = 0 would give NaN above: decide by index)
-                            if (col_token(col) > pos_rel) e0 = 0.f;
-                            if (col_token(col + 1) > pos_rel) e1 = 0.f;
+                        for (int i = 0; i < 32; ++i) {
+                            const int w = 32 * h + i;                      // P word: tile w / 8, token pair (w % 8)
+                            const int tile = w >> 3, q = w & 7;
+                            const int col = (q >> 2) * 64 + tile * 8 + 2 * (q & 3);   // score column of token 16 tile + 2 q
+                            float e0 = ex2(fmaf(s[col], p.scale_log2, neg_m));
+                            float e1 = ex2(fmaf(s[col + 1], p.scale_log2, neg_m));
+                            if constexpr (kMasked) {  // (s = -inf and scale = 0 would give NaN above: decide by index)
+                                if (col_token(col) > pos_rel) e0 = 0.f;
+                                if (col_token(col + 1) > pos_rel) e1 = 0.f;
+                            }
+                            pw[i] = pack_bf16x2(e0, e1);
+                            rs4[i & 3] += bf16lo_to_f32(pw[i]) + bf16hi_to_f32(pw[i]);
+                            if constexpr (kLse) xs4[i & 3] += e0 + e1;
                         }
-                        pw[i] = pack_bf16x2(e0, e1);
-                        rsum += bf16lo_to_f32(pw[i]) + bf16hi_to_f32(pw[i]);
-                        xsum += e0 + e1;
+                        tmem_st32(s_addr + 32 * h, pw);
                     }
-                    tmem_st32(s_addr + 32 * h, pw);
-                }
-                l_run += rsum;
-                lx_run += xsum;
+                    l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+                    if constexpr (kLse) lx_run += (xs4[0] + xs4[1]) + (xs4[2] + xs4[3]);
+                };
+                if (masked) exp_pass(std::true_type{});
+                else exp_pass(std::false_type{});
                 tmem_wait_st();
                 tc_fence_before_sync();
                 mbar_arrive(p_full + 8 * t);
@@ -390,8 +406,10 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     }
                 }
             }
-            if (live && p.lse_out)
-                p.lse_out[grow_idx * p.num_q_heads + kvh * G + rg] = (m_used + log2f(lx_run)) * 0.69314718055994530942f;
+            if constexpr (kLse) {
+                if (live && p.lse_out)
+                    p.lse_out[grow_idx * p.num_q_heads + kvh * G + rg] = (m_used + log2f(lx_run)) * 0.69314718055994530942f;
+            }
         }
     }
     tc_fence_before_sync();
@@ -399,22 +417,31 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     if (warp == 9) tmem_dealloc<512>(tmem);
 }
 
-template <int D>
+template <int D, bool kLse>
 cudaError_t configure_prefill()
 {
     static PerDeviceOnce once;
-    return set_max_smem_once(prefill_attn_kernel<D>, PfCfg<D>::kSmemBytes, once);
+    return set_max_smem_once(prefill_attn_kernel<D, kLse>, PfCfg<D>::kSmemBytes, once);
 }
 
+template <int D, bool kLse>
+cudaError_t launch_prefill_inst(const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
+                                const PrefillParams &p, cudaLaunchConfig_t &cfg)
+{
+    const cudaError_t e = configure_prefill<D, kLse>();
+    if (e != cudaSuccess) return e;
+    cfg.blockDim = dim3(PfCfg<D>::kThreads);
+    cfg.dynamicSmemBytes = PfCfg<D>::kSmemBytes;
+    return cudaLaunchKernelEx(&cfg, prefill_attn_kernel<D, kLse>, tm_q, tm_k, tm_v, p);
+}
+
+// (the instance without lse_out skips the unrounded row sums: one FADD per score in the loop the tensor pipe waits for)
 template <int D>
 cudaError_t launch_prefill_variant(const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                                    const PrefillParams &p, cudaLaunchConfig_t &cfg)
 {
-    const cudaError_t e = configure_prefill<D>();
-    if (e != cudaSuccess) return e;
-    cfg.blockDim = dim3(PfCfg<D>::kThreads);
-    cfg.dynamicSmemBytes = PfCfg<D>::kSmemBytes;
-    return cudaLaunchKernelEx(&cfg, prefill_attn_kernel<D>, tm_q, tm_k, tm_v, p);
+    return p.lse_out ? launch_prefill_inst<D, true>(tm_q, tm_k, tm_v, p, cfg)
+                     : launch_prefill_inst<D, false>(tm_q, tm_k, tm_v, p, cfg);
 }
 
 }  // namespace
