@@ -50,7 +50,10 @@ struct PfCfg {
     static constexpr int kStageBytes = kTilesPerBlock * kTileBytes;   // one 128-token K (or V) block
     static constexpr int kQTileBytes = 128 * D * 2;
     static constexpr int kKStages = 2, kVStages = 2;
-    static constexpr int kThreads = 320;  // 2 softmax warpgroups + producer warp + MMA warp
+    // 2 softmax warpgroups + a third warpgroup holding the producer warp, the MMA warp and two idle warps (a whole
+    // warpgroup, so that it can hand its registers to the softmax warpgroups with setmaxnreg)
+    static constexpr int kThreads = 384;
+    static constexpr int kSoftmaxRegs = 208, kOtherRegs = 80;  // the CTA's own pool: 8 x (208 - 168) <= 4 x (168 - 80)
     static constexpr int kNumBars = 1 + 2 * kKStages + 2 * kVStages + 2 + 2 + 1;
     static constexpr int kSmemBytes = 1024 + 2 * kQTileBytes + (kKStages + kVStages) * kStageBytes + 8 * kNumBars + 64;
     static constexpr int kOCol = 256;     // TMEM column of O0; O1 follows at + D
@@ -82,7 +85,7 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void *tmap,
 __host__ __device__ constexpr int col_token(int col) { return 16 * ((col & 63) >> 3) + 8 * (col >> 6) + (col & 7); }
 
 template <int D, bool kLse>
-// (168 registers is the most ten warps can have: two of the SM's four sub-partitions hold three of them)
+// (compiled at 168 registers, the most twelve warps can be launched with; the softmax warps then grow to 232)
 __global__ void __launch_bounds__(PfCfg<D>::kThreads, 1)
 prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                     const __grid_constant__ CUtensorMap tm_v, const PrefillParams p)
@@ -182,6 +185,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     tc_fence_after_sync();
     const uint32_t tmem = s_tmem;
 
+    if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::kOtherRegs));
     if (warp == 8) {
         // ------------------------------ producer -------------------------------------------------
         if (lane == 0) {
@@ -284,7 +289,9 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         }
         if (lane == 0) umma_commit(o_full);
         __syncwarp();
+    }
     } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::kSoftmaxRegs));
         // ------------------------------ softmax + epilogue: one thread per row ---------------------
         const int t = warp >> 2;                       // tile of the pair
         const int r = 32 * (warp & 3) + lane;          // row of the tile == TMEM lane
