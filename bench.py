@@ -777,6 +777,7 @@ def run_fp8(args) -> int:
         pools.append(W.to_hnd(f8) if args.kv_layout == "hnd" else f8)
         del f8
     torch.cuda.empty_cache()
+    flags = DEFAULT_LAUNCH_FLAGS if args.launch_flags is None else args.launch_flags
     nbytes = pools[0].algorithmic_bytes()
     bf16_bytes = int(pools[0].seq_lens.to(torch.int64).sum().item()) * pools[0].num_kv_heads * pools[0].head_dim * 4
     stream = torch.cuda.Stream(device)
@@ -794,16 +795,17 @@ def run_fp8(args) -> int:
             b = pools[i % len(pools)]
             comem.comem_decode_attn_fp8_async(b.q, b.k_pages, b.v_pages, b.k_scale, b.v_scale, b.block_table,
                                               b.seq_lens, b.softmax_scale, outs[i % len(pools)], ws, stream=stream,
-                                              kv_layout=b.kv_layout)
+                                              kv_layout=b.kv_layout, flags=flags)
         for i in range(len(pools)):
             step(i)
         stream.synchronize()
-        per_graph = max(len(pools), 4)
+        est_us = nbytes / 5e6 + 8
+        # (a short step needs a long graph: consecutive steps overlap through programmatic launch only inside one)
+        per_graph = max(len(pools), 4, min(256, int(5e3 / est_us)))
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g, stream=stream):
             for i in range(per_graph):
                 step(i)
-        est_us = nbytes / 5e6 + 8
         replays = max(4, min(int(2e6 / (est_us * per_graph)), max(1, args.steps // per_graph)))
         for _ in range(3):
             g.replay()
@@ -892,6 +894,7 @@ def run_fp8(args) -> int:
                "d2h_bytes_per_step": out_h.numel() * 2, "steps": n_e2e,
                "api": "comem_decode_step_host_fp8, pinned host buffers (host wall clock around the synchronous calls)"}
     print(json.dumps({"extra": "FP8 (E4M3 + page scales) KV cache", "config": workload_desc(args.workload), "e2e": e2e,
+                      "launch_flags": flags,
                       "kv_layout": pools[0].kv_layout,
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
