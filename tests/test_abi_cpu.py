@@ -147,3 +147,37 @@ def test_fp8_entry_point_validates_before_any_launch(lib):
     assert call(sinks=-1) == comem.COMEM_ERR_INVALID_ARG
     # valid arguments get as far as the device check (no GPU here) or the launch (never reached with these pointers)
     assert call() in (comem.COMEM_ERR_CUDA, comem.COMEM_ERR_UNSUPPORTED, comem.COMEM_ERR_WORKSPACE)
+
+
+def test_round2_entry_points_validate_arguments_on_the_host(lib):
+    """Host-side validation of the round-2 calls (no device work is reached): null pointers, bad sizes, unknown launch
+    flags.  Each returns a status code; none crashes, none falls back to a CPU path."""
+    import ctypes as C
+    vp = C.c_void_p
+    lib.comem_pages_copy_async.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int, C.c_size_t, vp]
+    lib.comem_pages_copy_async.restype = C.c_int
+    buf = (C.c_char * 4096)()
+    p = C.cast(buf, vp)
+    assert lib.comem_pages_copy_async(None, p, p, p, p, p, 1, 4096, None) == comem.COMEM_ERR_INVALID_ARG
+    assert lib.comem_pages_copy_async(p, p, p, p, p, p, 1, 100, None) == comem.COMEM_ERR_INVALID_ARG      # not a multiple of 16
+    assert lib.comem_pages_copy_async(p, p, p, p, p, p, -1, 4096, None) == comem.COMEM_ERR_INVALID_ARG
+    lib.comem_decode_attn_offload_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
+                                                    vp, C.c_int, C.c_int, C.c_int64, C.c_int64, vp, vp, C.c_size_t, vp, vp]
+    lib.comem_decode_attn_offload_async.restype = C.c_int
+    assert lib.comem_decode_attn_offload_async(p, p, p, None, p, p, p, 8, 2, 128, 16, C.c_float(0.1), p, 1, 4, 8, 8, None, p,
+                                               1 << 30, None, None) == comem.COMEM_ERR_INVALID_ARG       # no host K pool
+    # unknown launch flag bits are rejected before anything is launched
+    opts = comem.LaunchOpts(0, -1, 1 << 10)
+    lib.comem_decode_attn_async.restype = C.c_int
+    st = lib.comem_decode_attn_async(p, p, p, p, p, 8, 2, 128, 16, C.c_float(0.1), p, 1, 4, 8, None, p,
+                                     comem.comem_decode_attn_workspace_bytes(1, 8, 2, 128, 16, 4), None, C.byref(opts))
+    assert st in (comem.COMEM_ERR_INVALID_ARG, comem.COMEM_ERR_WORKSPACE)
+    # the Algorithm-1 step scheduler: null model / event, bad token counts
+    ev = comem.KstepEvent(1, 0, 0, 1, 0, 0)
+    m = comem.KstepModel()
+    lib.comem_kstep_step_async.restype = C.c_int
+    assert lib.comem_kstep_step_async(None, 64, 32, 1, 0, C.byref(m), None, None, None, None, None, None) == comem.COMEM_ERR_INVALID_ARG
+    assert lib.comem_kstep_step_async(C.byref(ev), 64, 32, 1, 0, C.byref(m), None, None, None, None, None, None) == comem.COMEM_ERR_INVALID_ARG
+    lib.comem_decode_step_host_fp8.restype = C.c_int
+    assert lib.comem_decode_step_host_fp8(None, p, p, p, p, p, p, p, p, 8, 2, 128, 16, C.c_float(0.1), p, 1, 4, 8, None, p, 1 << 20,
+                                          None, 0) == comem.COMEM_ERR_INVALID_ARG
