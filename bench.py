@@ -246,11 +246,22 @@ def timed_steps(torch, comem, replicas, pools, outs, ws, stream, steps, warmup, 
         a, r = divmod(steps, chunk) if use_graph else (0, 0)
         g_full = capture(0, chunk) if a else None
         g_rest = capture(a * chunk, r) if r else None
-        sampler.warm = True          # the run-up: same kernels, same rate as the timed region
+        # the run-up: the same graphs at the same rate as the timed region, for >= 30 ms, so that the clock sampler
+        # (an NVML query takes about a millisecond) has a record of the SM clock under this very load even when the
+        # timed region itself lasts half a millisecond
         for g in (g_full, g_rest):
             if g is not None:
-                for _ in range(3):
+                r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                r0.record(stream)
+                g.replay()
+                r1.record(stream)
+                stream.synchronize()
+                n_run = max(3, min(2000, int(30.0 / max(r0.elapsed_time(r1), 1e-3)) + 1)) if use_graph else 3
+                sampler.warm = True
+                for _ in range(n_run):
                     g.replay()
+                stream.synchronize()
+                sampler.warm = False
         stream.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         replicas.barrier()
