@@ -66,7 +66,8 @@ enum {
  *   grid_ctas            > 0: size of this call's persistent decode grid (its share of the SMs: the agent batch and
  *                        the memory-model batch of the k-step-off pipeline, run side by side when their
  *                        grids sum to the SM count; comem_sm_partition picks the split).  0: the default
- *                        (comem_set_grid_ctas' value if set, else one CTA per SM).  Ignored by the prefill kernel.
+ *                        (comem_set_grid_ctas' value if set, else one CTA per SM).  comem_prefill_attn_async: > 0 makes the prefill
+ *                        kernel persistent on that many SMs (default there: one CTA per work item).
  *   programmatic_launch  1 / 0: launch with / without programmatic stream serialization (the next launch of the
  *                        stream starts its prologue on SMs the previous one has released: shortest back-to-back steps,
  *                        but a stream's NEXT kernel then parks on every free SM; use 0 with an SM partition).

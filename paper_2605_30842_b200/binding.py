@@ -475,7 +475,7 @@ def comem_kv_append_fp8_async(k_pages, v_pages, k_scale, v_scale, block_table, s
 
 
 def comem_prefill_attn_async(q, k_pages, v_pages, block_table, seq_lens, q_start, softmax_scale: float, out,
-                             lse_out=None, stream=None, programmatic_launch=None) -> None:
+                             lse_out=None, stream=None, programmatic_launch=None, grid_ctas=None) -> None:
     """Causal prefill attention of each sequence's last q_start[b+1] - q_start[b] tokens over the paged cache
     (one tcgen05 kernel on ``stream``).  q, out: bf16 [total_q, Hq, D]; q_start: int32 [batch + 1] on the device."""
     assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.dim() == 3
@@ -492,7 +492,7 @@ def comem_prefill_attn_async(q, k_pages, v_pages, block_table, seq_lens, q_start
         _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), _ptr(q_start), q.shape[1],
         k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
         block_table.shape[0], q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _stream(stream),
-        _opts(None, programmatic_launch))
+        _opts(grid_ctas, programmatic_launch))
     if st != COMEM_OK:
         raise ComemError(st, "comem_prefill_attn_async")
 

@@ -651,7 +651,11 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
     const int64_t pair_pos = 2 * (int64_t)p.rows_per_tile;
     const int64_t items = ((int64_t)total_q / pair_pos + (batch < total_q ? batch : total_q)) * num_kv_heads;
     if (items >= (int64_t)1 << 31) return COMEM_ERR_UNSUPPORTED;
-    const cudaError_t le = launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, (int)items,
+    // default: one CTA per work item (the hardware scheduler balances them); with grid_ctas the kernel is persistent on
+    // that many SMs and each CTA takes every grid_ctas-th item (the SM-partition policy of the k-step-off pipeline)
+    int grid = (int)items;
+    if (opts && opts->grid_ctas > 0 && opts->grid_ctas < grid) grid = opts->grid_ctas;
+    const cudaError_t le = launch_prefill_attn(tm_q, tm_k, tm_v, p, head_dim, grid,
                                                static_cast<cudaStream_t>(cuda_stream), pdl_for(opts));
     if (le != cudaSuccess) {
         if (std::getenv("COMEM_DEBUG_ERRORS")) fprintf(stderr, "comem_prefill_attn_async: %s\n", cudaGetErrorString(le));

@@ -109,6 +109,7 @@ extern "C" int comem_kstep_step_async(const comem_kstep_event *e, int turn_token
     st_.memory_in_flight = in_flight ? 1 : 0;
 
     // the agent's share of the SMs while a memory job runs beside it: proportional to the bytes each streams per step
+    // (decode grids and the persistent prefill grid alike)
     comem_launch_opts oa = {0, -1, 0};
     if (in_flight) {
         int ga = 0, gm = 0;

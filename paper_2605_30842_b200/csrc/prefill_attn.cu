@@ -110,14 +110,20 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int R = p.rows_per_tile, G = p.group;
 
-    if (threadIdx.x == 0) {
-        mbar_init(q_full, 1);
-        for (int s = 0; s < C::kKStages; ++s) { mbar_init(k_full + 8 * s, 1); mbar_init(k_empty + 8 * s, 1); }
-        for (int s = 0; s < C::kVStages; ++s) { mbar_init(v_full + 8 * s, 1); mbar_init(v_empty + 8 * s, 1); }
-        for (int t = 0; t < 2; ++t) { mbar_init(s_full + 8 * t, 1); mbar_init(p_full + 8 * t, 128); }
-        mbar_init(o_full, 1);
+    // (thread 0; `again`: a persistent CTA starts its next work item with every barrier back in phase 0)
+    auto init_barriers = [&](bool again) {
+        auto one = [&](uint32_t bar, uint32_t count) {
+            if (again) mbar_inval(bar);
+            mbar_init(bar, count);
+        };
+        one(q_full, 1);
+        for (int s = 0; s < C::kKStages; ++s) { one(k_full + 8 * s, 1); one(k_empty + 8 * s, 1); }
+        for (int s = 0; s < C::kVStages; ++s) { one(v_full + 8 * s, 1); one(v_empty + 8 * s, 1); }
+        for (int t = 0; t < 2; ++t) { one(s_full + 8 * t, 1); one(p_full + 8 * t, 128); }
+        one(o_full, 1);
         fence_mbar_init();
-    }
+    };
+    if (threadIdx.x == 0) init_barriers(false);
     if (warp == 8 && lane == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -126,10 +132,12 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     pdl_wait_prior_grid();  // q, q_start, seq_lens and the cache may come from the kernels queued before this one
 
     // ---- which work item: items are ordered (sequence, kv head, pair of query tiles from the LAST pair down) ----
-    // (the CTAs resident together then stream the same kv head's cache, which stays in L2, and the long items run first)
-    if (warp == 0) {
+    // (the CTAs resident together then stream the same kv head's cache, which stays in L2, and the long items run first).
+    // A CTA takes the items blockIdx.x, blockIdx.x + gridDim.x, ...: with the default grid (one CTA per item) that is
+    // one item; with comem_launch_opts.grid_ctas the kernel is persistent on that many SMs (the memory model's prefill
+    // beside the agent's decode steps, section 5c of DESIGN.md).  Warp 0 looks the item up and publishes it in s_item.
+    auto find_item = [&](const long long idx) {
         const int P2 = 2 * R, hkv = p.num_kv_heads;
-        const long long idx = blockIdx.x;
         long long before = 0;  // pairs of the sequences before this chunk of 32
         int found = 0;
         for (int b0 = 0; b0 < p.batch && !found; b0 += 32) {
@@ -166,18 +174,17 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             before += __shfl_sync(kAll, incl, 31);
         }
         if (lane == 0) s_item[6] = found;
-    }
-    __syncthreads();
-    pdl_launch_dependents();
-    if (!s_item[6]) return;  // the grid is an upper bound on the number of items
-    const int b = s_item[0], kvh = s_item[1], i0 = s_item[2], n_b = s_item[3], L_b = s_item[4], qs = s_item[5];
-    const int nv = min(2 * R, n_b - i0);            // valid positions of the pair
-    const bool act1 = nv > R;                        // does tile 1 hold any valid row?
-    const int pos0 = L_b - n_b + i0;                 // position of the pair's first query
-    const int kv_need = pos0 + nv;                   // keys 0 .. pos_hi are needed, pos_hi = pos0 + nv - 1
-    const int ntiles = (kv_need + 15) >> 4;
-    const int nblk = (ntiles + kTilesPerBlock - 1) / kTilesPerBlock;
-    if (nblk <= 0) return;                           // n_b > L_b: invalid input (documented as undefined); no hang
+    };
+// the published item, read by every thread after barrier A of the item loop
+#define COMEM_PF_ITEM()                                                                                              \
+    const int b = s_item[0], kvh = s_item[1], i0 = s_item[2], n_b = s_item[3], L_b = s_item[4], qs = s_item[5];       \
+    const int nv = min(2 * R, n_b - i0);            /* valid positions of the pair */                                 \
+    const bool act1 = nv > R;                        /* does tile 1 hold any valid row? */                             \
+    const int pos0 = L_b - n_b + i0;                 /* position of the pair's first query */                          \
+    const int kv_need = pos0 + nv;                   /* keys 0 .. pos_hi are needed, pos_hi = pos0 + nv - 1 */          \
+    const int ntiles = (kv_need + 15) >> 4;                                                                           \
+    const int nblk = (ntiles + kTilesPerBlock - 1) / kTilesPerBlock;                                                  \
+    (void)b; (void)kvh; (void)qs; (void)act1; (void)L_b
 
     if (warp == 9) tmem_alloc<512>(smem_u32(&s_tmem));
     tc_fence_before_sync();
@@ -185,8 +192,16 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     tc_fence_after_sync();
     const uint32_t tmem = s_tmem;
 
+    // Item loop, once per role group (the register split must dominate each group's code).  Per item: barrier A (the
+    // item is published, the barriers are fresh), the roles, barrier B (everybody is done with the item).
     if (warp >= 8) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::kOtherRegs));
+    for (bool first = true;; first = false) {
+    __syncthreads();  // A
+    if (first) pdl_launch_dependents();
+    if (!s_item[6]) break;  // past the last item (the grid is an upper bound on the number of items)
+    COMEM_PF_ITEM();
+    if (nblk <= 0) { __syncthreads(); continue; }  // n_b > L_b: invalid input (documented as undefined); no hang
     if (warp == 8) {
         // ------------------------------ producer -------------------------------------------------
         if (lane == 0) {
@@ -290,8 +305,20 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         if (lane == 0) umma_commit(o_full);
         __syncwarp();
     }
+    tc_fence_before_sync();
+    __syncthreads();  // B
+    }
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::kSoftmaxRegs));
+        for (long long idx = blockIdx.x;; idx += gridDim.x) {
+        if (warp == 0) find_item(idx);
+        if (threadIdx.x == 0 && idx != (long long)blockIdx.x) init_barriers(true);
+        __syncthreads();  // A
+        if (idx == (long long)blockIdx.x) pdl_launch_dependents();
+        if (!s_item[6]) break;
+        COMEM_PF_ITEM();
+        if (nblk <= 0) { __syncthreads(); continue; }
+        tc_fence_after_sync();
         // ------------------------------ softmax + epilogue: one thread per row ---------------------
         const int t = warp >> 2;                       // tile of the pair
         const int r = 32 * (warp & 3) + lane;          // row of the tile == TMEM lane
@@ -418,7 +445,11 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     p.lse_out[grow_idx * p.num_q_heads + kvh * G + rg] = (m_used + log2f(lx_run)) * 0.69314718055994530942f;
             }
         }
+        tc_fence_before_sync();
+        __syncthreads();  // B
+        }
     }
+#undef COMEM_PF_ITEM
     tc_fence_before_sync();
     __syncthreads();
     if (warp == 9) tmem_dealloc<512>(tmem);

@@ -73,3 +73,23 @@ def test_page_permutation_bit_identical():
     out2, _ = gpu_prefill(pb, want_lse=False)
     torch.cuda.synchronize()
     assert torch.equal(out0.view(torch.int16), out2.view(torch.int16))
+
+
+@pytest.mark.parametrize("grid", [1, 3, 16, 100, 100000])
+def test_persistent_grid_is_bit_identical(grid):
+    """comem_launch_opts.grid_ctas on the prefill call: the kernel becomes persistent on that many SMs (each CTA takes every
+    grid-th work item, re-initialising its barriers in between).  A row is computed by one thread in a fixed order
+    whatever CTA runs it, so the bits are those of the default launch; with and without lse_out."""
+    pb = W.make_prefill_batch([700, 4100, 33, 1], [700, 300, 33, 1], 32, 4, 128, 16, seed=811, device="cuda", poison_unused=True)
+    ref, ref_lse = gpu_prefill(pb)
+    out = torch.full_like(pb.q, float("nan"))
+    lse = torch.full((pb.total_q, pb.num_q_heads), float("nan"), dtype=torch.float32, device="cuda")
+    comem.comem_prefill_attn_async(pb.q, pb.k_pages, pb.v_pages, pb.block_table, pb.seq_lens, pb.q_start, pb.softmax_scale,
+                                   out, lse_out=lse, grid_ctas=grid)
+    out2 = torch.full_like(pb.q, float("nan"))
+    comem.comem_prefill_attn_async(pb.q, pb.k_pages, pb.v_pages, pb.block_table, pb.seq_lens, pb.q_start, pb.softmax_scale,
+                                   out2, grid_ctas=grid)
+    torch.cuda.synchronize()
+    assert torch.equal(out.view(torch.int16), ref.view(torch.int16))
+    assert torch.equal(out2.view(torch.int16), ref.view(torch.int16))
+    assert torch.equal(lse.view(torch.int32), ref_lse.view(torch.int32))
