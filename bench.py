@@ -589,9 +589,10 @@ def run_c5(args) -> int:
 
 
 def run_affine(args) -> int:
-    """SURVEY.md §8(d) affine check of eq. 5 (t = L*S/W): batch 16, 64q/8kv, D 128, page 16,
-    context L in {4K .. 128K}; least-squares fit t = a + b*L.  16 * 4096 B / b is the streaming rate,
-    a the fixed cost per step.  One JSON line; an extra, not the driver's bench line."""
+    """SURVEY.md §8(d) affine check of eq. 5 (t = L*S/W) at the paper's batch sizes (Fig. 2, L84-92: batch 1 /
+    16 / 64; section 4.4, L257: 32 -> 256): 64q/8kv, D 128, page 16, context L from 1K up to what 16 GiB of K+V hold;
+    least-squares fit t = a + b*L per batch.  batch * 4096 B / b is the streaming rate W, a the fixed cost per step
+    (Fig. 2's shape: flat while a dominates, linear beyond).  One JSON line; an extra, not the driver's bench line."""
     import numpy as np
     import torch
     import paper_2605_30842_b200 as comem
@@ -603,42 +604,51 @@ def run_affine(args) -> int:
     cuda_build.build()
     comem.load_library()
     stream = torch.cuda.Stream(device)
-    B, pts = 16, []
-    for L in (4096, 8192, 16384, 32768, 65536, 131072):
-        R = max(1, min(8, (1 << 30) // (B * L * 4096)))          # rotate pools while one step is < 1 GiB (L2-cold)
-        pools = [W.make_batch([L] * B, 64, 8, 128, 16, 7000 + i, device) for i in range(R)]
-        outs = [torch.empty_like(b.q) for b in pools]
-        ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream)
-        with torch.cuda.stream(stream):
-            def enq():
-                for b, o in zip(pools, outs):
-                    comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
-                                                  b.softmax_scale, o, ws, stream=stream)
-            enq()
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                enq()
-            for _ in range(3):
-                g.replay()
-            n = max(2, int(20e-3 / (B * L * 4096 / 7e12) / R))     # ~20 ms of streaming per point
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            stream.synchronize()
-            e0.record(stream)
-            for _ in range(n):
-                g.replay()
-            e1.record(stream)
-            stream.synchronize()
-        us = e0.elapsed_time(e1) / (n * R) * 1e3
-        pts.append((L, us, pools[0].algorithmic_bytes() / us / 1e3))
-        del pools, outs, ws, g
-        torch.cuda.empty_cache()
-    Ls, ts = np.array([p[0] for p in pts], float), np.array([p[1] for p in pts], float)
-    b_fit, a_fit = np.polyfit(Ls, ts, 1)
-    print(json.dumps({"affine_check": "t_us = a + b * L at batch 16, 64q/8kv, D128, page 16 (PAPER.md eq. 5)",
-                      "points": [{"L": int(l), "us_per_step": round(u, 2), "gbs": round(gb, 1)} for l, u, gb in pts],
-                      "a_us": a_fit, "b_us_per_token": b_fit, "slope_gbs": B * 4096 / b_fit / 1e3,
-                      "max_rel_residual": float(np.max(np.abs(a_fit + b_fit * Ls - ts) / ts))}), flush=True)
+    flags = DEFAULT_LAUNCH_FLAGS if args.launch_flags is None else args.launch_flags
+    rows = []
+    for B in (1, 16, 64, 128, 256):
+        pts = []
+        for L in (1024, 4096, 8192, 16384, 32768, 65536, 131072):
+            if B * L * 4096 > (16 << 30):
+                continue
+            R = max(1, min(8, (1 << 30) // (B * L * 4096)))          # rotate pools while one step is < 1 GiB (L2-cold)
+            pools = [W.make_batch([L] * B, 64, 8, 128, 16, 7000 + i, device) for i in range(R)]
+            outs = [torch.empty_like(b.q) for b in pools]
+            ws = comem.alloc_workspace(pools[0].q, pools[0].k_pages, pools[0].block_table, stream=stream)
+            est_us = B * L * 4096 / 7e6 + 10
+            per_graph = max(R, min(256, int(5e3 / est_us)))           # short steps need a long graph (PDL overlap)
+            with torch.cuda.stream(stream):
+                def enq(n):
+                    for i in range(n):
+                        b = pools[i % R]
+                        comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens,
+                                                      b.softmax_scale, outs[i % R], ws, stream=stream, flags=flags)
+                enq(R)
+                stream.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=stream):
+                    enq(per_graph)
+                for _ in range(3):
+                    g.replay()
+                n = max(2, int(20e3 / (est_us * per_graph)))         # ~20 ms of streaming per point
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                stream.synchronize()
+                e0.record(stream)
+                for _ in range(n):
+                    g.replay()
+                e1.record(stream)
+                stream.synchronize()
+            us = e0.elapsed_time(e1) / (n * per_graph) * 1e3
+            pts.append((L, us, pools[0].algorithmic_bytes() / us / 1e3))
+            del pools, outs, ws, g
+            torch.cuda.empty_cache()
+        Ls, ts = np.array([p[0] for p in pts], float), np.array([p[1] for p in pts], float)
+        b_fit, a_fit = np.polyfit(Ls, ts, 1)
+        rows.append({"batch": B, "points": [{"L": int(l), "us_per_step": round(u, 2), "gbs": round(gb, 1)} for l, u, gb in pts],
+                     "a_us": a_fit, "b_us_per_token": b_fit, "slope_gbs": B * 4096 / b_fit / 1e3,
+                     "max_rel_residual": float(np.max(np.abs(a_fit + b_fit * Ls - ts) / ts))})
+    print(json.dumps({"affine_check": "t_us = a + b * L per batch, 64q/8kv, D128, page 16 (PAPER.md eq. 5, Fig. 2)",
+                      "launch_flags": flags, "batches": rows}), flush=True)
     return 0
 
 
