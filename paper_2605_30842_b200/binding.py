@@ -552,6 +552,39 @@ def comem_decode_step_host(q_host, new_k_host, new_v_host, k_pages, v_pages, blo
         raise ComemError(st, "comem_decode_step_host")
 
 
+class DecodeStepHost:
+    """comem_decode_step_host with the arguments marshalled ONCE: a serving loop calls the same step on the same
+    buffers thousands of times, and building twenty ctypes arguments from torch tensors costs more host time than the
+    GPU needs for a 32K-token step.  ``step = DecodeStepHost(...)`` checks and converts everything, ``step()`` is one
+    foreign call.  The tensors must stay alive and in place; ``rebind(q_host=..., new_k_host=..., new_v_host=...,
+    out_host=...)`` swaps host buffers (e.g. a ring of pinned rows) without re-marshalling the rest."""
+
+    def __init__(self, q_host, new_k_host, new_v_host, k_pages, v_pages, block_table, seq_lens, softmax_scale: float,
+                 out_host, workspace, lse_host=None, stream=None):
+        assert q_host.device.type == "cpu" and out_host.device.type == "cpu"
+        assert q_host.dtype == torch.bfloat16 and out_host.dtype == torch.bfloat16
+        assert q_host.is_contiguous() and out_host.is_contiguous() and out_host.shape == q_host.shape
+        self._fn = load_library().comem_decode_step_host
+        self._keep = (q_host, new_k_host, new_v_host, k_pages, v_pages, block_table, seq_lens, out_host, workspace, lse_host)
+        self._args = [_ptr(q_host), _ptr(new_k_host), _ptr(new_v_host), _ptr(k_pages), _ptr(v_pages), _ptr(block_table),
+                      _ptr(seq_lens), q_host.shape[1], k_pages.shape[2], q_host.shape[2], k_pages.shape[1],
+                      ctypes.c_float(softmax_scale), _ptr(out_host), q_host.shape[0], block_table.shape[1],
+                      k_pages.shape[0], _ptr(lse_host), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                      _stream(stream)]
+
+    def rebind(self, q_host=None, new_k_host=None, new_v_host=None, out_host=None):
+        for i, t in ((0, q_host), (1, new_k_host), (2, new_v_host), (12, out_host)):
+            if t is not None:
+                assert t.device.type == "cpu" and t.is_contiguous()
+                self._args[i] = _ptr(t)
+        self._keep = self._keep + (q_host, new_k_host, new_v_host, out_host)
+        return self
+
+    def __call__(self) -> None:
+        st = self._fn(*self._args)
+        if st != COMEM_OK:
+            raise ComemError(st, "comem_decode_step_host")
+
 
 def comem_decode_step_host_fp8(q_host, new_k_host, new_v_host, k_pages, v_pages, k_scale, v_scale, block_table, seq_lens,
                                softmax_scale: float, out_host, workspace, lse_host=None, stream=None,

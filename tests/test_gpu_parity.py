@@ -198,6 +198,22 @@ def test_decode_step_host(oracle):
     assert np.max(np.abs(lse_h.numpy().reshape(-1) - ref_lse)) < 1e-3
 
 
+def test_decode_step_host_prebound_call_object():
+    """comem.DecodeStepHost (arguments marshalled once) drives the same C entry point: over a few steps, with the host
+    rows swapped through rebind(), it leaves the cache, the lengths and the outputs exactly as the plain call does."""
+    a = W.make_batch([900, 47], 16, 2, 128, 16, seed=64, device=DEV, spare_tokens=8)
+    b = W.make_batch([900, 47], 16, 2, 128, 16, seed=64, device=DEV, spare_tokens=8)
+    wa, wb = comem.alloc_workspace(a.q, a.k_pages, a.block_table), comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    rows = [tuple(t.cpu().pin_memory() for t in W.decode_step_rows(a, i, 6400)) for i in range(5)]
+    oa, ob = torch.empty_like(rows[0][0]).pin_memory(), torch.empty_like(rows[0][0]).pin_memory()
+    step = comem.DecodeStepHost(*rows[0], b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, ob, wb)
+    for i, (q, nk, nv) in enumerate(rows):
+        comem.comem_decode_step_host(q, nk, nv, a.k_pages, a.v_pages, a.block_table, a.seq_lens, a.softmax_scale, oa, wa)
+        step.rebind(q_host=q, new_k_host=nk, new_v_host=nv)()
+        assert torch.equal(oa.view(torch.int16), ob.view(torch.int16)), i
+    assert torch.equal(a.seq_lens, b.seq_lens) and torch.equal(a.k_pages.view(torch.int16), b.k_pages.view(torch.int16))
+
+
 def test_decode_step_host_pageable_fallback(oracle):
     """Pageable (un-pinned) host buffers take the cudaMemcpyAsync path; same answer as the zero-copy path."""
     outs = []
