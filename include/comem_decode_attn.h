@@ -462,6 +462,10 @@ int comem_schedule_host(const int32_t *seq_lens_host, int batch, int num_kv_head
  * COMEM_ERR_INVALID_ARG.  With the environment variable COMEM_DEBUG_VALIDATE=1 the synchronous
  * entry points (comem_decode_attn, comem_decode_step_host) run it first and return its verdict
  * instead of computing on bad data; the *_async entry points never validate.
+ * COMEM_DEBUG_STALE_GUESS=1 (read once per process) is a testing aid for the decode kernel's recovery paths: every launch
+ * computes its first, speculative split-KV schedule from lengths 16 tokens short -- as if the append kernel queued before
+ * it had not run yet -- so the validation after the wait fails on every launch and the schedule is recomputed (classic
+ * order) or the early attempt aborted and rerun (COMEM_LAUNCH_KV_PREFIX_IMMUTABLE).  Results are unchanged, bit for bit.
  */
 int comem_validate_inputs(const int32_t *block_table, const int32_t *seq_lens, int batch,
                           int max_pages_per_seq, int page_size, int64_t num_pages, void *workspace,

@@ -259,6 +259,13 @@ bool debug_validate()
     return on;
 }
 
+// testing aid for the kernel's recovery paths (a schedule guess that fails its validation): see decode_split.cu
+bool debug_stale_guess()
+{
+    static const bool on = [] { const char *e = std::getenv("COMEM_DEBUG_STALE_GUESS"); return e && e[0] == '1'; }();
+    return on;
+}
+
 bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 }  // namespace
@@ -453,6 +460,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
 
     DecodeParams p;
     p.host_tier = host_tier ? 1 : 0;
+    p.debug_stale_guess = debug_stale_guess() ? 1 : 0;
     p.k_scale = kv_fp8 ? k_scale : nullptr;
     p.v_scale = kv_fp8 ? v_scale : nullptr;
     p.kv_hnd = hnd;

@@ -40,6 +40,7 @@ struct DecodeParams {
                                  // grid starts writes K/V rows (or their block-table entries / page scales) below each
                                  // sequence's last 16-token tile, so the ring may be filled before griddepcontrol.wait
     int q_stable;                // COMEM_LAUNCH_Q_STABLE: ... nor q: the consumers may start before the wait too
+    int debug_stale_guess;       // COMEM_DEBUG_STALE_GUESS=1 (testing aid): the speculative schedule is computed from stale lengths
     int host_tier;               // a second pool in pinned host memory is addressed by block-table entries < 0 (bf16 only)
     int kv_hnd;                  // FP8 cache only: pools laid out [P][Hkv][ps][D] (a tile is 2 KiB contiguous) instead of [P][ps][Hkv][D]
 };

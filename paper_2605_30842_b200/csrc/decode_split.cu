@@ -205,6 +205,10 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     int nc = 0, al_first = 0, al_count = 0;  // aligned: first CTA and CTA count of this CTA's segment
     bool aligned = false;
     const int cta = blockIdx.x;
+    // (COMEM_DEBUG_STALE_GUESS=1, a testing aid: the FIRST schedule is computed from lengths 16 tokens short, as if the
+    // append kernel had not run yet, so that the validation fails and the recovery paths run on every launch)
+    int guess_bias = p.debug_stale_guess ? kTileTokens : 0;
+    auto guess_len = [&](int L) { return L > guess_bias ? L - guess_bias : L; };
     auto compute_schedule = [&]() {
         // exclusive prefix of tiles per sequence (warp 0); kept small: no unrolling
         if (warp == 0) {
@@ -212,7 +216,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
 #ifdef COMEM_TRACE
                 if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 11] = globaltimer_ns();
 #endif
-                const int mine = lane < p.batch ? seq_tiles(__ldcg(p.seq_lens + lane), p.window, p.sinks) : 0;
+                const int mine = lane < p.batch ? seq_tiles(guess_len(__ldcg(p.seq_lens + lane)), p.window, p.sinks) : 0;
                 int incl = mine;
 #ifdef COMEM_TRACE
                 if (p.trace && threadIdx.x == 0) p.trace[blockIdx.x * 16 + 12] = globaltimer_ns() + (mine == -12345);
@@ -230,7 +234,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 int sum = 0;
 #pragma unroll 1
                 for (int i = 0; i < per; ++i)
-                    if (b0 + i < p.batch) sum += seq_tiles(__ldcg(p.seq_lens + b0 + i), p.window, p.sinks);
+                    if (b0 + i < p.batch) sum += seq_tiles(guess_len(__ldcg(p.seq_lens + b0 + i)), p.window, p.sinks);
                 int incl = sum;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -242,7 +246,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 for (int i = 0; i < per; ++i)
                     if (b0 + i < p.batch) {
                         prefix[b0 + i] = run;
-                        run += seq_tiles(__ldcg(p.seq_lens + b0 + i), p.window, p.sinks);
+                        run += seq_tiles(guess_len(__ldcg(p.seq_lens + b0 + i)), p.window, p.sinks);
                     }
                 if (lane == 31) prefix[p.batch] = incl;
             }
@@ -301,6 +305,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         }
     };
     compute_schedule();  // speculative
+    guess_bias = 0;        // (any later call computes the real schedule)
     // EARLY MODE (COMEM_LAUNCH_KV_PREFIX_IMMUTABLE, p.kv_immutable): the caller has PROMISED that nothing still running
     // writes the cached rows below each sequence's last tile, their block-table entries or their page scales.  Then
     // this CTA does not sit in griddepcontrol.wait while the previous kernel drains: its producers stream those tiles

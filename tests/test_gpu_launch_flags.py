@@ -142,3 +142,50 @@ def test_early_mode_with_growing_context(flags):
     torch.cuda.synchronize()
     for step in range(steps):
         assert torch.equal(bits(o3[step]), bits(o2[step])), step
+
+
+def test_recovery_paths_forced_by_a_stale_schedule_guess():
+    """COMEM_DEBUG_STALE_GUESS=1 makes every launch compute its first schedule from lengths 16 tokens short: the
+    validation after the wait fails on every launch, so the classic re-computation and the early mode's abort (drain,
+    barrier re-initialisation, rerun in the classic order) run deterministically.  In a fresh process (the switch is
+    read once), every flag combination must give the bits of an un-flagged run of THIS process."""
+    import os
+    import subprocess
+    import sys
+    code = r'''
+import torch
+import paper_2605_30842_b200 as comem
+from paper_2605_30842_b200 import workloads as W
+def bits(t): return t.contiguous().view(torch.int16)
+ok = True
+for lens, hq, hkv, d, ps in [([32768], 64, 8, 128, 16), ([20000, 37, 0, 50001, 8191, 16, 300], 64, 8, 128, 16), ([700, 64, 4097], 12, 3, 64, 32), ([17], 8, 1, 128, 16)]:
+    b = W.make_batch(lens, hq, hkv, d, ps, seed=901, device="cuda", poison_unused=True)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    outs = {}
+    for flags in (0, 1, 5, 7, 2):
+        o = torch.full_like(b.q, float("nan"))
+        for _ in range(3):
+            comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, o, ws, flags=flags)
+        torch.cuda.synchronize()
+        outs[flags] = o
+    ok = ok and torch.isfinite(outs[0].float()).all().item()
+    ok = ok and torch.equal(bits(outs[0]), bits(outs[1])) and torch.equal(bits(outs[0]), bits(outs[5]))
+    ok = ok and torch.equal(bits(outs[2]), bits(outs[7]))
+    f = W.quantize_batch_fp8(b) if d == 128 else None
+    if f is not None:
+        ws8 = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+        o8 = {}
+        for flags in (0, 5):
+            o = torch.full_like(f.q, float("nan"))
+            comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens, f.softmax_scale, o, ws8, flags=flags)
+            torch.cuda.synchronize()
+            o8[flags] = o
+        ok = ok and torch.equal(bits(o8[0]), bits(o8[5]))
+print("RESULT", ok)
+'''
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    ref = {}
+    for stale in ("0", "1"):
+        env = dict(os.environ, COMEM_DEBUG_STALE_GUESS=stale, PYTHONPATH=root)
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        assert "RESULT True" in r.stdout, (stale, r.stdout[-500:], r.stderr[-1500:])
