@@ -387,7 +387,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 const float neg_m = -m_used;
                 auto exp_pass = [&](auto masked_tag) {
                     constexpr bool kMasked = decltype(masked_tag)::value;
-                    float rs4[4] = {0.f, 0.f, 0.f, 0.f}, xs4[4] = {0.f, 0.f, 0.f, 0.f};  // independent partial sums (fixed order)
+                    float rs4[4] = {0.f, 0.f, 0.f, 0.f};  // independent partial sums (fixed order)
+                    [[maybe_unused]] float xs4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         uint32_t pw[32];
