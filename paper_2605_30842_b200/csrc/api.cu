@@ -126,11 +126,11 @@ EncodeFn encode_fn()
 struct MapKey {
     const void *ptr;
     int64_t num_pages;
-    int ps, hkv, d, elem_bytes, hnd;
+    int ps, hkv, d, elem_bytes, hnd, box_rows;
     bool operator==(const MapKey &o) const
     {
         return ptr == o.ptr && num_pages == o.num_pages && ps == o.ps && hkv == o.hkv && d == o.d &&
-               elem_bytes == o.elem_bytes && hnd == o.hnd;
+               elem_bytes == o.elem_bytes && hnd == o.hnd && box_rows == o.box_rows;
     }
 };
 struct MapEntry {
@@ -142,13 +142,16 @@ struct MapEntry {
 //   dim0 = 128 bytes of d, dim1 = P * ps token rows (stride Hkv*D B), dim2 = 1, dim3 = Hkv (stride D B),
 // box {128, 16, 1, 1}: a [16 tokens][128 B] tile, 128-byte swizzled, read with 16-byte shared loads.
 // HND layout [P][Hkv][ps][D]: dim1 = ps slots (stride D B), dim2 = Hkv (stride ps*D B), dim3 = P (stride Hkv*ps*D B).
+// box_rows: token rows per box of the bf16 map: 16 (a whole tile, the decode kernels and the prefill kernel's V), or 8
+// (the prefill kernel's K: half tiles, so that the 8-row groups of a 128-token block sit at one uniform pitch and
+// S = Q K^T is one N = 128 instruction per k-step).
 int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, CUtensorMap *out, int elem_bytes = 2,
-                   int hnd = 0)
+                   int hnd = 0, int box_rows = kTileTokens)
 {
     static std::mutex mu;
     static std::vector<MapEntry> cache;
     static size_t next_evict = 0;
-    const MapKey key{pool, num_pages, ps, hkv, d, elem_bytes, hnd};
+    const MapKey key{pool, num_pages, ps, hkv, d, elem_bytes, hnd, box_rows};
     std::lock_guard<std::mutex> lock(mu);
     for (const MapEntry &e : cache)
         if (e.key == key) { *out = e.map; return COMEM_OK; }
@@ -156,7 +159,7 @@ int get_tensor_map(const void *pool, int64_t num_pages, int ps, int hkv, int d, 
     if (!enc) return COMEM_ERR_CUDA;
     const cuuint64_t gdim[4] = {64, (cuuint64_t)num_pages * ps, (cuuint64_t)(d / 64), (cuuint64_t)hkv};
     const cuuint64_t gstride[3] = {(cuuint64_t)hkv * d * 2, 128, (cuuint64_t)d * 2};
-    const cuuint32_t box[4] = {64, (cuuint32_t)kTileTokens, (cuuint32_t)(d / 64), 1};
+    const cuuint32_t box[4] = {64, (cuuint32_t)box_rows, (cuuint32_t)(d / 64), 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     MapEntry e;
     e.key = key;
@@ -653,7 +656,7 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
 
     CUtensorMap tm_q, tm_k, tm_v;
     if ((st = make_q_tensor_map(q, total_q, num_q_heads, head_dim, g, p.rows_per_tile, &tm_q)) != COMEM_OK) return st;
-    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k)) != COMEM_OK) return st;
+    if ((st = get_tensor_map(k_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_k, 2, 0, 8)) != COMEM_OK) return st;
     if ((st = get_tensor_map(v_pages, num_pages, page_size, num_kv_heads, head_dim, &tm_v)) != COMEM_OK) return st;
     // upper bound on sum_b ceil(n_b / 2R): the chunk lengths live on the device
     const int64_t pair_pos = 2 * (int64_t)p.rows_per_tile;

@@ -13,13 +13,15 @@
 //     (256 rows per 64 KiB of K+V: the L2 -> shared-memory traffic per flop that one tile would need is
 //     above what the L2 delivers);
 //   * warp 8 = producer: the pair's two Q tiles by one TMA load each (4-D box {64 d, G heads, R positions,
-//     D/64}), then per 128-token KV block eight 16-token K tiles and eight V tiles straight from the block
-//     table (the decode kernel's tensor map, 128-byte swizzle) into two-stage K and V rings;
-//   * warp 9 = MMA issuer (one lane): S_t = Q_t K^T as 2 x (D/16) instructions M128 N64 K16 whose B operand
-//     takes its 8-row groups 1 tile apart (stride-dimension offset = one 16-token tile), i.e. rows 0-7 of
-//     the block's eight tiles, then rows 8-15: a fixed permutation of the score columns, undone when P is
-//     written; O_t += P_t V as one instruction M128 N(D) K16 per 16-token tile with P read from tensor memory
-//     and V, token-major in shared memory exactly as the TMA laid it, as an MN-major operand;
+//     D/64}), then per 128-token KV block sixteen 8-token K half tiles and eight 16-token V tiles straight from the
+//     block table (128-byte swizzle; V through the decode kernel's tensor map) into two-stage K and V rings;
+//   * warp 9 = MMA issuer (one lane): S_t = Q_t K^T as D/16 instructions M128 N128 K16 -- K is loaded in HALF tiles of
+//     8 token rows (a second tensor map over the pool, box {64, 8, D/64, 1}), so the 16 eight-row groups of a block sit
+//     at one pitch (the descriptor's stride-dimension offset) and the whole block is one N dimension in token order.
+//     (A shared-memory x shared-memory MMA re-reads its 4 KiB A slice of Q per instruction: two N = 64 instructions per
+//     k-step, as the 16-row tiles forced, were bound by shared-memory bandwidth, 958 -> 1 060 TFLOP/s.)  O_t += P_t V as
+//     one instruction M128 N(D) K16 per 16-token tile with P read from tensor memory and V, token-major in shared memory
+//     exactly as the TMA laid it, as an MN-major operand;
 //   * warps 0-3 / 4-7 = softmax of tile 0 / 1, one thread per row (TMEM lane = row): tcgen05.ld the 128
 //     scores, causal mask by index, running max with a lazy rescale of O (only when the max grew by more
 //     than 2^8; the accumulator rescale is a TMEM read-modify-write by the row's own thread), exp2, P rounded
@@ -82,7 +84,7 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst_smem, const void *tmap,
 }
 
 // score column (S = Q K^T as issued: see the header) -> token of the 128-token block
-__host__ __device__ constexpr int col_token(int col) { return 16 * ((col & 63) >> 3) + 8 * (col >> 6) + (col & 7); }
+__host__ __device__ constexpr int col_token(int col) { return col; }  // (K is laid out in token order: see the producer)
 
 template <int D, bool kLse>
 // (compiled at 168 registers, the most twelve warps can be launched with; the softmax warps then grow to 232)
@@ -222,7 +224,13 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             if (lane == 0) mbar_arrive_expect_tx(k_full + 8 * sk, (uint32_t)nt * C::kTileBytes);
             for (int i = 0; i < nt; ++i) {
                 const int r = __shfl_sync(kAll, row, i);
-                if (lane == 0) tma_load_4d(k_smem + sk * C::kStageBytes + i * C::kTileBytes, &tm_k, k_full + 8 * sk, 0, r, 0, kvh);
+                // K in half tiles of 8 token rows (tm_k's box), 2 KiB each: [D/64 chunks][8 rows][128 B], so that the block's
+                // 8-row groups sit at one pitch and the MMA takes all 128 tokens as its N dimension, in token order
+                if (lane == 0) {
+                    tma_load_4d(k_smem + sk * C::kStageBytes + i * C::kTileBytes, &tm_k, k_full + 8 * sk, 0, r, 0, kvh);
+                    tma_load_4d(k_smem + sk * C::kStageBytes + i * C::kTileBytes + C::kTileBytes / 2, &tm_k, k_full + 8 * sk, 0,
+                                r + 8, 0, kvh);
+                }
             }
             pf_wait(v_empty + 8 * sv, ((uint32_t)(j / C::kVStages) & 1u) ^ 1u);
             if (lane == 0) mbar_arrive_expect_tx(v_full + 8 * sv, (uint32_t)nt * C::kTileBytes);
@@ -233,7 +241,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         }
     } else if (warp == 9) {
         // ------------------------------ MMA issuer -----------------------------------------------
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 64, false, false);
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(128, kBlockTokens, false, false);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, false, true);
         const int ntile_act = act1 ? 2 : 1;
         // S_t (block j) = Q_t K_j^T
@@ -243,10 +251,9 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             for (int ks = 0; ks < D / 16; ++ks) {
                 const uint32_t c = ks >> 2, kin = (ks & 3) * 32;
                 const uint64_t a = umma_smem_desc(qb + c * 16384 + kin, 0, 1024);
-                const uint64_t b0 = umma_smem_desc(kb + c * 2048 + kin, 0, C::kTileBytes);
-                const uint64_t b1 = umma_smem_desc(kb + c * 2048 + kin + 1024, 0, C::kTileBytes);
-                umma_ss(tmem + 128 * t, a, b0, idesc_qk, ks > 0);
-                umma_ss(tmem + 128 * t + 64, a, b1, idesc_qk, ks > 0);
+                // B: 16 groups of 8 token rows, C::kTileBytes / 2 apart; chunk c of a group at + c * 1 KiB
+                const uint64_t bk = umma_smem_desc(kb + c * 1024 + kin, 0, C::kTileBytes / 2);
+                umma_ss(tmem + 128 * t, a, bk, idesc_qk, ks > 0);
             }
         };
         // O_t += P_t V_j over the block's nt loaded tiles
@@ -394,9 +401,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         uint32_t pw[32];
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
-                            const int w = 32 * h + i;                      // P word: tile w / 8, token pair (w % 8)
-                            const int tile = w >> 3, q = w & 7;
-                            const int col = (q >> 2) * 64 + tile * 8 + 2 * (q & 3);   // score column of token 16 tile + 2 q
+                            const int col = 2 * (32 * h + i);              // P word w = 32 h + i: tokens 2w, 2w + 1 of the block
                             float e0 = ex2(fmaf(s[col], p.scale_log2, neg_m));
                             float e1 = ex2(fmaf(s[col + 1], p.scale_log2, neg_m));
                             if constexpr (kMasked) {  // (s = -inf and scale = 0 would give NaN above: decide by index)
