@@ -121,7 +121,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         one(q_full, 1);
         for (int s = 0; s < C::kKStages; ++s) { one(k_full + 8 * s, 1); one(k_empty + 8 * s, 1); }
         for (int s = 0; s < C::kVStages; ++s) { one(v_full + 8 * s, 1); one(v_empty + 8 * s, 1); }
-        for (int t = 0; t < 2; ++t) { one(s_full + 8 * t, 1); one(p_full + 8 * t, 128); }
+        for (int t = 0; t < 2; ++t) { one(s_full + 8 * t, 1); one(p_full + 8 * t, 4); }
         one(o_full, 1);
         fence_mbar_init();
     };
@@ -421,7 +421,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 else exp_pass(std::false_type{});
                 tmem_wait_st();
                 tc_fence_before_sync();
-                mbar_arrive(p_full + 8 * t);
+                __syncwarp();   // one arrival per warp (four per tile) instead of 128 serialised ones on one barrier
+                if (lane == 0) mbar_arrive(p_full + 8 * t);
             }
             // epilogue
             pf_wait(o_full, 0);
