@@ -267,7 +267,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         pf_wait(q_full, 0);
         pf_wait(k_full, 0);
         tc_fence_after_sync();
-        if (lane == 0) {
+        if (elect_one()) {
             for (int t = 0; t < ntile_act; ++t) {
                 issue_qk(t, 0);
                 umma_commit(s_full + 8 * t);
@@ -297,7 +297,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             for (int t = 0; t < ntile_act; ++t) {
                 pf_wait(p_full + 8 * t, (uint32_t)j & 1u);
                 tc_fence_after_sync();
-                if (lane == 0) {
+                if (elect_one()) {
                     issue_pv(t, j, nt);
                     if (t == ntile_act - 1) umma_commit(v_empty + 8 * sv);
                     if (more) {
@@ -309,7 +309,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 __syncwarp();
             }
         }
-        if (lane == 0) umma_commit(o_full);
+        if (elect_one()) umma_commit(o_full);
         __syncwarp();
     }
     tc_fence_before_sync();
