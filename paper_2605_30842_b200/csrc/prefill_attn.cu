@@ -206,7 +206,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     if (nblk <= 0) { __syncthreads(); continue; }  // n_b > L_b: invalid input (documented as undefined); no hang
     if (warp == 8) {
         // ------------------------------ producer -------------------------------------------------
-        if (lane == 0) {
+        if (elect_one()) {
             const uint32_t qbytes = (uint32_t)(64 * G * R * (D / 64) * 2);
             mbar_arrive_expect_tx(q_full, act1 ? 2 * qbytes : qbytes);
             tma_load_4d(q_smem, &tm_q, q_full, 0, kvh * G, qs + i0, 0);
@@ -221,22 +221,22 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             if (lane < nt) row = __ldg(bt + (tile >> p.page_tile_shift)) * p.page_size + ((tile & tpm) << 4);
             const int sk = j % C::kKStages, sv = j % C::kVStages;
             pf_wait(k_empty + 8 * sk, ((uint32_t)(j / C::kKStages) & 1u) ^ 1u);
-            if (lane == 0) mbar_arrive_expect_tx(k_full + 8 * sk, (uint32_t)nt * C::kTileBytes);
+            if (elect_one()) mbar_arrive_expect_tx(k_full + 8 * sk, (uint32_t)nt * C::kTileBytes);
             for (int i = 0; i < nt; ++i) {
                 const int r = __shfl_sync(kAll, row, i);
                 // K in half tiles of 8 token rows (tm_k's box), 2 KiB each: [D/64 chunks][8 rows][128 B], so that the block's
                 // 8-row groups sit at one pitch and the MMA takes all 128 tokens as its N dimension, in token order
-                if (lane == 0) {
+                if (elect_one()) {
                     tma_load_4d(k_smem + sk * C::kStageBytes + i * C::kTileBytes, &tm_k, k_full + 8 * sk, 0, r, 0, kvh);
                     tma_load_4d(k_smem + sk * C::kStageBytes + i * C::kTileBytes + C::kTileBytes / 2, &tm_k, k_full + 8 * sk, 0,
                                 r + 8, 0, kvh);
                 }
             }
             pf_wait(v_empty + 8 * sv, ((uint32_t)(j / C::kVStages) & 1u) ^ 1u);
-            if (lane == 0) mbar_arrive_expect_tx(v_full + 8 * sv, (uint32_t)nt * C::kTileBytes);
+            if (elect_one()) mbar_arrive_expect_tx(v_full + 8 * sv, (uint32_t)nt * C::kTileBytes);
             for (int i = 0; i < nt; ++i) {
                 const int r = __shfl_sync(kAll, row, i);
-                if (lane == 0) tma_load_4d(v_smem + sv * C::kStageBytes + i * C::kTileBytes, &tm_v, v_full + 8 * sv, 0, r, 0, kvh);
+                if (elect_one()) tma_load_4d(v_smem + sv * C::kStageBytes + i * C::kTileBytes, &tm_v, v_full + 8 * sv, 0, r, 0, kvh);
             }
         }
     } else if (warp == 9) {
