@@ -496,7 +496,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                             ks_i = __shfl_sync(kFull, ks, i);
                             vs_i = __shfl_sync(kFull, vs, i);
                         }
-                        if (lane == 0) {
+                        if (elect_one()) {  // (not `lane == 0`: see elect_one)
                             const int slot0 = (jj_i & tiles_per_page_mask) << kTileShift;
                             // block-table entry e >= 0: page e of the device pool; e < 0: page -1 - e of the host tier
                             const bool host_page = !kFp8 && pid_i < 0;

@@ -229,6 +229,15 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 #define COMEM_STAMP(i) do { } while (0)
 #endif
 
+// One lane of a converged warp, chosen by the hardware: unlike `lane == 0` the compiler knows the branch is taken by
+// exactly one lane, so the uniform-register operands of TMA and tcgen05 instructions need no per-lane loop around every instruction.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.b32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+
 // ---- named barriers (sub-CTA sync among the consumer warps) ----------------------------------
 __device__ __forceinline__ void named_bar_sync(int id, int threads)
 {

@@ -52,15 +52,6 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr)
 __device__ __forceinline__ void tc_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-// One lane of a converged warp, chosen by the hardware: unlike `lane == 0` the compiler knows the branch is taken by
-// exactly one lane, so the uniform-register operands of tcgen05.mma need no per-lane loop around every instruction.
-__device__ __forceinline__ bool elect_one()
-{
-    uint32_t pred;
-    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.b32 %0, 1, 0, p;\n\t}" : "=r"(pred));
-    return pred != 0;
-}
-
 // ---- MMA: D[tmem] (+)= A * B, issued by ONE thread --------------------------------------------
 // A and B from shared memory
 __device__ __forceinline__ void umma_ss(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate)
