@@ -29,6 +29,11 @@
 //     them in CTA-index order (merge.cuh), re-arming the counter for the next launch.  No CTA
 //     ever waits for another one.  With fuse_combine == 0 the kernel stops after S6 and the
 //     stand-alone K2 (combine.cu) does the merge.
+//   * EARLY MODE (launch flags COMEM_LAUNCH_KV_PREFIX_IMMUTABLE [| COMEM_LAUNCH_Q_STABLE]): the
+//     CTA does not sit in griddepcontrol.wait while the previous kernel drains -- its producers stream, and its
+//     consumers fold, every tile below the sequence's last one from the guessed schedule; the wait, the validation
+//     of the guess and a verdict on an mbarrier come at the first tile (or store) that needs the previous kernel's
+//     results; a wrong guess aborts the attempt and reruns it in the classic order.  Same bits either way.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
 #ifndef COMEM_BF16_PRODUCER_WARPS
