@@ -189,3 +189,38 @@ print("RESULT", ok)
         env = dict(os.environ, COMEM_DEBUG_STALE_GUESS=stale, PYTHONPATH=root)
         r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
         assert "RESULT True" in r.stdout, (stale, r.stdout[-500:], r.stderr[-1500:])
+
+
+def test_all_flags_on_the_fp8_cache_and_the_two_tier_cache(oracle):
+    """KV_PREFIX_IMMUTABLE | Q_STABLE | SPLIT_COMBINE on the other instances of the kernel: the FP8 cache (NHD and HND)
+    against its oracle and its own un-flagged SPLIT_COMBINE run, and the two-tier cache against the all-HBM bits."""
+    import numpy as np
+    ALL = IMM | QS | SC
+    f = W.quantize_batch_fp8(W.make_batch([9000, 17, 0, 640], 32, 8, 128, 16, seed=31, device=DEV, poison_unused=True))
+    for fb in (f, W.to_hnd(f)):
+        ws = comem.alloc_workspace(fb.q, fb.k_pages, fb.block_table, kv_layout=fb.kv_layout)
+        outs = {}
+        for flags in (SC, ALL):
+            o = torch.full_like(fb.q, float("nan"))
+            for _ in range(3):
+                comem.comem_decode_attn_fp8_async(fb.q, fb.k_pages, fb.v_pages, fb.k_scale, fb.v_scale, fb.block_table,
+                                                  fb.seq_lens, fb.softmax_scale, o, ws, kv_layout=fb.kv_layout, flags=flags)
+            torch.cuda.synchronize()
+            outs[flags] = o
+        assert torch.equal(bits(outs[SC]), bits(outs[ALL])), fb.kv_layout
+        c = fb.to("cpu")
+        ref, _ = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table, c.seq_lens,
+                                        c.softmax_scale, kv_layout=c.kv_layout)
+        d = np.abs(outs[ALL].double().cpu().numpy() - ref)
+        assert d.max() <= 2e-2 and d.mean() <= 2e-3 and np.linalg.norm(d) / np.linalg.norm(ref) <= 5e-3
+    b = W.make_batch([30000], 64, 8, 128, 16, seed=32, device=DEV, poison_unused=True)
+    ref_out, _ = gpu_run(b, flags=SC)
+    ob = W.offload_pages(b, 0.2, seed=3, coldest_first=False)
+    bb = ob.base
+    out = torch.full_like(bb.q, float("nan"))
+    ws = comem.alloc_workspace(bb.q, bb.k_pages, bb.block_table)
+    for _ in range(3):
+        comem.comem_decode_attn_offload_async(bb.q, bb.k_pages, bb.v_pages, ob.k_host, ob.v_host, bb.block_table, bb.seq_lens,
+                                              bb.softmax_scale, out, ws, flags=ALL)
+    torch.cuda.synchronize()
+    assert torch.equal(bits(out), bits(ref_out))
