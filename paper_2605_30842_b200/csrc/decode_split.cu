@@ -3,7 +3,8 @@
 // for one decode step of paged GQA attention.
 //
 // Shape of the kernel (sm_100a):
-//   * persistent grid, ONE CTA per SM (12 warps, ~214 KiB of shared memory), one contiguous range
+//   * persistent grid, ONE CTA per SM (12 warps launched at 144 registers -- the producer warpgroup then hands registers
+//     to the two consumer warpgroups, setmaxnreg 72 / 176 -- and ~214 KiB of shared memory), one contiguous range
 //     of 16-token tiles per CTA (schedule.cuh);
 //   * before griddepcontrol.wait (i.e. under the previous kernel's tail): mbarrier init, tensor-map
 //     prefetch, an L2 prefetch of the small control inputs (seq_lens, block table, q), the whole
@@ -56,6 +57,7 @@ namespace comem {
 namespace {
 
 constexpr int kConsumerWarps = 8;
+constexpr int kK1LaunchRegs = 144;  // see Cfg::kLaunchRegs
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 static_assert(kConsumerWarps == kMaxGroup, "S6 and merge.cuh map warp w to query head w of the group");
 constexpr int kPrefetchTiles = COMEM_PREFETCH_TILES;  // per CTA, L2-prefetched before the PDL wait (<= 32: one per lane)
@@ -73,6 +75,11 @@ struct Cfg {
     // one elected lane per producer warp; tiles are dealt round-robin to them (one lane is issue-rate bound)
     static constexpr int kProducerWarps = kFp8 ? 4 : COMEM_BF16_PRODUCER_WARPS;
     static constexpr int kThreads = kConsumerThreads + kProducerWarps * 32;
+    // Register budgets (COMEM_K1_SETMAXNREG): the kernel is LAUNCHED with kLaunchRegs per thread, so that the small
+    // combine kernel's CTAs fit beside it (384 x 144 leaves 10 240 of the SM's 65 536); the producer warpgroup then
+    // shrinks to kProducerRegs and hands the difference to the two consumer warpgroups:
+    // 8 x (kConsumerRegs - kLaunchRegs) <= 4 x (kLaunchRegs - kProducerRegs).
+    static constexpr int kLaunchRegs = kK1LaunchRegs, kProducerRegs = 72, kConsumerRegs = 176;
     static constexpr int kPrefetch = kFp8 ? (2 * kPrefetchTiles < 32 ? 2 * kPrefetchTiles : 32) : kPrefetchTiles;
     static_assert(kPrefetch <= 32, "one prefetched tile per lane");
     static constexpr int kTileBytes = kTileTokens * D * kElemBytes;  // one K (or V) tile
@@ -126,8 +133,15 @@ __device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch
     return s;
 }
 
+#ifndef COMEM_K1_SETMAXNREG
+#define COMEM_K1_SETMAXNREG 1  // measured: C2 over a cold 20-step run 22.6 -> 21.0 us, steady state 19.8 -> 19.5; C3 / C4 unchanged
+#endif
 template <int D, bool kFp8>
+#if COMEM_K1_SETMAXNREG
+__global__ void __maxnreg__(kK1LaunchRegs)
+#else
 __global__ void __launch_bounds__((Cfg<D, kFp8>::kThreads), 1)
+#endif
 decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                     const __grid_constant__ CUtensorMap tm_kh, const __grid_constant__ CUtensorMap tm_vh,
                     const DecodeParams p)
@@ -376,7 +390,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     pdl_launch_dependents();
     COMEM_STAMP(2);
 
-  for (;;) {  // one pass, or two when an early attempt is aborted
+    // One pass, or two when an early attempt is aborted.  The attempt loop is written once per role (producers,
+    // consumers) so that each role's register budget (setmaxnreg, below) dominates its own code.
     // S8: rows of empty sequences (reading R9): +0.0 and lse = -inf, dealt round-robin to the CTAs.
     auto write_empty_rows = [&]() {
         if (!p.fuse_combine) return;
@@ -388,12 +403,16 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 for (int h = threadIdx.x; h < p.num_q_heads; h += kThreads) p.lse_out[row0 + h] = -INFINITY;
         }
     };
-    if (!early) {
-        write_empty_rows();
-        if (c0 >= c1) return;  // nothing to stream (no tiles at all, or more CTAs than the schedule uses)
-    }
     // early mode: CTA-local index of the first tile that needs the wait (producers: xp, consumers: xc)
     int xp = 0, xc = 0;
+    bool early_pending = false, aborted = false;
+    // start of an attempt; false: this CTA has nothing to stream
+    auto attempt_begin = [&]() -> bool {
+    if (!early) {
+        write_empty_rows();
+        if (c0 >= c1) return false;  // nothing to stream (no tiles at all, or more CTAs than the schedule uses)
+    }
+    xp = xc = 0;
     if (early) {
         const SegPos sp = locate(c0, prefix, p.batch, p.num_kv_heads);
         const int64_t rem = c1 - c0;
@@ -404,9 +423,43 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         xc = p.q_stable ? x_wait : 0;
         xp = p.q_stable ? x_wait : (x_wait < C::kStages ? x_wait : C::kStages);
     }
-    bool early_pending = early, aborted = false;
+    early_pending = early;
+    aborted = false;
+    return true;
+    };
+    // end of an attempt; true: the early attempt was aborted, run again in the classic order
+    auto attempt_end = [&]() -> bool {
+    if (!early) return false;
+    // End of an early attempt: all threads meet; either it went through (the empty rows are still to write: global
+    // stores, so after the wait every thread has passed by now), or the guess was wrong and the CTA starts over in
+    // the classic order with fresh barriers and the real schedule.
+    __syncthreads();
+    if (*reinterpret_cast<volatile int *>(&s_abort) == 0) {
+        write_empty_rows();
+        return false;
+    }
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_inval(full0 + 8 * s);
+            mbar_inval(empty0 + 8 * s);
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 1);
+        }
+        mbar_inval(merge_bar);
+        mbar_init(merge_bar, 1);
+        fence_mbar_init();
+    }
+    compute_schedule();  // (its barrier also publishes the fresh mbarriers)
+    early = false;
+    return true;
+    };
 
     if (warp >= kConsumerWarps) {
+#if COMEM_K1_SETMAXNREG
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::kProducerRegs));
+#endif
+      do {
+        if (!attempt_begin()) return;
         // ------------------------------ S2: page-gather producers -----------------------------
         // Producer warp pw issues the CTA's tiles with (CTA-local index) % kProducerWarps == pw; tile
         // tl always lands in ring stage tl % kStages, in the ring's pass number tl / kStages.
@@ -535,7 +588,13 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             x += cnt;
             tl0 += cnt;
         }
+      } while (attempt_end());
     } else {
+#if COMEM_K1_SETMAXNREG
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::kConsumerRegs));
+#endif
+    do {
+    if (!attempt_begin()) return;
     // ------------------------------ consumers: S3..S6 -----------------------------------------
     const int quad = lane >> 2;  // score row = query head within the group
     const int qlane = lane & 3;
@@ -1027,30 +1086,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         for (int tt = t; tt < xp; tt += kConsumerWarps)
             mbar_wait(full0 + 8 * (tt & (C::kStages - 1)), (uint32_t)(tt / C::kStages) & 1u);
     }
+    } while (attempt_end());
     }  // consumers
-    if (!early) return;
-    // End of an early attempt: all threads meet; either it went through (the empty rows are still to write: global
-    // stores, so after the wait every thread has passed by now), or the guess was wrong and the CTA starts over in
-    // the classic order with fresh barriers and the real schedule.
-    __syncthreads();
-    if (*reinterpret_cast<volatile int *>(&s_abort) == 0) {
-        write_empty_rows();
-        return;
-    }
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < C::kStages; ++s) {
-            mbar_inval(full0 + 8 * s);
-            mbar_inval(empty0 + 8 * s);
-            mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, 1);
-        }
-        mbar_inval(merge_bar);
-        mbar_init(merge_bar, 1);
-        fence_mbar_init();
-    }
-    compute_schedule();  // (its barrier also publishes the fresh mbarriers)
-    early = false;
-  }  // attempts
 }
 
 template <int D, bool kFp8>
