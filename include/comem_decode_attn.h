@@ -89,9 +89,17 @@ enum {
  *                        segments (batch * num_kv_heads <= 64: one 32K sequence); no gain for large batches.  The combine
  *                        sums a segment's partials in a different (equally fixed) order than the fused kernel, so the
  *                        result is within rounding of the default's, and bit-identical to itself from run to run.
+ *     COMEM_LAUNCH_FP8_TENSOR           comem_decode_attn_fp8_async / comem_decode_step_host_fp8 only (COMEM_ERR_INVALID_ARG
+ *                        elsewhere): run the split kernel that feeds the E4M3 tiles straight to the tensor cores
+ *                        (tcgen05 kind::f8f6f4, q and P each split exactly into two E4M3 parts) instead of widening
+ *                        every byte to fp16 in the warps; the combine always runs as the second, dependent kernel.
+ *                        head_dim 128, no sliding window, batch <= 1024 (COMEM_ERR_UNSUPPORTED otherwise).  Same
+ *                        schedule and reduction structure, results within rounding of the default kernel's (P carries
+ *                        8 significant bits instead of 11) and bit-identical to themselves from run to run and under
+ *                        page permutation.  The other flags are accepted and ignored by this kernel.
  * Two host threads may enqueue concurrently with different options; nothing here is process state.
  */
-enum { COMEM_LAUNCH_KV_PREFIX_IMMUTABLE = 1, COMEM_LAUNCH_SPLIT_COMBINE = 2, COMEM_LAUNCH_Q_STABLE = 4 };
+enum { COMEM_LAUNCH_KV_PREFIX_IMMUTABLE = 1, COMEM_LAUNCH_SPLIT_COMBINE = 2, COMEM_LAUNCH_Q_STABLE = 4, COMEM_LAUNCH_FP8_TENSOR = 8 };
 typedef struct {
     int grid_ctas;
     int programmatic_launch;

@@ -135,6 +135,7 @@ def comem_grid_ctas(head_dim: int) -> int:
 COMEM_LAUNCH_KV_PREFIX_IMMUTABLE = 1
 COMEM_LAUNCH_SPLIT_COMBINE = 2
 COMEM_LAUNCH_Q_STABLE = 4
+COMEM_LAUNCH_FP8_TENSOR = 8
 
 
 class LaunchOpts(ctypes.Structure):

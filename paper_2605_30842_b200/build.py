@@ -16,7 +16,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcomem_decode.so")
-SOURCES = ["api.cu", "decode_split.cu", "combine.cu", "kv_append.cu", "kstep_pipeline.cu", "kstep_step.cu", "prefill_attn.cu", "read_ceiling.cu"]
+SOURCES = ["api.cu", "decode_split.cu", "combine.cu", "kv_append.cu", "kstep_pipeline.cu", "kstep_step.cu", "decode_fp8_tc.cu", "prefill_attn.cu", "read_ceiling.cu"]
 HEADERS = ["ptx.cuh", "schedule.cuh", "decode_params.cuh", "merge.cuh", "tcgen05.cuh", "prefill_params.cuh", os.path.join("..", "..", "include", "comem_decode_attn.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr"]

@@ -478,11 +478,15 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.part_cap = kMaxGridCtas;
     p.seg_counters = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.counters);
     const int flags = opts ? opts->flags : 0;
-    if (flags & ~(COMEM_LAUNCH_KV_PREFIX_IMMUTABLE | COMEM_LAUNCH_SPLIT_COMBINE | COMEM_LAUNCH_Q_STABLE)) return COMEM_ERR_INVALID_ARG;
+    if (flags & ~(COMEM_LAUNCH_KV_PREFIX_IMMUTABLE | COMEM_LAUNCH_SPLIT_COMBINE | COMEM_LAUNCH_Q_STABLE | COMEM_LAUNCH_FP8_TENSOR))
+        return COMEM_ERR_INVALID_ARG;
+    // COMEM_LAUNCH_FP8_TENSOR: the tcgen05 split kernel of decode_fp8_tc.cu (FP8 cache, D = 128, no window, batch <= 1024)
+    const bool fp8_tensor = (flags & COMEM_LAUNCH_FP8_TENSOR) != 0;
+    if (fp8_tensor && (!kv_fp8 || phases != (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE))) return COMEM_ERR_INVALID_ARG;
     // the small dependent combine serves steps of few segments only (elsewhere the fused merge costs nothing)
     const bool small_combine = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) && (flags & COMEM_LAUNCH_SPLIT_COMBINE) &&
                                batch * num_kv_heads <= kAlignedMaxSegs;
-    const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) && !small_combine;
+    const bool fused = phases == (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE) && !small_combine && !fp8_tensor;
     p.fuse_combine = fused ? 1 : 0;
     p.kv_immutable = (flags & COMEM_LAUNCH_KV_PREFIX_IMMUTABLE) ? 1 : 0;
     p.q_stable = (flags & COMEM_LAUNCH_Q_STABLE) ? 1 : 0;  // (only acts together with KV_PREFIX_IMMUTABLE)
@@ -502,6 +506,16 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     if ((st = grid_for(head_dim, &p.grid_ctas, opts)) != COMEM_OK) return st;
 
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (fp8_tensor) {
+        if (!fp8_tc_supported(p, head_dim)) return COMEM_ERR_UNSUPPORTED;
+        const bool small = batch * num_kv_heads <= kAlignedMaxSegs;
+        if (launch_decode_fp8_tc(tm_k, tm_v, p, stream) != cudaSuccess ||
+            (small ? launch_combine_small(p, head_dim, stream) : launch_combine(p, head_dim, stream)) != cudaSuccess) {
+            cudaGetLastError();
+            return COMEM_ERR_CUDA;
+        }
+        return COMEM_OK;
+    }
     if ((phases & COMEM_PHASE_SPLIT) &&
         launch_decode_split(tm_k, tm_v, p, head_dim, stream, kv_fp8, host_tier ? &tm_kh : nullptr,
                             host_tier ? &tm_vh : nullptr) != cudaSuccess) {

@@ -69,6 +69,10 @@ inline cudaError_t set_max_smem_once(Kernel kernel, int bytes, PerDeviceOnce &on
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                                 const DecodeParams &p, int head_dim, cudaStream_t stream, bool kv_fp8 = false,
                                 const CUtensorMap *tm_k_host = nullptr, const CUtensorMap *tm_v_host = nullptr);
+// FP8 cache with both contractions on tcgen05 (decode_fp8_tc.cu; COMEM_LAUNCH_FP8_TENSOR): the split kernel only, partial
+// records as launch_decode_split writes them with fuse_combine == 0
+bool fp8_tc_supported(const DecodeParams &p, int head_dim);
+cudaError_t launch_decode_fp8_tc(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p, cudaStream_t stream);
 cudaError_t launch_combine(const DecodeParams &p, int head_dim, cudaStream_t stream);
 // the small dependent combine (COMEM_LAUNCH_SPLIT_COMBINE; batch * Hkv <= kAlignedMaxSegs)
 cudaError_t launch_combine_small(const DecodeParams &p, int head_dim, cudaStream_t stream);

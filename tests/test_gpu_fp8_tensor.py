@@ -1,0 +1,178 @@
+"""GPU parity of the tcgen05 split kernel for the FP8 cache (COMEM_LAUNCH_FP8_TENSOR, csrc/decode_fp8_tc.cu) against
+oracle.decode_attn_fp8 on the same bytes, at the tolerances of the default FP8 kernel, plus the properties that fix
+bits (reruns, page placement, pool layout) and the error codes of what the kernel does not take."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2605_30842_b200 as comem
+from paper_2605_30842_b200 import workloads as W
+from test_gpu_fp8 import bits, fp8_batch, gate
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+TENSOR = comem.COMEM_LAUNCH_FP8_TENSOR
+
+
+def run_tc(f, grid=None, flags=TENSOR, window=0, sinks=0):
+    out = torch.full_like(f.q, float("nan"))
+    lse = torch.full((f.batch, f.num_q_heads), float("nan"), dtype=torch.float32, device=DEV)
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+    comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                      f.softmax_scale, out, ws, window, sinks, lse_out=lse, kv_layout=f.kv_layout,
+                                      grid_ctas=grid, flags=flags)
+    torch.cuda.synchronize()
+    return out, lse
+
+
+def check_tc(oracle, f, what, grid=None, flags=TENSOR):
+    out, lse = run_tc(f, grid, flags)
+    c = f.to("cpu")
+    ref, ref_lse = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table,
+                                          c.seq_lens, c.softmax_scale, 0, 0, kv_layout=c.kv_layout)
+    gate(out.double().cpu().numpy(), ref, lse.double().cpu().numpy(), ref_lse, what)
+    return out, lse
+
+
+@pytest.mark.parametrize("G,ps", [(1, 16), (4, 32), (8, 16), (3, 32), (5, 16), (8, 32)])
+def test_tensor_small_ragged(oracle, G, ps):
+    lens = [1, 15, 16, 17, 31, 33, 127, 128, 129, 512, 1000, 0, 2049]
+    f = fp8_batch(lens, 2 * G, 2, ps, seed=700 + G + ps)
+    check_tc(oracle, f, f"tensor G{G} ps{ps}")
+
+
+def test_tensor_long_ragged_grids_permutation_layout(oracle):
+    lens = [20000, 37, 0, 50001, 8191, 16, 300]
+    f = fp8_batch(lens, 64, 8, 16, seed=721)
+    base, base_lse = check_tc(oracle, f, "tensor ragged default grid")
+    again, again_lse = run_tc(f)
+    assert torch.equal(bits(base), bits(again)) and torch.equal(base_lse, again_lse)        # run to run
+    po, pl = run_tc(W.permute_pages_fp8(f, seed=9))
+    assert torch.equal(bits(base), bits(po)) and torch.equal(base_lse, pl)                  # page placement
+    ho, hl = check_tc(oracle, W.to_hnd(f), "tensor ragged HND")
+    assert torch.equal(bits(base), bits(ho)) and torch.equal(base_lse, hl)                  # pool layout
+    for grid in (1, 7, 61, 148, 296):
+        check_tc(oracle, f, f"tensor ragged grid {grid}", grid=grid)
+    # the other launch flags are accepted and change nothing
+    fo, fl = run_tc(f, flags=TENSOR | 7)
+    assert torch.equal(bits(base), bits(fo)) and torch.equal(base_lse, fl)
+
+
+def test_tensor_single_long_sequence(oracle):
+    f = fp8_batch([32768], 64, 8, 16, seed=722, k_scale=0.5)
+    check_tc(oracle, f, "tensor c2-shaped")
+    check_tc(oracle, W.to_hnd(f), "tensor c2-shaped HND")
+
+
+@pytest.mark.parametrize("nats,v_mean", [(12.0, 0.3), (14.0, 0.15)])
+def test_tensor_sink_token_small_v_scale(oracle, nats, v_mean):
+    """One sink token far above a flat 32K tail with page scales <= 2e-3: the tail's p * v_scale must keep its bits
+    through the E4M3 split (only the scale's mantissa and a relative power of two ride on p)."""
+    f = W.quantize_batch_fp8(W.sink_batch(32768, 32, 8, 128, 16, seed=730, device=DEV, sink_nats=nats, v_mean=v_mean,
+                                          v_std=v_mean / 3))
+    check_tc(oracle, f, f"tensor sink {nats} nats")
+
+
+def test_tensor_mixed_page_scales(oracle):
+    """v_scale exponents spread over 2^-12 .. 2^6 within a sequence: the running reference exponent moves, O is rescaled."""
+    b = W.make_batch([3000, 777], 32, 8, 128, 16, seed=731, device=DEV, poison_unused=True)
+    gen = torch.Generator(device=DEV)
+    gen.manual_seed(5)
+    expo = torch.randint(-12, 7, (b.v_pages.shape[0], 1, 8, 1), generator=gen, device=DEV).float()
+    b.v_pages.copy_((b.v_pages.float() * torch.exp2(expo)).to(torch.bfloat16))
+    check_tc(oracle, W.quantize_batch_fp8(b), "tensor mixed page scales")
+
+
+def test_tensor_rising_logits(oracle):
+    """Keys whose scores grow along the sequence: every super tile raises the running maximum (the slow path each time)."""
+    b = W.make_batch([4096, 1500], 16, 2, 128, 16, seed=732, device=DEV, poison_unused=True)
+    f = W.quantize_batch_fp8(b)
+    ramp = torch.linspace(0.2, 3.0, 4096, device=DEV)
+    for s in range(2):
+        n = int(f.seq_lens[s])
+        for t0 in range(0, n, 16):
+            pid = int(f.block_table[s, t0 // 16])
+            f.k_scale[pid] *= float(ramp[t0])
+    check_tc(oracle, f, "tensor rising logits")
+
+
+def test_tensor_all_byte_codes_exact(oracle):
+    """L = 1, unit scales: the weight is exactly 1 (hi = 128 * 2, lo = 0 after the split), so out = bf16(e4m3(V byte))
+    exactly for every finite byte code, and lse = scale * q . k checks the K side and the exact split of q."""
+    f = fp8_batch([1, 1], 8, 1, 16, seed=724)
+    codes = torch.arange(256, dtype=torch.uint8, device=DEV)
+    codes = torch.where((codes & 0x7f) == 0x7f, torch.zeros_like(codes), codes)
+    for b in range(2):
+        pid = int(f.block_table[b, 0])
+        f.v_pages[pid, 0, 0] = codes[128 * b:128 * (b + 1)]
+        f.k_pages[pid, 0, 0] = codes[128 * b:128 * (b + 1)].flip(0)
+        f.k_scale[pid, 0] = 1.0
+        f.v_scale[pid, 0] = 1.0
+    f = dataclasses.replace(f, q=(f.q.float() / 64).to(torch.bfloat16))
+    out, lse = run_tc(f)
+    want = codes.view(torch.float8_e4m3fn).float()
+    for b in range(2):
+        for h in range(8):
+            assert torch.equal(out[b, h].float(), want[128 * b:128 * (b + 1)]), (b, h)
+    c = f.to("cpu")
+    _, ref_lse = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table, c.seq_lens,
+                                        c.softmax_scale)
+    assert np.max(np.abs(lse.double().cpu().numpy() - ref_lse) / np.maximum(1.0, np.abs(ref_lse))) <= 1e-5
+
+
+@pytest.mark.parametrize("batch", [33, 64, 256, 1024])
+def test_tensor_large_batches(oracle, batch):
+    """The paper's batch sizes: many short segments per CTA, whole and cut, zeros mixed in."""
+    rng = np.random.default_rng(7400 + batch)
+    lens = [0 if rng.random() < 0.05 else int(rng.integers(1, 700)) for _ in range(batch)]
+    f = fp8_batch(lens, 16, 4, 16, seed=7400 + batch)
+    out, lse = check_tc(oracle, f, f"tensor batch {batch}")
+    po, pl = run_tc(W.permute_pages_fp8(f, seed=batch))
+    assert torch.equal(bits(out), bits(po))
+    assert torch.equal(lse.nan_to_num(neginf=-1e30), pl.nan_to_num(neginf=-1e30))
+
+
+@pytest.mark.parametrize("case", range(10))
+def test_tensor_randomised_shapes(oracle, case):
+    rng = np.random.default_rng(9700 + case)
+    G, hkv, ps = int(rng.integers(1, 9)), int(rng.integers(1, 9)), int(rng.choice([16, 32]))
+    batch = int(rng.integers(1, 11))
+    special = [0, 1, 15, 16, 17, ps - 1, ps, ps + 1, 127, 128, 129, 255, 256, 257]
+    lens = [int(rng.choice(special)) if rng.random() < 0.3 else int(rng.integers(1, 6000)) for _ in range(batch)]
+    if case % 4 == 0:
+        lens[0] = int(rng.integers(20000, 60000))
+    grid = int(rng.choice([0, 0, 3, 17, 61, 148, 211, 600]))
+    f = fp8_batch(lens, G * hkv, hkv, ps, seed=9800 + case)
+    if rng.random() < 0.5:
+        f = W.to_hnd(f)
+    what = f"tensor case {case}: G{G} hkv{hkv} ps{ps} {f.kv_layout} lens{lens} grid{grid}"
+    out, lse = check_tc(oracle, f, what, grid=grid or None)
+    out2, lse2 = run_tc(W.permute_pages_fp8(f, seed=case), grid=grid or None)
+    assert torch.equal(bits(out), bits(out2)), what
+    assert torch.equal(lse.nan_to_num(neginf=-1e30), lse2.nan_to_num(neginf=-1e30)), what
+
+
+def test_tensor_flag_rejections():
+    """The flag belongs to the FP8 entry points; head_dim 64, a sliding window and batch > 1024 are not taken."""
+    b = W.make_batch([100], 8, 2, 128, 16, seed=1, device=DEV)
+    out = torch.empty_like(b.q)
+    ws = comem.alloc_workspace(b.q, b.k_pages, b.block_table)
+    with pytest.raises(comem.ComemError) as e:
+        comem.comem_decode_attn_async(b.q, b.k_pages, b.v_pages, b.block_table, b.seq_lens, b.softmax_scale, out, ws,
+                                      flags=TENSOR)
+    assert e.value.status == comem.COMEM_ERR_INVALID_ARG
+    f = fp8_batch([300, 20], 8, 2, 16, seed=2)
+    with pytest.raises(comem.ComemError) as e:
+        run_tc(f, window=64, sinks=2)
+    assert e.value.status == comem.COMEM_ERR_UNSUPPORTED
+    f64 = W.quantize_batch_fp8(W.make_batch([300], 8, 2, 64, 16, seed=3, device=DEV))
+    with pytest.raises(comem.ComemError) as e:
+        run_tc(f64)
+    assert e.value.status == comem.COMEM_ERR_UNSUPPORTED
+    big = fp8_batch([5] * 1025, 4, 1, 16, seed=4)
+    with pytest.raises(comem.ComemError) as e:
+        run_tc(big)
+    assert e.value.status == comem.COMEM_ERR_UNSUPPORTED
+    torch.cuda.synchronize()
