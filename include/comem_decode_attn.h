@@ -383,6 +383,35 @@ int comem_prefill_attn_async(const void *q, const void *k_pages, const void *v_p
                              float softmax_scale, void *out, int batch, int total_q, int max_pages_per_seq,
                              int64_t num_pages, float *lse_out, void *cuda_stream, const comem_launch_opts *opts);
 
+/*
+ * comem_decode_attn_static_async — comem_decode_attn_async for callers that cannot allocate device memory (code under
+ * CUDA-graph capture, serving loops and harnesses that forbid cudaMalloc): the same decode-attention step (
+ * the same kernels, the same schedule, results bit-identical to comem_decode_attn_async with the same options), with
+ * its scratch (arrival counters + split partials) in a device array that is part of the library image instead of a
+ * caller-provided workspace.  It calls no cudaMalloc / cudaFree and no allocating library routine; the caller passes
+ * only inputs and outputs.  Arguments as comem_decode_attn_async, without `workspace`.
+ *
+ * Limits and sharing:
+ *   - the array is COMEM_STATIC_SCRATCH_BYTES (12 MiB) of device memory on EVERY GPU the process loads the library on,
+ *     held until the process exits; comem_static_scratch_bytes() returns the figure;
+ *   - a shape is accepted iff comem_decode_attn_workspace_bytes(batch, num_q_heads, num_kv_heads, head_dim, ..) <=
+ *     COMEM_STATIC_SCRATCH_BYTES (e.g. batch <= 64 at 64 q heads / 8 kv heads / head_dim 128; batch <= 256 at 16 / 4);
+ *     a larger shape returns COMEM_ERR_WORKSPACE and enqueues nothing;
+ *   - every call on a device shares the one array, which keeps the previous call's contents: each call first enqueues a
+ *     cudaMemsetAsync of the counter prefix (<= 64 KiB) on `cuda_stream`, then the kernel(s).  Calls that may OVERLAP on
+ *     the GPU (different streams, or graphs replayed concurrently) RACE on it: serialise them, or give the others a
+ *     workspace of their own through comem_decode_attn_async;
+ *   - the array's device address is looked up on the first call on each device (cudaGetSymbolAddress, with that device
+ *     current): make that first call outside stream capture.
+ */
+#define COMEM_STATIC_SCRATCH_BYTES (12 * 1024 * 1024)
+size_t comem_static_scratch_bytes(void);
+int comem_decode_attn_static_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
+                                   int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                                   void *cuda_stream, const comem_launch_opts *opts);
+
 /* Same on the legacy default stream, then cudaStreamSynchronize: also returns
  * execution errors (COMEM_ERR_CUDA). */
 int comem_decode_attn(const void *q, const void *k_pages, const void *v_pages,

@@ -49,6 +49,11 @@ def load_library():
     lib.comem_decode_attn_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
                                             i64, vp, vp, sz, vp, vp]
     lib.comem_decode_attn_async.restype = i32
+    lib.comem_decode_attn_static_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32, i32,
+                                                   i64, vp, vp, vp]
+    lib.comem_decode_attn_static_async.restype = i32
+    lib.comem_static_scratch_bytes.argtypes = []
+    lib.comem_static_scratch_bytes.restype = sz
     lib.comem_decode_attn_phases_async.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, f32, vp, i32,
                                                    i32, i64, vp, vp, sz, vp, i32, vp]
     lib.comem_decode_attn_phases_async.restype = i32
@@ -375,6 +380,26 @@ def comem_decode_attn_async(q, k_pages, v_pages, block_table, seq_lens, softmax_
         workspace.numel() * workspace.element_size(), _stream(stream), _opts(grid_ctas, programmatic_launch, flags))
     if st != COMEM_OK:
         raise ComemError(st, "comem_decode_attn_async")
+
+
+def comem_static_scratch_bytes() -> int:
+    return int(load_library().comem_static_scratch_bytes())
+
+
+def comem_decode_attn_static_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,
+                                   lse_out=None, stream=None, grid_ctas=None, programmatic_launch=None,
+                                   flags: int = 0) -> None:
+    """comem_decode_attn_async without a workspace: the scratch is a fixed device array inside the library (no
+    allocation; shapes up to comem_static_scratch_bytes(); calls that overlap on the GPU race on it)."""
+    _check_inputs(q, k_pages, v_pages, block_table, seq_lens)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    st = load_library().comem_decode_attn_static_async(
+        _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(seq_lens), q.shape[1],
+        k_pages.shape[2], q.shape[2], k_pages.shape[1], ctypes.c_float(softmax_scale), _ptr(out),
+        q.shape[0], block_table.shape[1], k_pages.shape[0], _ptr(lse_out), _stream(stream),
+        _opts(grid_ctas, programmatic_launch, flags))
+    if st != COMEM_OK:
+        raise ComemError(st, "comem_decode_attn_static_async")
 
 
 def comem_decode_attn_window_async(q, k_pages, v_pages, block_table, seq_lens, softmax_scale: float, out,

@@ -588,6 +588,61 @@ int comem_decode_attn_async(const void *q, const void *k_pages, const void *v_pa
                                           COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE, opts);
 }
 
+// ---- comem_decode_attn_static_async: the decode step for callers that cannot allocate -------------------------------
+// The scratch the step needs (arrival counters, split partials) lives in THIS file-scope device array instead of a
+// caller-allocated workspace: COMEM_STATIC_SCRATCH_BYTES (12 MiB) on every GPU that loads the library, until exit.
+// In host code `g_static_scratch` is only the symbol's host-side stand-in, never a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[COMEM_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_ptr(void **ptr)
+{
+    static std::atomic<void *> cache[64];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    const bool tracked = dev >= 0 && dev < 64;
+    void *q = tracked ? cache[dev].load(std::memory_order_acquire) : nullptr;
+    if (!q) {
+        if (cudaGetSymbolAddress(&q, g_static_scratch) != cudaSuccess || !q) {
+            cudaGetLastError();
+            return COMEM_ERR_CUDA;
+        }
+        if (tracked) cache[dev].store(q, std::memory_order_release);
+    }
+    *ptr = q;
+    return COMEM_OK;
+}
+
+size_t comem_static_scratch_bytes(void) { return COMEM_STATIC_SCRATCH_BYTES; }
+
+int comem_decode_attn_static_async(const void *q, const void *k_pages, const void *v_pages,
+                                   const int32_t *block_table, const int32_t *seq_lens, int num_q_heads,
+                                   int num_kv_heads, int head_dim, int page_size, float softmax_scale, void *out,
+                                   int batch, int max_pages_per_seq, int64_t num_pages, float *lse_out,
+                                   void *cuda_stream, const comem_launch_opts *opts)
+{
+    int st = check_shape(num_q_heads, num_kv_heads, head_dim, page_size, batch, max_pages_per_seq, num_pages);
+    if (st != COMEM_OK) return st;
+    const WorkspaceLayout wl = workspace_layout(batch, num_q_heads, num_kv_heads, head_dim);
+    if (wl.total > (size_t)COMEM_STATIC_SCRATCH_BYTES) return COMEM_ERR_WORKSPACE;  // shape beyond the static scratch
+    if ((st = check_device()) != COMEM_OK) return st;
+    void *scratch = nullptr;
+    if ((st = static_scratch_ptr(&scratch)) != COMEM_OK) return st;
+    // every call shares the array and finds the previous call's contents: the arrival counters must start at zero
+    // (a call that completed left them zero, one that was cut short did not)
+    if (cudaMemsetAsync(static_cast<char *>(scratch) + wl.flag, 0, wl.part_acc - wl.flag,
+                        static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess) {
+        cudaGetLastError();
+        return COMEM_ERR_CUDA;
+    }
+    return decode_attn_impl(q, k_pages, v_pages, block_table, seq_lens, num_q_heads, num_kv_heads, head_dim, page_size,
+                            softmax_scale, out, batch, max_pages_per_seq, num_pages, lse_out, scratch,
+                            COMEM_STATIC_SCRATCH_BYTES, cuda_stream, COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE, 0, 0, opts);
+}
+
 int comem_decode_attn_offload_async(const void *q, const void *k_pages, const void *v_pages, const void *k_pages_host,
                                     const void *v_pages_host, const int32_t *block_table, const int32_t *seq_lens,
                                     int num_q_heads, int num_kv_heads, int head_dim, int page_size, float softmax_scale,
