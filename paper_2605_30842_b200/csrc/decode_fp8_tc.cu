@@ -85,6 +85,12 @@ __device__ __forceinline__ void umma_f8_ss(uint32_t tmem_d, uint64_t desc_a, uin
         "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
         ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
 }
+// shared-memory descriptor of an MN-major operand WITHOUT swizzle: 16 bytes of the M / N index contiguous, 8 contraction
+// rows at a 16-byte pitch (a 128-byte core matrix), further groups of 8 rows lbo_bytes apart (probe-checked)
+__device__ __forceinline__ uint64_t umma_smem_desc_mn_plain(uint32_t smem_addr, uint32_t lbo_bytes)
+{
+    return (uint64_t)((smem_addr & 0x3ffffu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | (1ull << 46);
+}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 {
     asm volatile(
@@ -454,7 +460,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
         int qk_stage = 0, pv_stage = 0, prepared = -1;
         uint32_t qk_phase = 0;
         constexpr uint32_t idesc_qk = umma_idesc_e4m3(128, 16, false, false);
-        constexpr uint32_t idesc_pv = umma_idesc_e4m3(128, 16, true, false);
+        constexpr uint32_t idesc_pv = umma_idesc_e4m3(128, 16, true, true);
         // Qs of a portion: rows g (hi) and 8 + g (lo) of a [16][128 B] K-major tile, q[g] * 2^e = hi + lo / 16 with the
         // row's largest element scaled into [128, 256); qc[g] = scale_log2 * 2^-e.  Buffer seg % 4: the QK cursor is
         // less than four super tiles (hence at most three portions) ahead of the PV cursor.
@@ -531,7 +537,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
 #ifndef COMEM_TC_SKIP_PV
 #pragma unroll
                     for (int ks = 0; ks < 4; ++ks)
-                        umma_f8_ss(d, umma_smem_desc(va + 4096 * ks, 0, 1024), umma_smem_desc(pb + 32 * ks, 0, 1024), idesc_pv,
+                        umma_f8_ss(d, umma_smem_desc(va + 4096 * ks, 0, 1024), umma_smem_desc_mn_plain(pb + 512 * ks, 128), idesc_pv,
                                    (pv.ul >= 2 || ks > 0) ? 1u : 0u);
 #endif
                     umma_commit(empty0 + 8 * pv_stage);
@@ -548,10 +554,9 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
         const int t = 32 * wq + lane;  // token row of the super tile == TMEM lane; in S6: d
         const uint32_t lane_off = (uint32_t)(32 * wq) << 16;
         const uint32_t pbase = base + TcSmem::kP + g * 2048;
-        uint32_t poff[kMaxGroup];
-#pragma unroll
-        for (int g8 = 0; g8 < kMaxGroup; ++g8)
-            poff[g8] = pbase + g8 * 128 + ((((uint32_t)(t >> 4) ^ (uint32_t)g8) << 4) | (uint32_t)(t & 15));
+        // Ps is the MN-major B operand of O^T += V^T Ps^T, unswizzled: token t's 16 bytes {hi of heads 0..7, lo of heads
+        // 0..7} are contiguous, so a thread hands over its token with ONE 16-byte store
+        const uint32_t prow = pbase + 16 * t;
         Cursor cur;
         cur.start(c0, c1, prefix, p.batch, p.num_kv_heads);
         int stage = 0;
@@ -588,7 +593,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
                     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(sc.x), "=f"(sc.y) : "r"(scales0 + stage * (kSubTiles * 8) + (t >> 4) * 8));
 #ifdef COMEM_TC_SKIP_SOFTMAX
                     if (U >= 2) mbar_wait(pvdone0 + 8 * g, ((uint32_t)(U >> 1) & 1u) ^ 1u);
-                    if (r[0] == 0x12345u) sts8(poff[0], sc.x);
+                    if (r[0] == 0x12345u) sts8(prow, sc.x);
                     fence_proxy_async_smem();
                     tc_fence_before_sync();
                     __syncwarp();
@@ -677,18 +682,16 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
                         const int ee = evt - eref + 127 + kPShift;
                         pscale = (dead || evt == 0 || ee <= 0) ? 0.f : __uint_as_float((vb & 0x807fffffu) | ((uint32_t)ee << 23));
                     }
+                    uint32_t hi[kMaxGroup / 2], lo[kMaxGroup / 2];
 #pragma unroll
                     for (int i = 0; i < kMaxGroup / 2; ++i) {
                         const float p0 = ex2f(s[2 * i] - m[2 * i]), p1 = ex2f(s[2 * i + 1] - m[2 * i + 1]);
                         l[2 * i] += p0;
                         l[2 * i + 1] += p1;
-                        uint32_t hi, lo;
-                        split_e4m3x2(p0 * pscale, p1 * pscale, hi, lo);
-                        sts8(poff[2 * i], hi);
-                        sts8(poff[2 * i + 1], hi >> 8);
-                        sts8(poff[2 * i] + 1024, lo);
-                        sts8(poff[2 * i + 1] + 1024, lo >> 8);
+                        split_e4m3x2(p0 * pscale, p1 * pscale, hi[i], lo[i]);
                     }
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(prow), "r"(hi[0] | (hi[1] << 16)),
+                                 "r"(hi[2] | (hi[3] << 16)), "r"(lo[0] | (lo[1] << 16)), "r"(lo[2] | (lo[3] << 16)) : "memory");
                     fence_proxy_async_smem();
                     tc_fence_before_sync();
                     __syncwarp();
