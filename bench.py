@@ -55,7 +55,8 @@ def kernel_source_sha() -> str:
 
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2605_30842_b200", "csrc")
-    for f in ("decode_split.cu", "merge.cuh", "schedule.cuh", "ptx.cuh", "decode_params.cuh", "prefill_attn.cu", "tcgen05.cuh"):
+    for f in ("decode_split.cu", "merge.cuh", "schedule.cuh", "ptx.cuh", "decode_params.cuh", "prefill_attn.cu", "tcgen05.cuh",
+              "decode_fp8_tc.cu"):
         with open(os.path.join(d, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
@@ -923,10 +924,10 @@ def run_fp8(args) -> int:
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
                       "frac_of_measured_peak": gbs / peaks["hbm_gbs"], "peak": peaks["hbm_gbs"],
-                      "roofline": {"bound": "hbm", "kernel": "decode_split_kernel<128, 1>", "achieved": gbs,
+                      "roofline": {"bound": "hbm", "kernel": "decode_fp8_tc_kernel (tcgen05 kind::f8f6f4)" if flags & 8 else "decode_split_kernel<128, 1>", "achieved": gbs,
                                    "peak": peaks["hbm_gbs"], "unit": UNIT, "frac": gbs / peaks["hbm_gbs"],
                                    "us_per_launch": us,
-                                   "traffic": ncu_traffic("fp8_%s_%s" % (args.workload, pools[0].kv_layout.lower()))},
+                                   "traffic": ncu_traffic("fp8%s_%s_%s" % ("tc" if flags & 8 else "", args.workload, pools[0].kv_layout.lower()))},
                       "gpu_launches": replays * per_graph, "parity": parity, "oracle_seconds_one_sequence": oracle_s,
                       "bf16_cache_bytes_same_tokens": bf16_bytes,
                       "equivalent_bf16_gbs": bf16_bytes / us / 1e3, "clocks": sampler.summary(),
@@ -1251,6 +1252,77 @@ def measure_decode(ctx, name, steps, warmup, *, primary):
     return res
 
 
+def measure_fp8(ctx, peaks, steps, with_parity=True) -> dict:
+    """The FP8 (E4M3 + page scales) cache on C4's batch, HND pools: the warp-level kernel (F2FP + HMMA, launch flags of the
+    line) and the tcgen05 kernel (COMEM_LAUNCH_FP8_TENSOR), `steps` steps each from one replayed CUDA graph (a step reads
+    4 GiB: cold in L2), parity of each against the FP8 oracle on one whole sequence."""
+    torch, comem, args = ctx["torch"], ctx["comem"], ctx["args"]
+    device, stream = ctx["device"], ctx["stream"]
+    from paper_2605_30842_b200 import workloads as W
+
+    bf = make_pools("c4", device, 0, 0)[0]
+    f = W.to_hnd(W.quantize_batch_fp8(bf))
+    del bf
+    torch.cuda.empty_cache()
+    nbytes = f.algorithmic_bytes()
+    out = torch.empty_like(f.q)
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, stream=stream, kv_layout=f.kv_layout)
+    base_flags = DEFAULT_LAUNCH_FLAGS if args.launch_flags is None else args.launch_flags
+    res = {"workload": workload_desc("c4")["workload"] + ", cache quantised to E4M3 + per-page scales, HND pools",
+           "algorithmic_bytes_per_step": nbytes, "steps": steps, "unit": UNIT, "launch": "CUDA graph, replayed"}
+    for key, flags in (("warp_level", base_flags & 7), ("tcgen05", comem.COMEM_LAUNCH_FP8_TENSOR)):
+        sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), ctx["local_rank"])
+        sampler.start()
+        with torch.cuda.stream(stream):
+            def step():
+                comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table,
+                                                  f.seq_lens, f.softmax_scale, out, ws, stream=stream,
+                                                  kv_layout=f.kv_layout, flags=flags)
+            for _ in range(3):
+                step()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for _ in range(steps):
+                    step()
+            g.replay()
+            stream.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            sampler.active = True
+            e0.record(stream)
+            g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            sampler.active = False
+            clocks = sampler.summary()
+            us = e0.elapsed_time(e1) * 1e3 / steps
+            # ... and sustained: the same graph replayed for ~1.5 s (this kernel plus HBM at full rate reaches the board's
+            # power cap, the SM clock drops, and the two kernels part ways)
+            reps = max(2, int(1.5e6 / (us * steps)))
+            sampler.reset()
+            sampler.active = True
+            e0.record(stream)
+            for _ in range(reps):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            sampler.active = False
+        sampler.stop()
+        us_long = e0.elapsed_time(e1) * 1e3 / (steps * reps)
+        gbs = nbytes / us / 1e3
+        rec = {"kernel": "decode_fp8_tc_kernel" if flags & 8 else "decode_split_kernel<128, 1>", "launch_flags": flags,
+               "us_per_step": us, "achieved": gbs, "frac": gbs / peaks["hbm_gbs"], "frac_of_8TBps": gbs / 8000.0,
+               "gpu_launches": steps * (2 if flags & 8 else 1), "clocks": clocks,
+               "traffic": ncu_traffic("fp8tc_c4_hnd" if flags & 8 else "fp8_c4_hnd"),
+               "sustained": {"steps": steps * reps, "us_per_step": us_long, "achieved": nbytes / us_long / 1e3,
+                             "frac": nbytes / us_long / 1e3 / peaks["hbm_gbs"], "clocks": sampler.summary()}}
+        if with_parity:
+            rec["parity"], _ = fp8_parity(f, out, seq=3)
+        res[key] = rec
+        del g
+    return res
+
+
 def measure_prefill(ctx, peaks, with_parity=True) -> dict:
     """the paged causal prefill kernel (tcgen05) on the agent geometry -- an uncached full prefill
     of one 32 768-token context (Alg. 1 line 12) and a cached 512-token chunk over the same prefix (line 10).
@@ -1435,6 +1507,10 @@ def main() -> int:
         extra["c5"] = c5
         torch.cuda.empty_cache()
         extra["prefill"] = measure_prefill(ctx, peaks, with_parity=not args.no_cpu_baseline)
+        torch.cuda.empty_cache()
+        extra["c4_fp8"] = measure_fp8(ctx, peaks, max(3, min(args.steps, 100)), with_parity=not args.no_cpu_baseline)
+        for k_ in ("warp_level", "tcgen05"):
+            extra["c4_fp8"][k_]["frac_of_read_ceiling"] = extra["c4_fp8"][k_]["achieved"] / ceiling["read_ceiling_gbs"]
         torch.cuda.empty_cache()
 
     if rank == 0:
