@@ -1267,10 +1267,11 @@ def measure_fp8(ctx, peaks, steps, with_parity=True) -> dict:
     nbytes = f.algorithmic_bytes()
     out = torch.empty_like(f.q)
     ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, stream=stream, kv_layout=f.kv_layout)
-    base_flags = DEFAULT_LAUNCH_FLAGS if args.launch_flags is None else args.launch_flags
     res = {"workload": workload_desc("c4")["workload"] + ", cache quantised to E4M3 + per-page scales, HND pools",
            "algorithmic_bytes_per_step": nbytes, "steps": steps, "unit": UNIT, "launch": "CUDA graph, replayed"}
-    for key, flags in (("warp_level", base_flags & 7), ("tcgen05", comem.COMEM_LAUNCH_FP8_TENSOR)):
+    # (the warp-level kernel in the classic order: a 0.65 ms step has nothing for the early mode to hide, and the FP8
+    # consumers, bound by their issue slots, pay 5 % for its tests in the tile loop)
+    for key, flags in (("warp_level", 0), ("tcgen05", comem.COMEM_LAUNCH_FP8_TENSOR)):
         sampler = ClockSampler(str(getattr(torch.cuda.get_device_properties(device), 'uuid', '')), ctx["local_rank"])
         sampler.start()
         with torch.cuda.stream(stream):

@@ -35,6 +35,7 @@
 //     consumers fold, every tile below the sequence's last one from the guessed schedule; the wait, the validation
 //     of the guess and a verdict on an mbarrier come at the first tile (or store) that needs the previous kernel's
 //     results; a wrong guess aborts the attempt and reruns it in the classic order.  Same bits either way.
+//     The mode lives in its own instance of the kernel (template parameter kEarly), launched only when the flag is set.
 // The path is HBM-bound (G flop per byte); the legacy-shape tensor op is used only because at
 // G = 8 the plain-FMA roofline sits below the HBM roofline ("Why mma.sync").
 #ifndef COMEM_BF16_PRODUCER_WARPS
@@ -136,7 +137,10 @@ __device__ __forceinline__ SegPos locate(int64_t x, const int *prefix, int batch
 #ifndef COMEM_K1_SETMAXNREG
 #define COMEM_K1_SETMAXNREG 1  // measured: C2 over a cold 20-step run 22.6 -> 21.0 us, steady state 19.8 -> 19.5; C3 / C4 unchanged
 #endif
-template <int D, bool kFp8>
+// kEarly: the instance that holds the early mode (launched when COMEM_LAUNCH_KV_PREFIX_IMMUTABLE is set).  The classic
+// instance carries none of its tests in the tile loop: the FP8 consumers are bound by their issue slots, and the mode
+// costs them 5 % on long steps (C4 with the FP8 cache, same box: 747 us with the tests compiled in, 701 without).
+template <int D, bool kFp8, bool kEarly>
 #if COMEM_K1_SETMAXNREG
 __global__ void __maxnreg__(kK1LaunchRegs)
 #else
@@ -338,7 +342,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     // boundary: once in 16 decode steps per sequence) aborts the attempt: what was streamed is dropped, the barriers
     // are re-initialised and the CTA runs again in the classic order below.  Bits are the same in both modes: the
     // schedule, the tile -> warp map and every reduction order are unchanged.
-    bool early = p.kv_immutable != 0 && p.window <= 0 && c0 < c1;
+    bool early = kEarly && p.kv_immutable != 0 && p.window <= 0 && c0 < c1;
     __shared__ int s_abort;
     if (!early) {
         // Classic order.  Still before the wait: ask the TMA unit to pull this CTA's first tiles into L2.  Cached KV
@@ -499,7 +503,7 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             if (p.trace && threadIdx.x == kConsumerThreads) p.trace[blockIdx.x * 16 + 14] = globaltimer_ns();
 #endif
         };
-        while (x < c1 && !aborted) {
+        while (x < c1 && !(kEarly && aborted)) {
             const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
             const int64_t rem = c1 - x;
             const int cnt = (int)(rem < (int64_t)(sp.T - sp.j) ? rem : (int64_t)(sp.T - sp.j));
@@ -578,11 +582,11 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
                 }
             };
             int lo = 0;
-            if (early_pending) {  // (first segment only: xp lies inside it)
+            if (kEarly && early_pending) {  // (first segment only: xp lies inside it)
                 lo = xp - tl0 < cnt ? xp - tl0 : cnt;
                 issue_range(0, lo);
                 verdict();
-                if (aborted) break;
+                if (kEarly && aborted) break;
             }
             issue_range(lo, cnt);
             x += cnt;
@@ -657,9 +661,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     uint32_t phase = 0;
 
     while (x < c1) {
-        if (early_pending && xc <= n) {  // nothing of this segment may be touched before the wait (q included)
+        if (kEarly && early_pending && xc <= n) {  // nothing of this segment may be touched before the wait (q included)
             need_verdict();
-            if (aborted) break;
+            if (kEarly && aborted) break;
         }
         const SegPos sp = locate(x, prefix, p.batch, p.num_kv_heads);
         const int64_t rem = c1 - x;
@@ -731,9 +735,9 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         // with half the bytes per tile, a single chain per warp is latency-bound below the HBM rate.
         auto tiles_pass = [&](auto nt_tag) {
             constexpr int NT = decltype(nt_tag)::value;
-            if (early_pending && t + (NT - 1) * kConsumerWarps >= xc) {
+            if (kEarly && early_pending && t + (NT - 1) * kConsumerWarps >= xc) {
                 need_verdict();
-                if (aborted) return;
+                if (kEarly && aborted) return;
                 seq_len = __ldcg(p.seq_lens + sp.b);
                 wt = win_tiles(seq_len, p.window, p.sinks);
             }
@@ -969,11 +973,11 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
             t += NT * kConsumerWarps;
         };
         if constexpr (C::kTilesPerPass == 2) {
-            while (t + kConsumerWarps < n + cnt && !aborted) tiles_pass(std::integral_constant<int, 2>{});
+            while (t + kConsumerWarps < n + cnt && !(kEarly && aborted)) tiles_pass(std::integral_constant<int, 2>{});
         }
-        while (t < n + cnt && !aborted) tiles_pass(std::integral_constant<int, 1>{});
-        if (early_pending) need_verdict();  // S6 stores to global memory
-        if (aborted) break;
+        while (t < n + cnt && !(kEarly && aborted)) tiles_pass(std::integral_constant<int, 1>{});
+        if (kEarly && early_pending) need_verdict();  // S6 stores to global memory
+        if (kEarly && aborted) break;
 
         // S6: merge the consumer warps' states (warp-index order) and write the row or a partial.
         // Scratch layout per warp: acc as [head][D + 4] (the +4 pad makes both the fragment
@@ -1079,8 +1083,8 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
         x += cnt;
         n += cnt;
     }
-    if (pending_first && !aborted) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
-    if (aborted) {
+    if (pending_first && !(kEarly && aborted)) publish_and_merge(true, false, 0);  // the CTA's last segment was a whole one
+    if (kEarly && aborted) {
         // every tile the producers issued before the verdict must have landed before the barriers are re-initialised:
         // this warp's share of them that it has not consumed
         for (int tt = t; tt < xp; tt += kConsumerWarps)
@@ -1090,11 +1094,11 @@ decode_split_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_const
     }  // consumers
 }
 
-template <int D, bool kFp8>
+template <int D, bool kFp8, bool kEarly>
 cudaError_t configure_once()
 {
     static PerDeviceOnce once;
-    return set_max_smem_once(decode_split_kernel<D, kFp8>, (int)smem_bytes_for<D, kFp8>(kMaxBatch), once);
+    return set_max_smem_once(decode_split_kernel<D, kFp8, kEarly>, (int)smem_bytes_for<D, kFp8>(kMaxBatch), once);
 }
 
 }  // namespace
@@ -1117,15 +1121,23 @@ cudaError_t split_default_grid(int head_dim, int *grid_ctas)
     return cudaSuccess;
 }
 
+template <int D, bool kFp8, bool kEarly>
+static cudaError_t launch_instance(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const CUtensorMap &tm_kh,
+                                   const CUtensorMap &tm_vh, const DecodeParams &p, cudaLaunchConfig_t &cfg)
+{
+    const cudaError_t e = configure_once<D, kFp8, kEarly>();
+    if (e != cudaSuccess) return e;
+    cfg.blockDim = dim3(Cfg<D, kFp8>::kThreads);
+    cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch, p.fuse_combine != 0);
+    return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8, kEarly>, tm_k, tm_v, tm_kh, tm_vh, p);
+}
 template <int D, bool kFp8>
 static cudaError_t launch_variant(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const CUtensorMap &tm_kh,
                                   const CUtensorMap &tm_vh, const DecodeParams &p, cudaLaunchConfig_t &cfg)
 {
-    const cudaError_t e = configure_once<D, kFp8>();
-    if (e != cudaSuccess) return e;
-    cfg.blockDim = dim3(Cfg<D, kFp8>::kThreads);
-    cfg.dynamicSmemBytes = smem_bytes_for<D, kFp8>(p.batch, p.fuse_combine != 0);
-    return cudaLaunchKernelEx(&cfg, decode_split_kernel<D, kFp8>, tm_k, tm_v, tm_kh, tm_vh, p);
+    // the early-mode instance only where the mode can act (the flag is set and no sliding window)
+    if (p.kv_immutable != 0 && p.window <= 0) return launch_instance<D, kFp8, true>(tm_k, tm_v, tm_kh, tm_vh, p, cfg);
+    return launch_instance<D, kFp8, false>(tm_k, tm_v, tm_kh, tm_vh, p, cfg);
 }
 
 cudaError_t launch_decode_split(const CUtensorMap &tm_k, const CUtensorMap &tm_v, const DecodeParams &p,
