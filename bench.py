@@ -926,7 +926,7 @@ def run_fp8(args) -> int:
                       "pools": len(pools), "steps": replays * per_graph, "us_per_step": us,
                       "algorithmic_bytes_per_step": nbytes, "value": gbs, "unit": UNIT,
                       "frac_of_measured_peak": gbs / peaks["hbm_gbs"], "peak": peaks["hbm_gbs"],
-                      "roofline": {"bound": "hbm", "kernel": "decode_fp8_tc_kernel (tcgen05 kind::f8f6f4)" if flags & 8 else "decode_split_kernel<128, 1>", "achieved": gbs,
+                      "roofline": {"bound": "hbm", "kernel": "decode_fp8_tc_kernel (tcgen05 kind::f8f6f4)" if flags & 8 else "decode_split_kernel<128, 1, %d>" % (flags & 1), "achieved": gbs,
                                    "peak": peaks["hbm_gbs"], "unit": UNIT, "frac": gbs / peaks["hbm_gbs"],
                                    "us_per_launch": us,
                                    "traffic": ncu_traffic("fp8%s_%s_%s" % ("tc" if flags & 8 else "", args.workload, pools[0].kv_layout.lower()))},
@@ -1313,7 +1313,7 @@ def measure_fp8(ctx, peaks, steps, with_parity=True) -> dict:
         sampler.stop()
         us_long = e0.elapsed_time(e1) * 1e3 / (steps * reps)
         gbs = nbytes / us / 1e3
-        rec = {"kernel": "decode_fp8_tc_kernel" if flags & 8 else "decode_split_kernel<128, 1>", "launch_flags": flags,
+        rec = {"kernel": "decode_fp8_tc_kernel" if flags & 8 else "decode_split_kernel<128, 1, %d>" % (flags & 1), "launch_flags": flags,
                "us_per_step": us, "achieved": gbs, "frac": gbs / peaks["hbm_gbs"], "frac_of_8TBps": gbs / 8000.0,
                "gpu_launches": steps * (2 if flags & 8 else 1), "clocks": clocks,
                "traffic": ncu_traffic("fp8tc_c4_hnd" if flags & 8 else "fp8_c4_hnd"),
@@ -1531,7 +1531,7 @@ def main() -> int:
                     "algorithmic_bytes_per_step": prim["bytes_k_steps"] // steps,
                     "grid_ctas": comem.comem_grid_ctas(cfg["head_dim"]),
                     "replicas": world})
-        roof = {"bound": "hbm", "kernel": "decode_split_kernel<128, 0>", "achieved": achieved,
+        roof = {"bound": "hbm", "kernel": "decode_split_kernel<128, 0, %d>" % (1 if prim["launch_flags"] & 1 else 0), "achieved": achieved,
                 "peak": peak, "peak_source": peak_src, "unit": UNIT, "frac": achieved / peak,
                 "us_per_launch": ms_max / steps * 1e3,
                 "split_only_us": prim["ms_split_max"] / steps * 1e3,

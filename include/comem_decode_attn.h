@@ -89,8 +89,7 @@ enum {
  *                        segments (batch * num_kv_heads <= 64: one 32K sequence); no gain for large batches.  The combine
  *                        sums a segment's partials in a different (equally fixed) order than the fused kernel, so the
  *                        result is within rounding of the default's, and bit-identical to itself from run to run.
- *     COMEM_LAUNCH_FP8_TENSOR           comem_decode_attn_fp8_async / comem_decode_step_host_fp8 only (COMEM_ERR_INVALID_ARG
- *                        elsewhere): run the split kernel that feeds the E4M3 tiles straight to the tensor cores
+ *     COMEM_LAUNCH_FP8_TENSOR           comem_decode_attn_fp8_async only (COMEM_ERR_INVALID_ARG elsewhere): run the split kernel that feeds the E4M3 tiles straight to the tensor cores
  *                        (tcgen05 kind::f8f6f4, q and P each split exactly into two E4M3 parts) instead of widening
  *                        every byte to fp16 in the warps; the combine always runs as the second, dependent kernel.
  *                        head_dim 128, no sliding window, batch <= 1024 (COMEM_ERR_UNSUPPORTED otherwise).  Same
