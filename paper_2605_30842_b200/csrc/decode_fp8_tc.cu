@@ -270,6 +270,9 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
     // S1: the schedule of schedule.cuh, decided exactly as decode_split.cu decides it (the combine kernel recomputes it)
     int64_t total = 0, c0 = 0, c1 = 0;
     const int cta = blockIdx.x;
+    // (COMEM_DEBUG_STALE_GUESS=1, a testing aid as in decode_split.cu: the first schedule is computed from lengths 16 tokens short)
+    int guess_bias = p.debug_stale_guess ? kTileTokens : 0;
+    auto guess_len = [&](int L) { return L > guess_bias ? L - guess_bias : L; };
     auto compute_schedule = [&]() {
         if (warp == 0) {
             const int per = (p.batch + 31) >> 5;
@@ -277,7 +280,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
             int sum = 0;
 #pragma unroll 1
             for (int i = 0; i < per; ++i)
-                if (b0 + i < p.batch) sum += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                if (b0 + i < p.batch) sum += tiles_of(guess_len(__ldcg(p.seq_lens + b0 + i)));
             int incl = sum;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -289,7 +292,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
             for (int i = 0; i < per; ++i)
                 if (b0 + i < p.batch) {
                     prefix[b0 + i] = run;
-                    run += tiles_of(__ldcg(p.seq_lens + b0 + i));
+                    run += tiles_of(guess_len(__ldcg(p.seq_lens + b0 + i)));
                 }
             if (lane == 31) prefix[p.batch] = incl;
             __syncwarp();
@@ -338,6 +341,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
         }
     };
     compute_schedule();  // speculative
+    guess_bias = 0;
     const int tiles_per_page_mask = (1 << p.page_tile_shift) - 1;
     // tensor coordinates of tile jj of (sequence, kv head) in page pid: {d, token row, -, kv head}, or {d, slot, kv head, page} (HND)
     auto tile_coords = [&](int pid, int jj, int kvh, int &t1, int &t2, int &t3) {

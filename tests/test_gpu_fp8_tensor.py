@@ -176,3 +176,74 @@ def test_tensor_flag_rejections():
         run_tc(big)
     assert e.value.status == comem.COMEM_ERR_UNSUPPORTED
     torch.cuda.synchronize()
+
+
+def test_tensor_append_then_attend_loop(oracle):
+    """40 decode steps enqueued without host synchronisation: quantising append, then the tensor kernel, which computes
+    its schedule speculatively while the append kernel may still be bumping seq_lens (a length crosses a tile boundary
+    once in 16 steps: the validation after the wait must catch it).  Outputs against the oracle on the final cache at
+    the steps kept, and against the default kernel within the attention tolerances at every step."""
+    ps = 16
+    lens = [ps - 3, 5000, 0, 2 * ps - 1, 777, 12000]
+    b = W.make_batch(lens, 16, 4, 128, ps, seed=761, device=DEV, spare_tokens=48)
+    f = W.quantize_batch_fp8(b)
+    f.k_scale.copy_(torch.where(torch.isnan(f.k_scale) | (f.k_scale == 1.0), torch.full_like(f.k_scale, 0.011), f.k_scale))
+    f.v_scale.copy_(torch.where(torch.isnan(f.v_scale) | (f.v_scale == 1.0), torch.full_like(f.v_scale, 0.009), f.v_scale))
+    f = dataclasses.replace(f, seq_lens=f.seq_lens.clone())
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+    ws2 = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+    outs_t, outs_d, qs = [], [], []
+    for step in range(40):
+        q, nk, nv = W.decode_step_rows(b, step, seed_base=7700)
+        comem.comem_kv_append_fp8_async(f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens, nk, nv,
+                                        kv_layout=f.kv_layout)
+        ot, od = torch.full_like(q, float("nan")), torch.full_like(q, float("nan"))
+        comem.comem_decode_attn_fp8_async(q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                          f.softmax_scale, ot, ws, kv_layout=f.kv_layout, flags=TENSOR)
+        comem.comem_decode_attn_fp8_async(q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                          f.softmax_scale, od, ws2, kv_layout=f.kv_layout)
+        outs_t.append(ot), outs_d.append(od), qs.append(q)
+    torch.cuda.synchronize()
+    assert f.seq_lens.tolist() == [l + 40 for l in lens]
+    for step in range(40):
+        a, d = outs_t[step].double().cpu().numpy(), outs_d[step].double().cpu().numpy()
+        assert np.isfinite(a).all(), step
+        assert np.abs(a - d).max() <= 2 * 2e-2 and np.linalg.norm(a - d) <= 2 * 5e-3 * np.linalg.norm(d), step
+    # the last step against the oracle on the final cache
+    c = dataclasses.replace(f, q=qs[-1]).to("cpu")
+    ref, _ = oracle.decode_attn_fp8(c.q, c.k_pages, c.v_pages, c.k_scale, c.v_scale, c.block_table, c.seq_lens,
+                                    c.softmax_scale, 0, 0, kv_layout=c.kv_layout)
+    gate(outs_t[-1].double().cpu().numpy(), ref, np.full(ref.shape[:2], 0.0), np.full(ref.shape[:2], 0.0), "tensor loop, last step")
+
+
+def test_tensor_recovery_path_forced_by_a_stale_schedule_guess():
+    """COMEM_DEBUG_STALE_GUESS=1 (fresh process): the tensor kernel's first schedule comes from lengths 16 tokens short,
+    so its validation after the wait fails on every launch and the schedule is recomputed; same bits as without."""
+    import os
+    import subprocess
+    import sys
+    code = r'''
+import torch, hashlib
+import paper_2605_30842_b200 as comem
+from paper_2605_30842_b200 import workloads as W
+h = hashlib.sha256()
+for lens, hq, hkv, ps in [([32768], 64, 8, 16), ([20000, 37, 0, 50001, 8191, 16, 300], 64, 8, 16), ([700, 64, 4097], 12, 3, 32), ([17], 8, 1, 16)]:
+    f = W.quantize_batch_fp8(W.make_batch(lens, hq, hkv, 128, ps, seed=902, device="cuda", poison_unused=True))
+    ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+    o = torch.full_like(f.q, float("nan"))
+    for _ in range(3):
+        comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                          f.softmax_scale, o, ws, kv_layout=f.kv_layout, flags=comem.COMEM_LAUNCH_FP8_TENSOR)
+    torch.cuda.synchronize()
+    assert torch.isfinite(o.float()).all().item()
+    h.update(o.contiguous().view(torch.int16).cpu().numpy().tobytes())
+print("RESULT", h.hexdigest())
+'''
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    digests = []
+    for stale in ("0", "1"):
+        env = dict(os.environ, COMEM_DEBUG_STALE_GUESS=stale, PYTHONPATH=root)
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        assert "RESULT" in r.stdout, (stale, r.stdout[-500:], r.stderr[-1500:])
+        digests.append(r.stdout.split("RESULT")[1].strip())
+    assert digests[0] == digests[1]
