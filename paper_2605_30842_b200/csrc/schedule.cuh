@@ -100,13 +100,15 @@ constexpr int kAlignedMaxLossTiles = 6;
 COMEM_HD int aligned_boundary(int64_t tiles_to_end, int64_t total_tiles, int grid_ctas)
 {
     // same value either way; the 32-bit form keeps 64-bit divisions off the launch's critical path
-    if (total_tiles <= (int64_t)(0x7fffffff / 2) / grid_ctas)
+    if (total_tiles <= (int64_t)((0x7fffffff / 2) / grid_ctas))  // (a 32-bit division: grid_ctas is an int)
         return (int)(((uint32_t)tiles_to_end * (uint32_t)grid_ctas + (uint32_t)total_tiles / 2u) / (uint32_t)total_tiles);
     return (int)((tiles_to_end * grid_ctas + total_tiles / 2) / total_tiles);
 }
 // tiles on the busiest CTA if the work were cut evenly
 COMEM_HD int ideal_tiles_per_cta(int64_t total_tiles, int grid_ctas)
 {
+    if (total_tiles <= 0x7fffffff - kMaxGridCtasBound)  // same value; keeps a 64-bit division off the launch's critical path
+        return (int)(((uint32_t)total_tiles + (uint32_t)grid_ctas - 1u) / (uint32_t)grid_ctas);
     return (int)((total_tiles + grid_ctas - 1) / grid_ctas);
 }
 // is a segment of T tiles that was dealt c CTAs acceptable?
