@@ -508,10 +508,14 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
                 prepare_q(qk.sp, qk.seg);
                 prepared = qk.seg;
             }
-            const bool go_qk = can_qk && __shfl_sync(kFullMask32, (int)mbar_test(full0 + 8 * qk_stage, qk_phase), 0) != 0;
-            const bool go_pv = can_pv && __shfl_sync(kFullMask32, (int)mbar_test(pv_bar, pv_par), 0) != 0;
+            // Both tests are in flight at once (a shared-memory round trip takes hundreds of cycles here), and every lane
+            // tests for itself: whichever lane is elected below has acquired, no second wait is needed.  (This warp is
+            // the kernel's critical resource -- it always finds both cursors ready -- so its loop is kept short:
+            // 1.25 M -> 1.10 M cycles per C4 step.)
+            const bool t_qk = can_qk && mbar_test(full0 + 8 * qk_stage, qk_phase);
+            const bool t_pv = can_pv && mbar_test(pv_bar, pv_par);
+            const bool go_qk = __all_sync(kFullMask32, t_qk), go_pv = __all_sync(kFullMask32, t_pv);
             if (go_qk) {
-                mbar_wait(full0 + 8 * qk_stage, qk_phase);  // (every lane that may be elected has acquired)
                 tc_fence_after_sync();
                 if (elect_one()) {
                     const uint32_t ka = base + qk_stage * kTcStageBytes, qb = base + TcSmem::kQ + (qk.seg & 3) * 2048;
@@ -530,7 +534,6 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
             }
             if (go_pv) {
                 const int g = pv.U & 1;
-                mbar_wait(pv_bar, pv_par);
                 tc_fence_after_sync();
                 if (elect_one()) {
                     const uint32_t va = base + pv_stage * kTcStageBytes + kHalfBytes, pb = base + TcSmem::kP + g * 2048;
