@@ -16,13 +16,14 @@
 // (exact for elements above 2^-14 of the row's largest), and a row of P the same way (p * v_scale, 8 significant bits
 // after the split: the precision of the bf16 P of R16); the two accumulator columns are added in fp32.
 //
-// Roles (416 threads, one CTA per SM):
+// Roles (448 threads, one CTA per SM):
 //   warps 0..7   softmax: two groups of four warps (thread = token row = TMEM lane); group g takes the super tiles
 //                U = g (mod 2) of the CTA and keeps its own running maximum, normaliser and O accumulator, so the two
 //                groups never wait for each other; their states are merged at the end of the segment (S6);
-//   warp  8      prepares Qs (one segment ahead of the softmax warps), issues every tcgen05.mma: a QK cursor that runs
-//                up to four super tiles ahead (four S buffers in TMEM) and a PV cursor that follows the P tiles;
-//   warps 9..12  producers: block table + page scales 32 tiles at a time (two batches ahead), one TMA box per 16-token
+//   warp  8      prepares Qs per portion and issues S^T = K Qs^T, blocking on one barrier (the stage has landed); eight
+//                S buffers in TMEM, so that the ring's own hand-off covers their reuse;
+//   warp  9      issues O^T += V^T Ps^T, blocking on one barrier (the group's P tile is written), and frees the stage;
+//   warps 10..13 producers: block table + page scales 32 tiles at a time (two batches ahead), one TMA box per 16-token
 //                tile of K and of V into a 6-stage ring of 32 KiB super tiles (192 KiB in flight per SM).
 // The running maximum is LAZY: a tile whose scores do not exceed it (one barrier.red.or over the group) goes straight to
 // p = 2^(s - m); only a tile that raises it (or brings a page with a larger v_scale exponent) pays the cross-warp
@@ -40,31 +41,35 @@ constexpr int kTcSoftmaxWarps = 8;
 constexpr int kTcGroupThreads = 128;
 constexpr int kTcMmaWarp = 8;
 constexpr int kTcProducerWarps = 4;
-constexpr int kTcFirstProducer = 9;
-constexpr int kTcThreads = 32 * (kTcSoftmaxWarps + 1 + kTcProducerWarps);
+constexpr int kTcPvWarp = 9;
+constexpr int kTcFirstProducer = 10;
+constexpr int kTcThreads = 32 * (kTcSoftmaxWarps + 2 + kTcProducerWarps);
 constexpr int kTcD = 128;
 constexpr int kSubTiles = 8;                       // 16-token tiles per super tile
 constexpr int kSubBytes = kTileTokens * kTcD;      // one K (or V) tile: 2 KiB
 constexpr int kHalfBytes = kSubTiles * kSubBytes;  // K (or V) part of a stage: 16 KiB
 constexpr int kTcStageBytes = 2 * kHalfBytes;
 constexpr int kTcStages = 6;                       // (5: +1.3 %, 4: +6 % on C4 in a burst)
-constexpr int kSBufs = 4;                          // S^T buffers in TMEM (16 columns each)
-constexpr int kTmemCols = 128;                     // S: columns 0..63, O of group g: 64 + 16 g
-constexpr int kOCol = 64;
+constexpr int kSBufs = 8;                          // S^T buffers in TMEM (16 columns each); >= kTcStages + 2, see the QK warp
+constexpr int kQBufs = 8;                          // Qs buffers (portion seg % 8)
+constexpr int kTmemCols = 256;                     // S: columns 0..127, O of group g: 128 + 16 g
+constexpr int kOCol = 128;
 constexpr int kPShift = 7;                         // p * f * 2^(ev - eref) * 2^7 < 256 <= E4M3's 448
 constexpr unsigned kFullMask32 = 0xffffffffu;
+static_assert(kSBufs == 8 && kQBufs == 8, "buffer parities below are written for eight");
+
 
 // shared-memory carve-up behind the 1024-aligned ring
 struct TcSmem {
     static constexpr int kP = kTcStages * kTcStageBytes;  // 2 x 2 KiB: Ps of group 0 / 1
-    static constexpr int kQ = kP + 2 * 2048;              // 4 x 2 KiB: Qs of portion seg % 4
-    static constexpr int kAcc = kQ + 4 * 2048;            // S6: [2 groups][8 heads][128] fp32
+    static constexpr int kQ = kP + 2 * 2048;              // 8 x 2 KiB: Qs of portion seg % 8
+    static constexpr int kAcc = kQ + kQBufs * 2048;            // S6: [2 groups][8 heads][128] fp32
     static constexpr int kState = kAcc + 2 * 8 * 128 * 4; // S6: m [2 groups][8], then l [2 groups][4 warps][8]
     static constexpr int kRed = kState + (16 + 64) * 4;   // lazy max: [2 groups][4 warps][8 + 1 (+ pad)] fp32
-    static constexpr int kQc = kRed + 2 * 4 * 12 * 4;     // [4 buffers][8]: scale_log2 * 2^-e of the q rows
-    static constexpr int kScales = kQc + 4 * 8 * 4;       // [stages][8 tiles] {k_scale, v_scale}
+    static constexpr int kQc = kRed + 2 * 4 * 12 * 4;     // [8 buffers][8]: scale_log2 * 2^-e of the q rows
+    static constexpr int kScales = kQc + kQBufs * 8 * 4;       // [stages][8 tiles] {k_scale, v_scale}
     static constexpr int kBars = kScales + kTcStages * kSubTiles * 8;
-    static constexpr int kNumBars = 2 * kTcStages + kSBufs + 2 + 2 + 4;  // full, empty, s_full, p_full, pv_done, q_full
+    static constexpr int kNumBars = 2 * kTcStages + kSBufs + 2 + 2 + kQBufs;  // full, empty, s_full, p_full, pv_done, q_full
     static constexpr int kPrefix = kBars + kNumBars * 8;
 };
 __host__ __device__ constexpr size_t tc_smem_bytes(int batch) { return 1024 + TcSmem::kPrefix + ((size_t)batch + 1) * 4 + 16; }
@@ -134,18 +139,6 @@ __device__ __forceinline__ void split_e4m3x2(float a, float b, uint32_t &hi, uin
     hi = f32x2_to_e4m3x2(a, b);
     const float2 back = e4m3x2_to_f32x2(hi);
     lo = f32x2_to_e4m3x2((a - back.x) * 16.f, (b - back.y) * 16.f);
-}
-// non-blocking test of an mbarrier phase (mbarrier.try_wait may suspend the thread for a system-dependent time: not
-// what a thread polling two barriers wants)
-__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    return ok != 0;
 }
 __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
 __device__ __forceinline__ float ex2f(float x)
@@ -456,19 +449,16 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
             x += cnt;
         }
     } else if (warp == kTcMmaWarp) {
-        // ------------------------------ Qs, and every tcgen05.mma ----------------------------------------------------
-        Cursor qk, pv;
+        // ------------------------------ Qs, and S^T = K Qs^T ----------------------------------------------------------
+        Cursor qk;
         qk.start(c0, c1, prefix, p.batch, p.num_kv_heads);
-        pv.start(c0, c1, prefix, p.batch, p.num_kv_heads);
-        int qk_stage = 0, pv_stage = 0, prepared = -1;
+        int qk_stage = 0, prepared = -1;
         uint32_t qk_phase = 0;
         constexpr uint32_t idesc_qk = umma_idesc_e4m3(128, 16, false, false);
-        constexpr uint32_t idesc_pv = umma_idesc_e4m3(128, 16, true, true);
         // Qs of a portion: rows g (hi) and 8 + g (lo) of a [16][128 B] K-major tile, q[g] * 2^e = hi + lo / 16 with the
-        // row's largest element scaled into [128, 256); qc[g] = scale_log2 * 2^-e.  Buffer seg % 4: the QK cursor is
-        // less than four super tiles (hence at most three portions) ahead of the PV cursor.
+        // row's largest element scaled into [128, 256); qc[g] = scale_log2 * 2^-e.  Buffer seg % 8 (see below).
         auto prepare_q = [&](const Portion &sp, int seg) {
-            const int buf = seg & 3;
+            const int buf = seg & (kQBufs - 1);
             const uint32_t qb = base + TcSmem::kQ + buf * 2048;
             const __nv_bfloat16 *q0 = p.q + ((int64_t)sp.b * p.num_q_heads + sp.kvh * p.group) * kTcD;
 #pragma unroll 1
@@ -497,58 +487,57 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
             __syncwarp();
             if (lane == 0) mbar_arrive(qfull0 + 8 * buf);
         };
-        // Two cursors, one issuing thread: QK may run up to kSBufs super tiles ahead of PV (a free S buffer, a landed
-        // stage), PV follows the finished P tiles.  Both barriers are POLLED (mbarrier.test_wait): a warp suspended in
-        // try_wait on one of them would not see the other flip.  (Measured on C4: this loop 641 us, blocking on whichever
-        // single cursor can move 760-860 us.)
-        while (!pv.done) {
-            const bool can_qk = !qk.done && qk.U < pv.U + kSBufs, can_pv = pv.U < qk.U;
-            const uint32_t pv_bar = pfull0 + 8 * (pv.U & 1), pv_par = (uint32_t)(pv.U >> 1) & 1u;
-            if (can_qk && prepared != qk.seg) {
+        // This warp issues S^T = K Qs^T only and waits on ONE barrier (the stage has landed), so it can block on it.
+        // Nothing else gates it: S buffer U % 8 is free again when QK(U + 8) can be issued, because that needs ring
+        // stage (U + 2) % 6 refilled, i.e. PV(U + 2) complete, i.e. the softmax group of U past its tile U + 2 -- and Qs
+        // buffer seg % 8 likewise (a portion is at least one super tile).
+        while (!qk.done) {
+            if (prepared != qk.seg) {
                 prepare_q(qk.sp, qk.seg);
                 prepared = qk.seg;
             }
-            // Both tests are in flight at once (a shared-memory round trip takes hundreds of cycles here), and every lane
-            // tests for itself: whichever lane is elected below has acquired, no second wait is needed.  (This warp is
-            // the kernel's critical resource -- it always finds both cursors ready -- so its loop is kept short:
-            // 1.25 M -> 1.10 M cycles per C4 step.)
-            const bool t_qk = can_qk && mbar_test(full0 + 8 * qk_stage, qk_phase);
-            const bool t_pv = can_pv && mbar_test(pv_bar, pv_par);
-            const bool go_qk = __all_sync(kFullMask32, t_qk), go_pv = __all_sync(kFullMask32, t_pv);
-            if (go_qk) {
-                tc_fence_after_sync();
-                if (elect_one()) {
-                    const uint32_t ka = base + qk_stage * kTcStageBytes, qb = base + TcSmem::kQ + (qk.seg & 3) * 2048;
-                    const uint32_t d = tmem + 16 * (qk.U & (kSBufs - 1));
+            mbar_wait(full0 + 8 * qk_stage, qk_phase);
+            tc_fence_after_sync();
+            if (elect_one()) {
+                const uint32_t ka = base + qk_stage * kTcStageBytes, qb = base + TcSmem::kQ + (qk.seg & (kQBufs - 1)) * 2048;
+                const uint32_t d = tmem + 16 * (qk.U & (kSBufs - 1));
 #pragma unroll
-                    for (int ks = 0; ks < 4; ++ks)
-                        umma_f8_ss(d, umma_smem_desc(ka + 32 * ks, 0, 1024), umma_smem_desc(qb + 32 * ks, 0, 1024), idesc_qk, ks > 0);
-                    umma_commit(sfull0 + 8 * (qk.U & (kSBufs - 1)));
-                }
-                __syncwarp();
-                if (++qk_stage == kTcStages) {
-                    qk_stage = 0;
-                    qk_phase ^= 1u;
-                }
-                qk.next(prefix, p.batch, p.num_kv_heads);
+                for (int ks = 0; ks < 4; ++ks)
+                    umma_f8_ss(d, umma_smem_desc(ka + 32 * ks, 0, 1024), umma_smem_desc(qb + 32 * ks, 0, 1024), idesc_qk, ks > 0);
+                umma_commit(sfull0 + 8 * (qk.U & (kSBufs - 1)));
             }
-            if (go_pv) {
-                const int g = pv.U & 1;
-                tc_fence_after_sync();
-                if (elect_one()) {
-                    const uint32_t va = base + pv_stage * kTcStageBytes + kHalfBytes, pb = base + TcSmem::kP + g * 2048;
-                    const uint32_t d = tmem + kOCol + 16 * g;
+            __syncwarp();
+            if (++qk_stage == kTcStages) {
+                qk_stage = 0;
+                qk_phase ^= 1u;
+            }
+            qk.next(prefix, p.batch, p.num_kv_heads);
+        }
+    } else if (warp == kTcPvWarp) {
+        // ------------------------------ O^T += V^T Ps^T: one barrier (the group's P tile is written), blocking ----------
+        // (One warp issuing both contractions was the kernel's critical resource: it polled two barriers and always
+        // found both ready -- 1 413 cycles per tile; the two issuers never wait for each other.)
+        Cursor pv;
+        pv.start(c0, c1, prefix, p.batch, p.num_kv_heads);
+        int pv_stage = 0;
+        constexpr uint32_t idesc_pv = umma_idesc_e4m3(128, 16, true, true);
+        while (!pv.done) {
+            const int g = pv.U & 1;
+            mbar_wait(pfull0 + 8 * g, (uint32_t)(pv.U >> 1) & 1u);
+            tc_fence_after_sync();
+            if (elect_one()) {
+                const uint32_t va = base + pv_stage * kTcStageBytes + kHalfBytes, pb = base + TcSmem::kP + g * 2048;
+                const uint32_t d = tmem + kOCol + 16 * g;
 #pragma unroll
-                    for (int ks = 0; ks < 4; ++ks)
-                        umma_f8_ss(d, umma_smem_desc(va + 4096 * ks, 0, 1024), umma_smem_desc_mn_plain(pb + 512 * ks, 128), idesc_pv,
-                                   (pv.ul >= 2 || ks > 0) ? 1u : 0u);
-                    umma_commit(empty0 + 8 * pv_stage);
-                    umma_commit(pvdone0 + 8 * g);
-                }
-                __syncwarp();
-                if (++pv_stage == kTcStages) pv_stage = 0;
-                pv.next(prefix, p.batch, p.num_kv_heads);
+                for (int ks = 0; ks < 4; ++ks)
+                    umma_f8_ss(d, umma_smem_desc(va + 4096 * ks, 0, 1024), umma_smem_desc_mn_plain(pb + 512 * ks, 128), idesc_pv,
+                               (pv.ul >= 2 || ks > 0) ? 1u : 0u);
+                umma_commit(empty0 + 8 * pv_stage);  // (QK of this stage completed before its softmax started)
+                umma_commit(pvdone0 + 8 * g);
             }
+            __syncwarp();
+            if (++pv_stage == kTcStages) pv_stage = 0;
+            pv.next(prefix, p.batch, p.num_kv_heads);
         }
     } else {
         // ------------------------------ softmax warps: S4, P, S6 ----------------------------------------------------
@@ -564,9 +553,9 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
         int stage = 0;
         while (!cur.done) {
             const Portion sp = cur.sp;
-            const int seg = cur.seg, buf = seg & 3;
+            const int seg = cur.seg, buf = seg & (kQBufs - 1);
             const int64_t x0 = cur.x;
-            mbar_wait(qfull0 + 8 * buf, (uint32_t)(seg >> 2) & 1u);
+            mbar_wait(qfull0 + 8 * buf, (uint32_t)(seg >> 3) & 1u);
             float c[kMaxGroup];
 #pragma unroll
             for (int g8 = 0; g8 < kMaxGroup; ++g8) c[g8] = qc[buf * 8 + g8];
@@ -586,7 +575,7 @@ decode_fp8_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_cons
                     int live = cur.sub_tiles() << kTileShift;
                     live = live < seq_len - tok0 ? live : seq_len - tok0;
                     const int sb = U & (kSBufs - 1);
-                    mbar_wait(sfull0 + 8 * sb, (uint32_t)(U >> 2) & 1u);
+                    mbar_wait(sfull0 + 8 * sb, (uint32_t)(U >> 3) & 1u);
                     tc_fence_after_sync();
                     uint32_t r[16];
                     tmem_ld16(tmem + lane_off + 16 * sb, r);
