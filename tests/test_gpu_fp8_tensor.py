@@ -247,3 +247,17 @@ print("RESULT", h.hexdigest())
         assert "RESULT" in r.stdout, (stale, r.stdout[-500:], r.stderr[-1500:])
         digests.append(r.stdout.split("RESULT")[1].strip())
     assert digests[0] == digests[1]
+
+
+@pytest.mark.parametrize("batch,hkv,hi", [(1000, 8, 40), (517, 2, 130), (64, 8, 16)])
+def test_tensor_many_one_tile_portions(oracle, batch, hkv, hi):
+    """Sequences of one to a few tiles: a CTA walks dozens of portions of a single super tile each, so the eight Qs buffers
+    and the eight S buffers cycle as fast as they can (their reuse is covered by the ring's hand-off, not by a barrier)."""
+    rng = np.random.default_rng(8800 + batch)
+    lens = [int(rng.integers(1, hi + 1)) for _ in range(batch)]
+    f = fp8_batch(lens, 4 * hkv, hkv, 16, seed=8800 + batch)
+    out, lse = check_tc(oracle, f, f"tensor tiny sequences {batch}")
+    again, again_lse = run_tc(f)
+    assert torch.equal(bits(out), bits(again)) and torch.equal(lse, again_lse)
+    for grid in (37, 148):
+        check_tc(oracle, f, f"tensor tiny sequences {batch} grid {grid}", grid=grid)
