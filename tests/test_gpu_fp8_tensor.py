@@ -261,3 +261,37 @@ def test_tensor_many_one_tile_portions(oracle, batch, hkv, hi):
     assert torch.equal(bits(out), bits(again)) and torch.equal(lse, again_lse)
     for grid in (37, 148):
         check_tc(oracle, f, f"tensor tiny sequences {batch} grid {grid}", grid=grid)
+
+
+@pytest.mark.parametrize("G,hkv", [(8, 8), (4, 2), (3, 5)])
+def test_tensor_hnd_32_token_pages(oracle, G, hkv):
+    """HND pools with 32-token pages (two tiles per page, config 4's layout): grids that cut the segments at odd tiles,
+    ragged ends inside a page's first and second tile, page permutation, reruns."""
+    lens = [20000, 37, 0, 50001, 8191, 16, 17, 300, 48, 49, 4097]
+    f = W.to_hnd(fp8_batch(lens, G * hkv, hkv, 32, seed=880 + G))
+    base, base_lse = check_tc(oracle, f, f"tensor HND ps32 G{G} hkv{hkv}")
+    again, again_lse = run_tc(f)
+    assert torch.equal(bits(base), bits(again)) and torch.equal(base_lse, again_lse)
+    po, pl = run_tc(W.permute_pages_fp8(f, seed=11))
+    assert torch.equal(bits(base), bits(po)) and torch.equal(base_lse, pl)
+    for grid in (1, 3, 7, 61, 147, 148, 149, 296, 601):
+        check_tc(oracle, f, f"tensor HND ps32 grid {grid}", grid=grid)
+
+
+def test_tensor_c4_shape_sampled(oracle):
+    """Config 4's geometry (32q / 8kv, 32-token pages, HND), 4 x 131072 tokens: two whole sequences against the oracle."""
+    bf = W.make_batch([131072, 131072, 100000, 65537], 32, 8, 128, 32, seed=890, device=DEV, poison_unused=True)
+    f = W.to_hnd(W.quantize_batch_fp8(bf))
+    del bf
+    out, lse = run_tc(f)
+    ps = f.page_size
+    for b in (1, 3):
+        n = W.pages_needed(int(f.seq_lens[b]), ps)
+        ids = f.block_table[b, :n].long()
+        sub = W.Fp8DecodeBatch(q=f.q[b:b + 1].cpu(), k_pages=f.k_pages[ids].cpu(), v_pages=f.v_pages[ids].cpu(),
+                               k_scale=f.k_scale[ids].cpu(), v_scale=f.v_scale[ids].cpu(),
+                               block_table=torch.arange(n, dtype=torch.int32).view(1, n),
+                               seq_lens=f.seq_lens[b:b + 1].cpu(), softmax_scale=f.softmax_scale, kv_layout="HND")
+        ref, ref_lse = oracle.decode_attn_fp8(sub.q, sub.k_pages, sub.v_pages, sub.k_scale, sub.v_scale, sub.block_table,
+                                              sub.seq_lens, sub.softmax_scale, kv_layout="HND")
+        gate(out[b:b + 1].double().cpu().numpy(), ref, lse[b:b + 1].double().cpu().numpy(), ref_lse, f"tensor c4 shape seq {b}")
