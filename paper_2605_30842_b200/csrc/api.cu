@@ -430,6 +430,10 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
                             int64_t num_pages_host = 0)
 {
     if (sink_tokens < 0) return COMEM_ERR_INVALID_ARG;
+    // unknown launch-flag bits: rejected on the host before anything else is looked at
+    if (opts && (opts->flags & ~(COMEM_LAUNCH_KV_PREFIX_IMMUTABLE | COMEM_LAUNCH_SPLIT_COMBINE | COMEM_LAUNCH_Q_STABLE |
+                                 COMEM_LAUNCH_FP8_TENSOR)))
+        return COMEM_ERR_INVALID_ARG;
     if (kv_fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return COMEM_ERR_INVALID_ARG;
     if (kv_layout != COMEM_KV_LAYOUT_NHD && !(kv_fp8 && kv_layout == COMEM_KV_LAYOUT_HND)) return COMEM_ERR_INVALID_ARG;
     if ((phases & ~(COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE)) != 0 || phases == 0) return COMEM_ERR_INVALID_ARG;
@@ -477,9 +481,7 @@ static int decode_attn_impl(const void *q, const void *k_pages, const void *v_pa
     p.part_state = reinterpret_cast<float *>(static_cast<char *>(workspace) + wl.part_state);
     p.part_cap = kMaxGridCtas;
     p.seg_counters = reinterpret_cast<int *>(static_cast<char *>(workspace) + wl.counters);
-    const int flags = opts ? opts->flags : 0;
-    if (flags & ~(COMEM_LAUNCH_KV_PREFIX_IMMUTABLE | COMEM_LAUNCH_SPLIT_COMBINE | COMEM_LAUNCH_Q_STABLE | COMEM_LAUNCH_FP8_TENSOR))
-        return COMEM_ERR_INVALID_ARG;
+    const int flags = opts ? opts->flags : 0;  // (validated at the top)
     // COMEM_LAUNCH_FP8_TENSOR: the tcgen05 split kernel of decode_fp8_tc.cu (FP8 cache, D = 128, no window, batch <= 1024)
     const bool fp8_tensor = (flags & COMEM_LAUNCH_FP8_TENSOR) != 0;
     if (fp8_tensor && (!kv_fp8 || phases != (COMEM_PHASE_SPLIT | COMEM_PHASE_COMBINE))) return COMEM_ERR_INVALID_ARG;

@@ -171,7 +171,7 @@ def test_round2_entry_points_validate_arguments_on_the_host(lib):
     lib.comem_decode_attn_async.restype = C.c_int
     st = lib.comem_decode_attn_async(p, p, p, p, p, 8, 2, 128, 16, C.c_float(0.1), p, 1, 4, 8, None, p,
                                      comem.comem_decode_attn_workspace_bytes(1, 8, 2, 128, 16, 4), None, C.byref(opts))
-    assert st in (comem.COMEM_ERR_INVALID_ARG, comem.COMEM_ERR_WORKSPACE)
+    assert st == comem.COMEM_ERR_INVALID_ARG     # whatever the alignment of `buf` happens to be
     # the Algorithm-1 step scheduler: null model / event, bad token counts
     ev = comem.KstepEvent(1, 0, 0, 1, 0, 0)
     m = comem.KstepModel()
