@@ -295,3 +295,40 @@ def test_tensor_c4_shape_sampled(oracle):
         ref, ref_lse = oracle.decode_attn_fp8(sub.q, sub.k_pages, sub.v_pages, sub.k_scale, sub.v_scale, sub.block_table,
                                               sub.seq_lens, sub.softmax_scale, kv_layout="HND")
         gate(out[b:b + 1].double().cpu().numpy(), ref, lse[b:b + 1].double().cpu().numpy(), ref_lse, f"tensor c4 shape seq {b}")
+
+
+def test_tensor_against_the_default_kernel_over_random_shapes():
+    """Sixty seeded shapes (hundreds of one-tile sequences, ragged mid-size batches, one long sequence among short ones;
+    group 1..8, 1..8 kv heads, both page sizes and pool layouts, grids 1..1000): the tensor kernel's output is finite,
+    the same on a second run, and within twice the attention tolerances of the default FP8 kernel's on the same bytes."""
+    rng = np.random.default_rng(2024)
+
+    def run(f, flags, grid):
+        out = torch.full_like(f.q, float("nan"))
+        ws = comem.alloc_workspace(f.q, f.k_pages, f.block_table, kv_layout=f.kv_layout)
+        comem.comem_decode_attn_fp8_async(f.q, f.k_pages, f.v_pages, f.k_scale, f.v_scale, f.block_table, f.seq_lens,
+                                          f.softmax_scale, out, ws, 0, 0, kv_layout=f.kv_layout, flags=flags, grid_ctas=grid)
+        torch.cuda.synchronize()
+        return out.double()
+
+    for case in range(60):
+        G, hkv, ps = int(rng.integers(1, 9)), int(rng.integers(1, 9)), int(rng.choice([16, 32]))
+        kind = case % 4
+        if kind == 0:
+            lens = [int(rng.integers(0, 40)) for _ in range(int(rng.integers(1, 900)))]
+        elif kind == 1:
+            lens = [int(rng.integers(1, 3000)) for _ in range(int(rng.integers(1, 40)))]
+        elif kind == 2:
+            lens = [int(rng.integers(100, 140)) for _ in range(int(rng.integers(1, 300)))]
+        else:
+            lens = [int(rng.integers(20000, 70000))] + [int(rng.integers(0, 300)) for _ in range(int(rng.integers(0, 20)))]
+        grid = int(rng.choice([0, 1, 2, 5, 37, 148, 149, 300, 1000])) or None
+        f = fp8_batch(lens, G * hkv, hkv, ps, seed=5000 + case)
+        if rng.random() < 0.5:
+            f = W.to_hnd(f)
+        what = (case, G, hkv, ps, f.kv_layout, len(lens), grid)
+        a, a2, b = run(f, TENSOR, grid), run(f, TENSOR, grid), run(f, 0, grid)
+        assert torch.isfinite(a).all(), what
+        assert torch.equal(a, a2), what
+        assert (a - b).abs().max().item() <= 2 * 2e-2, what
+        assert ((a - b).norm() / b.norm().clamp_min(1e-30)).item() <= 2 * 5e-3, what
